@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of libtina: fused PFB at P=1024, M=16 (BASELINE.json config 4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4|c5|c5bf16|c2|c3|c1]
+
+One "step" = one pass of the whole hot path (subfilter stage + DFT contraction, one
+tina_pfb_batched call) over one batch of synthetic input shaped like config 4:
+8 streams x 8192 spectra x 1024 channels, 16 taps (537.9 MB in, 536.9 MB out -- both larger
+than the 126 MB L2, so consecutive steps cannot be served from cache; no explicit flush).
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the definitions.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import tina_inputs as ti  # noqa: E402
+
+METRIC = "pfb_input_gsamples_per_s"
+UNIT = "GSamples/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        d["_source"] = "measured"
+        return d
+    d = dict(FALLBACK_PEAKS)
+    d["_source"] = "fallback"
+    return d
+
+
+def workload_spec(name: str):
+    """(kind, dict) for each BASELINE.json config; c4 is the headline."""
+    if name == "c4":
+        return dict(call="pfb", P=1024, M=16, S=8, F=8192, real=False, prec=0)
+    if name == "c5":
+        return dict(call="pfb", P=4096, M=8, S=1, F=32761, real=True, prec=0)
+    if name == "c5bf16":
+        return dict(call="pfb", P=4096, M=8, S=1, F=32761, real=True, prec=1)
+    if name == "c1":
+        return dict(call="pfb", P=16, M=4, S=1, F=4096, real=False, prec=0)
+    if name == "c2":
+        return dict(call="dft", B=65536, N=256)
+    if name == "c3":
+        return dict(call="fir", C=64, L=1 << 20, K=64)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def useful_flops_and_bytes(w):
+    """Algorithmic flops (DFT contraction, the dominant kernel's tensor work) and HBM bytes
+    per step -- SURVEY.md section 8(d) / DESIGN.md "Algorithmic work"."""
+    if w["call"] == "pfb":
+        P, M, S, F = w["P"], w["M"], w["S"], w["F"]
+        frames = S * F
+        if w["real"]:
+            flops = frames * (2.0 * P * P + 4.0 * P)
+            byts = S * (F + M - 1) * P * 4 + frames * (P // 2 + 1) * 8 + P * M * 4
+        else:
+            flops = frames * 8.0 * P * P
+            byts = S * (F + M - 1) * P * 8 + frames * P * 8 + P * M * 4
+        samples = S * (F + M - 1) * P
+        return flops, float(byts), samples, frames
+    if w["call"] == "dft":
+        B, N = w["B"], w["N"]
+        return B * 8.0 * N * N, B * N * 16.0, B * N, B
+    C, L, K = w["C"], w["L"], w["K"]
+    return C * (L - K + 1) * 2.0 * K, C * L * 4.0 + C * (L - K + 1) * 4.0, C * L, C
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append((time.time(), ln.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.1] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [c.strip() for c in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax = float(f[1])
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_inputs(w, seed_offset: int = 0):
+    """Seeded synthetic host arrays for the workload (tina_inputs recipes)."""
+    if w["call"] == "pfb":
+        if (w["P"], w["M"], w["real"]) == (1024, 16, False):
+            case = ti.pfb_case(1024, 16, w["F"], streams=w["S"], seed=ti.SEED_BASE + 4 + 100 * seed_offset,
+                               tones=3, name="c4")
+        else:
+            idx = 5 if w["real"] else 1
+            case = ti.pfb_case(w["P"], w["M"], w["F"], real=w["real"], streams=w["S"],
+                               seed=ti.SEED_BASE + idx + 100 * seed_offset)
+        return case
+    if w["call"] == "dft":
+        return ti.config2(w["B"], w["N"])
+    return ti.config3(w["C"], w["L"], w["K"])
+
+
+def cpu_oracle_rate(w, budget_s: float = 15.0):
+    """Time the float64 oracle, as it stands, on a bounded sample of the workload.
+    Returns (GSamples/s, cores, sample description, seconds)."""
+    import oracle
+    oracle.build()
+    cores = oracle.num_threads()
+    if w["call"] == "pfb":
+        P, M = w["P"], w["M"]
+        probe = max(cores, 8)
+        case = ti.pfb_case(P, M, probe, real=w["real"], seed=1)
+        t0 = time.perf_counter(); oracle.pfb(case.x[0], P, M, case.window); dt = time.perf_counter() - t0
+        n = int(min(max(probe, budget_s / max(dt / probe, 1e-9)), 4096))
+        n = max(cores, n - n % cores)
+        case = ti.pfb_case(P, M, n, real=w["real"], seed=2)
+        t0 = time.perf_counter(); oracle.pfb(case.x[0], P, M, case.window); dt = time.perf_counter() - t0
+        return n * P / dt / 1e9, cores, f"{n} frames of one stream (P={P}, M={M}), float64 direct sums", dt
+    if w["call"] == "dft":
+        N = w["N"]; n = 4096
+        x = ti.config2(n, N)
+        t0 = time.perf_counter(); oracle.dft(x); dt = time.perf_counter() - t0
+        return n * N / dt / 1e9, cores, f"{n} signals of N={N}", dt
+    C, L, K = 8, 1 << 20, w["K"]
+    x, taps, _ = ti.config3(C, L, K)
+    t0 = time.perf_counter(); oracle.fir(x, taps); dt = time.perf_counter() - t0
+    return C * L / dt / 1e9, cores, f"{C} channels of L={L}, K={K}", dt
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle (oracle/, as it stands) on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    flops, byts, samples, frames = useful_flops_and_bytes(w)
+    rates, secs = [], []
+    budget = max(2.0, min(15.0, 120.0 / max(args.steps + args.warmup, 1)))
+    for i in range(args.warmup + args.steps):
+        r, cores, sample, dt = cpu_oracle_rate(w, budget_s=budget)
+        if i >= args.warmup:
+            rates.append(r); secs.append(dt)
+    value = float(np.mean(rates))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": args.workload, **{k: v for k, v in w.items() if k != "call"},
+                   "note": "each step = a bounded sample of the workload run through the float64 oracle"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+    import paper_2408_16551_b200 as tina
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- libtina has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    tina.lib()
+
+    flops, byts, samples, frames = useful_flops_and_bytes(w)
+    peaks = load_peaks()
+    stream = torch.cuda.current_stream()
+
+    # ---- inputs resident in HBM (each rank its own seeded batch: frames are independent, so
+    #      ranks shard the units with no data-path collective -> weak scaling) --------------
+    data = make_inputs(w, seed_offset=rank)
+    if w["call"] == "pfb":
+        x_host = torch.from_numpy(data.x)
+        w_host = torch.from_numpy(data.window)
+        xd, wd = x_host.cuda(), w_host.cuda()
+        NK = w["P"] // 2 + 1 if w["real"] else w["P"]
+        out = torch.empty((w["S"], w["F"], NK), dtype=torch.complex64, device="cuda")
+        step = lambda: tina.pfb(xd, w["P"], w["M"], wd, prec=w["prec"], out=out)
+    elif w["call"] == "dft":
+        xd = torch.from_numpy(data).cuda()
+        out = torch.empty_like(xd); back = torch.empty_like(xd)
+        def step():
+            tina.dft(xd, out=out); tina.dft(out, inverse=True, out=back)
+        flops *= 2; byts *= 2
+    else:
+        xh, taps, _ = data
+        xd, td = torch.from_numpy(xh).cuda(), torch.from_numpy(taps).cuda()
+        out = torch.empty((w["C"], w["L"] - w["K"] + 1), dtype=torch.float32, device="cuda")
+        step = lambda: tina.fir(xd, td, out=out)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    launches0 = tina.launch_count()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t_wall0 = time.time()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for a, b in evs:
+        a.record(stream); step(); b.record(stream)
+    e1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    launches = tina.launch_count() - launches0
+    total_ms = e0.elapsed_time(e1)
+    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * samples / (ms_per_step * 1e-3) / 1e9
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+
+    # ---- e2e: host buffers through the C ABI (H2D + kernel + D2H inside the timed region) --
+    e2e = None
+    if w["call"] == "pfb":
+        xp, wp = x_host.pin_memory(), w_host.pin_memory()
+        outp = torch.empty((w["S"], w["F"], NK), dtype=torch.complex64, pin_memory=True)
+        n_e2e = max(2, min(args.steps, 5))
+        tina.pfb_host(xp, w["P"], w["M"], wp, prec=w["prec"], out=outp)      # warm-up (allocates staging)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            tina.pfb_host(xp, w["P"], w["M"], wp, prec=w["prec"], out=outp)  # synchronous call
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * samples / dt / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": int(xp.numel() * xp.element_size() + wp.numel() * 4),
+               "d2h_bytes_per_step": int(outp.numel() * 8), "ms_per_step": dt * 1e3, "steps": n_e2e}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    tensor_bound = w["call"] in ("pfb", "dft") and tina.last_path() == 2
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as fh:
+            traffic = json.load(fh).get(args.workload)
+    sustained = total_ms > 1500.0
+    if tensor_bound:
+        peak = peaks["bf16_tflops_sustained" if sustained else "bf16_tflops"]
+        achieved = flops / (kern_ms * 1e-3) / 1e12
+        passes = 1 if w.get("prec", 0) == 1 else 3
+        roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": traffic, "peak_source": f"{peaks['_source']} bf16 {'sustained' if sustained else 'burst'}",
+                "issued_passes": passes, "issued_frac": passes * achieved / peak,
+                "hbm_gbs_achieved": byts / (kern_ms * 1e-3) / 1e9, "hbm_frac": byts / (kern_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    else:
+        achieved = byts / (kern_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": f"{peaks['_source']} copy"}
+    roof["kernel_ms"] = kern_ms
+
+    cpu_val, cores, sample, _ = cpu_oracle_rate(w) if world == 1 else (None, None, None, None)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16x3->f32" if (tensor_bound and w.get("prec", 0) == 0) else ("bf16" if tensor_bound else "f32"),
+        "data": "synthetic", "spectra_per_s": world * frames / (ms_per_step * 1e-3),
+        "config": {"workload": args.workload, **{k: v for k, v in w.items() if k != "call"},
+                   "l2": "inputs and outputs each exceed the 126 MB L2; no explicit flush",
+                   "path": {0: "none", 1: "cuda-core", 2: "tcgen05"}[tina.last_path()],
+                   "parallelism": f"frame-sharded replicas x{world}, no collective"},
+        "roofline": roof, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+    }
+    if cpu_val is not None:
+        line["cpu_baseline"] = {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4")
+    args = ap.parse_args()
+    w = workload_spec(args.workload)
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

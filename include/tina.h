@@ -1,0 +1,126 @@
+/*
+ * tina.h -- C ABI of libtina: the FIR / DFT / IDFT / Polyphase-Filter-Bank hot path of
+ * arxiv 2408.16551 ("TINA"), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * All data pointers are DEVICE pointers owned by the caller (e.g. allocated by PyTorch)
+ * unless a function name ends in `_host`.  Every call validates its arguments on the
+ * host, enqueues its kernels on `stream` (a cudaStream_t passed as void*, NULL = the
+ * legacy default stream) and returns WITHOUT synchronising.  The caller must keep
+ * x / taps / window / out alive and unmodified until the stream has passed the enqueued
+ * work.  The library owns only its plan cache (twiddle matrices + TMA tensor maps, created
+ * lazily on first use of a (size, kind, direction, precision) tuple -- that first call
+ * allocates device memory and synchronises once), released by tina_clear_plan_cache().
+ *
+ * Errors: integer status only; nothing is written to the outputs on error; no exceptions,
+ * no exit(), no CPU fallback, no other backend.  tina_last_error() gives thread-local text.
+ * Thread-safety: the plan cache is behind a mutex; everything else is re-entrant.
+ *
+ * Notation (0-based everywhere; PAPER.md = /root/reference/PAPER.md):
+ *   P  channels / polyphase branches        M  taps per branch
+ *   NB = floor(n_samples / P) input blocks   F = NB - M + 1 output frames ("spectra")
+ */
+#ifndef TINA_H_
+#define TINA_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TINA_OK                = 0,
+    TINA_ERR_NULL_POINTER  = 1,
+    TINA_ERR_BAD_SHAPE     = 2,  /* sizes < 1, L < M, F < 1, in-place call, odd P for the real kind */
+    TINA_ERR_UNSUPPORTED   = 3,  /* size outside the supported set stated per function              */
+    TINA_ERR_ALIGNMENT     = 4,  /* a base pointer is not 16-byte aligned                            */
+    TINA_ERR_CUDA          = 5,  /* a CUDA runtime / driver call failed; see tina_last_error()       */
+    TINA_ERR_OUT_OF_MEMORY = 6
+} tina_status;
+
+typedef enum { TINA_COMPLEX = 0, TINA_REAL = 1 } tina_kind;       /* "real_or_complex" input   */
+
+typedef enum {
+    TINA_PREC_FP32 = 0,   /* fp32-accurate: error-compensated bf16x3 tensor-core contraction
+                             (rel. L2 per frame <= 1e-5 against a float64 reference)           */
+    TINA_PREC_BF16 = 1    /* single-pass bf16 operands, fp32 accumulate (<= 2e-2)              */
+} tina_precision;
+
+/* ---------------------------------------------------------------------------------------
+ * FIR filter, Eq. (15), valid mode:
+ *     y[c][j] = sum_{k=0}^{M-1} taps[k] * x[c][j + M-1 - k],   j in [0, L-M+1)
+ * i.e. a true convolution y(i) = sum_k a(k) x(i-k) evaluated for every i whose whole
+ * history exists; the impulse response equals the taps in order.
+ *   x    [C][L]       float32, row-major (device)
+ *   taps [M]          float32, shared by all C channels (device)
+ *   y    [C][L-M+1]   float32, row-major (device), must not overlap x
+ * Supported: C >= 1, 1 <= M <= 4096, L >= M.  Errors: NULL_POINTER, BAD_SHAPE,
+ * UNSUPPORTED (M > 4096), ALIGNMENT (x, y not 16-byte aligned), CUDA.                      */
+tina_status tina_fir(const float* x, const float* taps, float* y,
+                     int C, long long L, int M, void* stream);
+
+/* ---------------------------------------------------------------------------------------
+ * DFT / inverse DFT as a dense contraction against the Fourier matrix,
+ * Eq. (12) / Eq. (14):
+ *     out[b][k] = s * sum_{n=0}^{N-1} x[b][n] * exp(-+ 2 pi i n k / N)
+ * forward (inverse == 0): sign -, s = 1;  inverse (inverse != 0): sign +, s = 1/N.
+ *   x, out [B][N] complex64, interleaved (re, im) float32 (device); in-place (x == out)
+ *   is NOT supported -> BAD_SHAPE.
+ * Supported: B >= 1, 2 <= N <= 8192.  N % 32 == 0 runs on the tcgen05 tensor-core path,
+ * any other N on the generic CUDA-core path (fp32 regardless of `prec`).                  */
+tina_status tina_dft(const void* x, void* out, long long B, int N, int inverse,
+                     tina_precision prec, void* stream);
+
+/* ---------------------------------------------------------------------------------------
+ * Polyphase filter bank: subfilter stage Eq. (20) followed by a P-point DFT
+ * across the branches, fused in one kernel (the subfiltered signals never
+ * touch HBM):
+ *     y[f][p] = sum_{m=0}^{M-1} window[m P + p] * x[(f + M-1 - m) P + p]
+ *     out[f][k] = sum_{p=0}^{P-1} y[f][p] * exp(-2 pi i p k / P)
+ * with x_p(n') = x[n' P + p], h_p(m) = window[m P + p], frame f <-> n' = f + M-1.
+ *   x       n_samples complex64 (kind = COMPLEX) or float32 (kind = REAL) (device);
+ *           the trailing n_samples mod P samples are ignored
+ *   window  [P*M] float32 prototype filter (device)
+ *   out     [F][P] complex64 (COMPLEX, k in [0,P)) or [F][P/2+1] complex64 (REAL, half
+ *           spectrum k in [0,P/2]) (device), F = tina_pfb_num_frames(n_samples, P, M)
+ * Supported: 2 <= P <= 8192 (even for REAL), 1 <= M <= 64, F >= 1.  COMPLEX with
+ * P % 32 == 0 and REAL with P % 64 == 0 run on the tensor-core path; other P on the
+ * generic CUDA-core path (fp32 regardless of `prec`).
+ * tina_pfb_batched: S independent streams in one launch, x [S][n_samples],
+ * out [S][F][...]; n_samples must then keep every stream 16-byte aligned
+ * (n_samples even for COMPLEX, % 4 == 0 for REAL) else ALIGNMENT.                          */
+tina_status tina_pfb(const void* x, long long n_samples, int P, int M, const float* window,
+                     tina_kind kind, tina_precision prec, void* out, void* stream);
+tina_status tina_pfb_batched(const void* x, int S, long long n_samples, int P, int M,
+                             const float* window, tina_kind kind, tina_precision prec,
+                             void* out, void* stream);
+
+/* Subfilter stage only (Eq. (20); Fig. 3 left column):
+ *   y [S][F][P] complex64 (COMPLEX) or float32 (REAL).  Same argument rules as above.      */
+tina_status tina_pfb_fir_batched(const void* x, int S, long long n_samples, int P, int M,
+                                 const float* window, tina_kind kind, void* y, void* stream);
+
+/* Host-buffer convenience wrappers (the end-to-end path timed as `e2e` by bench.py):
+ * x_host / window_host / out_host are HOST pointers (pinned memory recommended); the call
+ * allocates device staging buffers on first use (cached, grown as needed), copies in on
+ * `stream`, runs the device path, copies the result back and SYNCHRONISES the stream.      */
+tina_status tina_pfb_batched_host(const void* x_host, int S, long long n_samples, int P, int M,
+                                  const float* window_host, tina_kind kind, tina_precision prec,
+                                  void* out_host, void* stream);
+
+/* F = floor(n_samples / P) - M + 1; <= 0 means the input is too short.                     */
+long long   tina_pfb_num_frames(long long n_samples, int P, int M);
+
+const char* tina_status_string(tina_status s);   /* static storage                          */
+const char* tina_last_error(void);               /* thread-local detail text, "" if none    */
+tina_status tina_clear_plan_cache(void);         /* frees cached twiddles / staging buffers */
+int         tina_version(void);                  /* major*10000 + minor*100 + patch         */
+
+/* Introspection used by the tests and bench.py: number of kernel launches the library has
+ * enqueued since process start (monotonic), and which path the last device call used
+ * (0 = none yet, 1 = generic CUDA-core, 2 = tcgen05 tensor-core).                           */
+long long   tina_launch_count(void);
+int         tina_last_path(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TINA_H_ */

@@ -1,0 +1,198 @@
+"""ctypes binding of libtina.so -- argument marshalling only; every step runs in the CUDA kernels.
+
+Functions mirror include/tina.h: fir <-> tina_fir, dft <-> tina_dft, pfb <-> tina_pfb_batched,
+pfb_fir <-> tina_pfb_fir_batched, pfb_host <-> tina_pfb_batched_host.
+The library is loaded lazily; a missing or unloadable libtina.so raises (no fallback of any kind).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+COMPLEX, REAL = 0, 1
+PREC_FP32, PREC_BF16 = 0, 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libtina.so")
+_lib = None
+
+EXPORTS = ["tina_fir", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
+           "tina_pfb_batched_host", "tina_pfb_num_frames", "tina_status_string", "tina_last_error",
+           "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path"]
+
+
+class TinaError(RuntimeError):
+    def __init__(self, status: int, name: str, detail: str):
+        super().__init__(f"{name} ({status}): {detail}")
+        self.status, self.name, self.detail = status, name, detail
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2408_16551_b200.build` "
+                          "(or __graft_entry__.build()); there is no fallback path")
+    L = ctypes.CDLL(_LIB_PATH)
+    ll, vp, ci = ctypes.c_longlong, ctypes.c_void_p, ctypes.c_int
+    L.tina_fir.argtypes = [vp, vp, vp, ci, ll, ci, vp]
+    L.tina_dft.argtypes = [vp, vp, ll, ci, ci, ci, vp]
+    L.tina_pfb.argtypes = [vp, ll, ci, ci, vp, ci, ci, vp, vp]
+    L.tina_pfb_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, ci, vp, vp]
+    L.tina_pfb_fir_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, vp, vp]
+    L.tina_pfb_batched_host.argtypes = [vp, ci, ll, ci, ci, vp, ci, ci, vp, vp]
+    for f in ("tina_fir", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
+              "tina_pfb_batched_host", "tina_clear_plan_cache", "tina_version", "tina_last_path"):
+        getattr(L, f).restype = ci
+    L.tina_pfb_num_frames.argtypes = [ll, ci, ci]
+    L.tina_pfb_num_frames.restype = ll
+    L.tina_launch_count.restype = ll
+    L.tina_status_string.argtypes = [ci]
+    L.tina_status_string.restype = ctypes.c_char_p
+    L.tina_last_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _check(st: int) -> None:
+    if st != 0:
+        L = lib()
+        raise TinaError(st, L.tina_status_string(st).decode(), L.tina_last_error().decode())
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev(t, dtype, what):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{what}: expected a CUDA tensor")
+    if t.dtype != dtype:
+        raise TypeError(f"{what}: expected dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError(f"{what}: must be contiguous")
+    return t
+
+
+def pfb_num_frames(n_samples: int, P: int, M: int) -> int:
+    return int(lib().tina_pfb_num_frames(n_samples, P, M))
+
+
+def launch_count() -> int:
+    return int(lib().tina_launch_count())
+
+
+def last_path() -> int:
+    return int(lib().tina_last_path())
+
+
+def clear_plan_cache() -> None:
+    _check(lib().tina_clear_plan_cache())
+
+
+def version() -> int:
+    return int(lib().tina_version())
+
+
+def fir(x, taps, out=None, stream=None):
+    """tina_fir: x [C, L] float32 CUDA, taps [M] float32 CUDA -> y [C, L-M+1] float32."""
+    import torch
+    x = _dev(x, torch.float32, "x")
+    taps = _dev(taps, torch.float32, "taps")
+    if x.dim() != 2 or taps.dim() != 1:
+        raise ValueError("x must be [C, L], taps [M]")
+    C, L = x.shape
+    M = taps.shape[0]
+    if out is None:
+        out = torch.empty((C, max(L - M + 1, 0)), dtype=torch.float32, device=x.device)
+    _dev(out, torch.float32, "out")
+    _check(lib().tina_fir(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream)))
+    return out
+
+
+def dft(x, inverse: bool = False, prec: int = PREC_FP32, out=None, stream=None):
+    """tina_dft: x [B, N] complex64 CUDA -> [B, N] complex64."""
+    import torch
+    x = _dev(x, torch.complex64, "x")
+    if x.dim() != 2:
+        raise ValueError("x must be [B, N]")
+    B, N = x.shape
+    if out is None:
+        out = torch.empty_like(x)
+    _dev(out, torch.complex64, "out")
+    _check(lib().tina_dft(x.data_ptr(), out.data_ptr(), B, N, int(bool(inverse)), prec, _stream_ptr(stream)))
+    return out
+
+
+def _pfb_args(x, P, M, window):
+    import torch
+    if x.dim() == 1:
+        x = x[None, :]
+    if x.dim() != 2:
+        raise ValueError("x must be [n_samples] or [S, n_samples]")
+    if x.dtype == torch.complex64:
+        kind = COMPLEX
+    elif x.dtype == torch.float32:
+        kind = REAL
+    else:
+        raise TypeError("x must be complex64 (complex kind) or float32 (real kind)")
+    _dev(x, x.dtype, "x")
+    _dev(window, torch.float32, "window")
+    if window.numel() != P * M:
+        raise ValueError("window must have P*M entries")
+    S, n = x.shape
+    F = pfb_num_frames(n, P, M)
+    return x, kind, S, n, F
+
+
+def pfb(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=None):
+    """tina_pfb_batched: x [S, n_samples] (or [n_samples]) complex64 | float32 CUDA,
+    window [P*M] float32 CUDA -> [S, F, P] (complex kind) or [S, F, P/2+1] (real kind) complex64."""
+    import torch
+    squeeze = x.dim() == 1
+    x, kind, S, n, F = _pfb_args(x, P, M, window)
+    NK = P if kind == COMPLEX else P // 2 + 1
+    if out is None:
+        out = torch.empty((S, max(F, 0), NK), dtype=torch.complex64, device=x.device)
+    _dev(out, torch.complex64, "out")
+    _check(lib().tina_pfb_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind, prec,
+                                  out.data_ptr(), _stream_ptr(stream)))
+    return out[0] if squeeze else out
+
+
+def pfb_fir(x, P: int, M: int, window, out=None, stream=None):
+    """tina_pfb_fir_batched: subfilter stage only -> y [S, F, P] (dtype of x)."""
+    import torch
+    squeeze = x.dim() == 1
+    x, kind, S, n, F = _pfb_args(x, P, M, window)
+    if out is None:
+        out = torch.empty((S, max(F, 0), P), dtype=x.dtype, device=x.device)
+    _dev(out, x.dtype, "out")
+    _check(lib().tina_pfb_fir_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind,
+                                      out.data_ptr(), _stream_ptr(stream)))
+    return out[0] if squeeze else out
+
+
+def pfb_host(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=None):
+    """tina_pfb_batched_host: x, window, out are HOST tensors (pinned recommended); synchronous."""
+    import torch
+    if x.dim() == 1:
+        x = x[None, :]
+    if x.is_cuda or window.is_cuda:
+        raise TypeError("pfb_host takes host tensors")
+    kind = COMPLEX if x.dtype == torch.complex64 else REAL
+    if kind == REAL and x.dtype != torch.float32:
+        raise TypeError("x must be complex64 or float32")
+    S, n = x.shape
+    F = pfb_num_frames(n, P, M)
+    NK = P if kind == COMPLEX else P // 2 + 1
+    if out is None:
+        out = torch.empty((S, max(F, 0), NK), dtype=torch.complex64, pin_memory=True)
+    _check(lib().tina_pfb_batched_host(x.data_ptr(), S, n, P, M, window.data_ptr(), kind, prec,
+                                       out.data_ptr(), _stream_ptr(stream)))
+    return out

@@ -1,0 +1,200 @@
+// tina_api.cu -- the C ABI of libtina (include/tina.h): argument validation, dispatch
+// between the tcgen05 path and the generic CUDA-core path, host-buffer wrappers.
+#include "tina_common.cuh"
+
+#include <cstring>
+#include <mutex>
+
+namespace tina {
+
+std::atomic<long long> g_launches{0};
+std::atomic<int> g_last_path{kPathNone};
+static thread_local char t_err[512] = "";
+
+void set_error(const char* fmt, ...)
+{
+    va_list ap; va_start(ap, fmt);
+    vsnprintf(t_err, sizeof(t_err), fmt, ap);
+    va_end(ap);
+}
+
+tina_status fail(tina_status s, const char* fmt, ...)
+{
+    va_list ap; va_start(ap, fmt);
+    vsnprintf(t_err, sizeof(t_err), fmt, ap);
+    va_end(ap);
+    return s;
+}
+
+tina_status check_cuda(cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return TINA_OK;
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? TINA_ERR_OUT_OF_MEMORY : TINA_ERR_CUDA;
+}
+
+// Device staging buffers for the *_host entry points (grown on demand, freed by
+// tina_clear_plan_cache).
+struct Staging { void* p = nullptr; size_t n = 0; };
+static std::mutex g_stage_mu;
+static Staging g_stage[3];
+
+static tina_status stage_reserve(int i, size_t bytes)
+{
+    Staging& s = g_stage[i];
+    if (s.n >= bytes) return TINA_OK;
+    if (s.p) cudaFree(s.p);
+    s.p = nullptr; s.n = 0;
+    cudaError_t e = cudaMalloc(&s.p, bytes);
+    if (e != cudaSuccess) return check_cuda(e, "cudaMalloc(staging)");
+    s.n = bytes;
+    return TINA_OK;
+}
+
+static tina_status pfb_validate(const void* x, int S, long long n_samples, int P, int M,
+                                const float* window, tina_kind kind, const void* out,
+                                const char* who, long long* F_out)
+{
+    if (!x || !window || !out) return fail(TINA_ERR_NULL_POINTER, "%s: null pointer", who);
+    if (kind != TINA_COMPLEX && kind != TINA_REAL) return fail(TINA_ERR_BAD_SHAPE, "%s: bad kind", who);
+    if (S < 1 || P < 2 || M < 1 || n_samples < 1) return fail(TINA_ERR_BAD_SHAPE, "%s: S, M >= 1 and P >= 2 required", who);
+    if (kind == TINA_REAL && (P & 1)) return fail(TINA_ERR_BAD_SHAPE, "%s: P must be even for the real kind", who);
+    if (P > kMaxP) return fail(TINA_ERR_UNSUPPORTED, "%s: P > %d", who, kMaxP);
+    if (M > kMaxTapsPfb) return fail(TINA_ERR_UNSUPPORTED, "%s: M > %d", who, kMaxTapsPfb);
+    const long long F = n_samples / P - M + 1;
+    if (F < 1) return fail(TINA_ERR_BAD_SHAPE, "%s: n_samples too short (F = %lld)", who, F);
+    if (x == out) return fail(TINA_ERR_BAD_SHAPE, "%s: in-place not supported", who);
+    if (!aligned16(x) || !aligned16(out) || !aligned16(window))
+        return fail(TINA_ERR_ALIGNMENT, "%s: x, window, out must be 16-byte aligned", who);
+    if (S > 1) {
+        const long long mod = (kind == TINA_REAL) ? 4 : 2;
+        if (n_samples % mod) return fail(TINA_ERR_ALIGNMENT, "%s: n_samples must be a multiple of %lld when S > 1", who, mod);
+    }
+    *F_out = F;
+    return TINA_OK;
+}
+
+}  // namespace tina
+
+using namespace tina;
+
+extern "C" {
+
+tina_status tina_fir(const float* x, const float* taps, float* y, int C, long long L, int M, void* stream)
+{
+    if (!x || !taps || !y) return fail(TINA_ERR_NULL_POINTER, "tina_fir: null pointer");
+    if (C < 1 || M < 1 || L < M) return fail(TINA_ERR_BAD_SHAPE, "tina_fir: need C >= 1, M >= 1, L >= M");
+    if (M > kMaxTapsFir) return fail(TINA_ERR_UNSUPPORTED, "tina_fir: M > %d", kMaxTapsFir);
+    if ((const void*)x == (const void*)y) return fail(TINA_ERR_BAD_SHAPE, "tina_fir: in-place not supported");
+    if (!aligned16(x) || !aligned16(y)) return fail(TINA_ERR_ALIGNMENT, "tina_fir: x, y must be 16-byte aligned");
+    return simt_fir(x, taps, y, C, L, M, (cudaStream_t)stream);
+}
+
+tina_status tina_dft(const void* x, void* out, long long B, int N, int inverse,
+                     tina_precision prec, void* stream)
+{
+    if (!x || !out) return fail(TINA_ERR_NULL_POINTER, "tina_dft: null pointer");
+    if (B < 1 || N < 2) return fail(TINA_ERR_BAD_SHAPE, "tina_dft: need B >= 1, N >= 2");
+    if (N > kMaxP) return fail(TINA_ERR_UNSUPPORTED, "tina_dft: N > %d", kMaxP);
+    if (prec != TINA_PREC_FP32 && prec != TINA_PREC_BF16) return fail(TINA_ERR_BAD_SHAPE, "tina_dft: bad precision");
+    if (x == out) return fail(TINA_ERR_BAD_SHAPE, "tina_dft: in-place not supported");
+    if (!aligned16(x) || !aligned16(out)) return fail(TINA_ERR_ALIGNMENT, "tina_dft: x, out must be 16-byte aligned");
+    // A DFT batch is a PFB with M = 1 and unit taps over one stream of B*N samples.
+    if (umma_supported(N, false))
+        return umma_pfb(x, 1, B * (long long)N, N, 1, nullptr, false, inverse != 0, prec, out, (cudaStream_t)stream);
+    return simt_pfb(x, 1, B * (long long)N, N, 1, nullptr, false, inverse != 0, out, (cudaStream_t)stream);
+}
+
+tina_status tina_pfb_batched(const void* x, int S, long long n_samples, int P, int M,
+                             const float* window, tina_kind kind, tina_precision prec,
+                             void* out, void* stream)
+{
+    long long F;
+    tina_status st = pfb_validate(x, S, n_samples, P, M, window, kind, out, "tina_pfb", &F);
+    if (st != TINA_OK) return st;
+    if (prec != TINA_PREC_FP32 && prec != TINA_PREC_BF16) return fail(TINA_ERR_BAD_SHAPE, "tina_pfb: bad precision");
+    const bool real = kind == TINA_REAL;
+    if (umma_supported(P, real))
+        return umma_pfb(x, S, n_samples, P, M, window, real, false, prec, out, (cudaStream_t)stream);
+    return simt_pfb(x, S, n_samples, P, M, window, real, false, out, (cudaStream_t)stream);
+}
+
+tina_status tina_pfb(const void* x, long long n_samples, int P, int M, const float* window,
+                     tina_kind kind, tina_precision prec, void* out, void* stream)
+{
+    return tina_pfb_batched(x, 1, n_samples, P, M, window, kind, prec, out, stream);
+}
+
+tina_status tina_pfb_fir_batched(const void* x, int S, long long n_samples, int P, int M,
+                                 const float* window, tina_kind kind, void* y, void* stream)
+{
+    long long F;
+    tina_status st = pfb_validate(x, S, n_samples, P, M, window, kind, y, "tina_pfb_fir", &F);
+    if (st != TINA_OK) return st;
+    return simt_pfb_fir(x, S, n_samples, P, M, window, kind == TINA_REAL, y, (cudaStream_t)stream);
+}
+
+tina_status tina_pfb_batched_host(const void* x_host, int S, long long n_samples, int P, int M,
+                                  const float* window_host, tina_kind kind, tina_precision prec,
+                                  void* out_host, void* stream)
+{
+    if (!x_host || !window_host || !out_host) return fail(TINA_ERR_NULL_POINTER, "tina_pfb_batched_host: null pointer");
+    if (S < 1 || P < 2 || M < 1 || n_samples < 1) return fail(TINA_ERR_BAD_SHAPE, "tina_pfb_batched_host: bad shape");
+    if (kind != TINA_COMPLEX && kind != TINA_REAL) return fail(TINA_ERR_BAD_SHAPE, "tina_pfb_batched_host: bad kind");
+    const long long F = n_samples / P - M + 1;
+    if (F < 1) return fail(TINA_ERR_BAD_SHAPE, "tina_pfb_batched_host: n_samples too short");
+    const size_t esz = kind == TINA_REAL ? 4 : 8;
+    const size_t nk = kind == TINA_REAL ? (size_t)P / 2 + 1 : (size_t)P;
+    const size_t xb = (size_t)S * n_samples * esz, wb = (size_t)P * M * 4, ob = (size_t)S * F * nk * 8;
+    std::lock_guard<std::mutex> lk(g_stage_mu);
+    tina_status st;
+    if ((st = stage_reserve(0, xb)) != TINA_OK) return st;
+    if ((st = stage_reserve(1, wb)) != TINA_OK) return st;
+    if ((st = stage_reserve(2, ob)) != TINA_OK) return st;
+    cudaStream_t cs = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(g_stage[0].p, x_host, xb, cudaMemcpyHostToDevice, cs);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g_stage[1].p, window_host, wb, cudaMemcpyHostToDevice, cs);
+    if (e != cudaSuccess) return check_cuda(e, "H2D copy");
+    st = tina_pfb_batched(g_stage[0].p, S, n_samples, P, M, (const float*)g_stage[1].p, kind, prec, g_stage[2].p, stream);
+    if (st != TINA_OK) return st;
+    e = cudaMemcpyAsync(out_host, g_stage[2].p, ob, cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
+    return check_cuda(e, "D2H copy / synchronize");
+}
+
+long long tina_pfb_num_frames(long long n_samples, int P, int M)
+{
+    if (P < 1 || M < 1 || n_samples < 0) return 0;
+    return n_samples / P - M + 1;
+}
+
+const char* tina_status_string(tina_status s)
+{
+    switch (s) {
+        case TINA_OK: return "TINA_OK";
+        case TINA_ERR_NULL_POINTER: return "TINA_ERR_NULL_POINTER";
+        case TINA_ERR_BAD_SHAPE: return "TINA_ERR_BAD_SHAPE";
+        case TINA_ERR_UNSUPPORTED: return "TINA_ERR_UNSUPPORTED";
+        case TINA_ERR_ALIGNMENT: return "TINA_ERR_ALIGNMENT";
+        case TINA_ERR_CUDA: return "TINA_ERR_CUDA";
+        case TINA_ERR_OUT_OF_MEMORY: return "TINA_ERR_OUT_OF_MEMORY";
+    }
+    return "TINA_ERR_UNKNOWN";
+}
+
+const char* tina_last_error(void) { return t_err; }
+
+tina_status tina_clear_plan_cache(void)
+{
+    umma_clear_plans();
+    std::lock_guard<std::mutex> lk(g_stage_mu);
+    for (auto& s : g_stage) { if (s.p) cudaFree(s.p); s.p = nullptr; s.n = 0; }
+    return TINA_OK;
+}
+
+int tina_version(void) { return 100; }  /* 0.1.0 */
+
+long long tina_launch_count(void) { return g_launches.load(); }
+int tina_last_path(void) { return g_last_path.load(); }
+
+}  // extern "C"

@@ -1,0 +1,44 @@
+// tina_common.cuh -- shared host-side helpers of libtina (status text, launch counter).
+#pragma once
+#include <cuda_runtime.h>
+#include <atomic>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+
+#include "../../include/tina.h"
+
+namespace tina {
+
+constexpr int kMaxP = 8192;      // upper bound on P / N (DFT size)
+constexpr int kMaxTapsPfb = 64;  // upper bound on M for the PFB
+constexpr int kMaxTapsFir = 4096;
+
+enum Path { kPathNone = 0, kPathSimt = 1, kPathUmma = 2 };
+
+extern std::atomic<long long> g_launches;
+extern std::atomic<int> g_last_path;
+
+void set_error(const char* fmt, ...);
+tina_status fail(tina_status s, const char* fmt, ...);
+tina_status check_cuda(cudaError_t e, const char* what);
+
+inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// ---- generic CUDA-core path (tina_simt.cu) ------------------------------------------
+tina_status simt_fir(const float* x, const float* taps, float* y, int C, long long L, int M,
+                     cudaStream_t st);
+// PFB / DFT on CUDA cores: window == nullptr means M == 1 with unit taps (plain DFT).
+tina_status simt_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window,
+                     bool real, bool inverse, void* out, cudaStream_t st);
+tina_status simt_pfb_fir(const void* x, int S, long long n_samples, int P, int M,
+                         const float* window, bool real, void* y, cudaStream_t st);
+
+// ---- tcgen05 tensor-core path (tina_umma.cu) ----------------------------------------
+bool umma_supported(int P, bool real);
+tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window,
+                     bool real, bool inverse, tina_precision prec, void* out, cudaStream_t st);
+void umma_clear_plans();
+
+}  // namespace tina

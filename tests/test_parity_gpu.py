@@ -1,0 +1,218 @@
+"""GPU parity: libtina (through the C ABI binding) vs the float64 oracle, element by element
+on identical seeded inputs.  Tolerances (BASELINE.json north_star):
+relative L2 per output frame <= 1e-5 (fp32 configs), <= 2e-2 (bf16 config)."""
+import numpy as np
+import pytest
+
+import tina_inputs as ti
+from conftest import rel_l2_rows
+
+pytestmark = pytest.mark.gpu
+
+TOL_FP32 = 1e-5
+TOL_BF16 = 2e-2
+
+
+@pytest.fixture(scope="module")
+def tina():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2408_16551_b200 as t
+    t.lib()  # raises if libtina.so is missing -- no fallback
+    return t
+
+
+def _cuda(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _run_pfb(tina, case, prec=0):
+    import torch
+    x = _cuda(case.x)
+    w = _cuda(case.window)
+    out = tina.pfb(x, case.P, case.M, w, prec=prec)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+# ------------------------------------------------------------------ FIR
+@pytest.mark.parametrize("C,L,K", [(1, 64, 64), (3, 5000, 64), (2, 2048 + 63, 64), (2, 2049 + 63, 64),
+                                   (5, 777, 1), (2, 9000, 7), (1, 4500, 200), (4, 100000, 64)])
+def test_fir_parity_small(tina, oracle, C, L, K):
+    import torch
+    rng = np.random.default_rng(100 + C * 7 + K)
+    x = ti.noise_real(rng, C * L).reshape(C, L)
+    a = ti.random_taps(rng, K)                       # asymmetric: a flipped kernel would fail
+    y = tina.fir(_cuda(x), _cuda(a))
+    torch.cuda.synchronize()
+    ref = oracle.fir(x, a)
+    assert y.shape == ref.shape
+    assert rel_l2_rows(y.cpu().numpy(), ref) <= TOL_FP32
+
+
+def test_fir_impulse_response_is_taps(tina):
+    import torch
+    K = 64
+    a = ti.random_taps(np.random.default_rng(5), K)
+    x = np.zeros((1, 2 * K - 1), np.float32); x[0, K - 1] = 1
+    y = tina.fir(_cuda(x), _cuda(a))
+    torch.cuda.synchronize()
+    assert np.array_equal(y.cpu().numpy()[0], a)
+
+
+def test_config3_fir_full(tina, oracle):
+    """c3 at full size; per-channel rel L2 and per-4096-sample-block rel L2."""
+    import torch
+    x, taps, taps_asym = ti.config3()
+    xd = _cuda(x)
+    for a in (taps, taps_asym):
+        y = tina.fir(xd, _cuda(a))
+        torch.cuda.synchronize()
+        y = y.cpu().numpy()
+        ref = oracle.fir(x, a)
+        assert y.shape == (64, (1 << 20) - 63)
+        assert rel_l2_rows(y, ref) <= TOL_FP32
+        nblk = ref.shape[1] // 4096
+        yb = y[:, : nblk * 4096].reshape(-1, 4096)
+        rb = ref[:, : nblk * 4096].reshape(-1, 4096)
+        assert rel_l2_rows(yb, rb) <= TOL_FP32
+
+
+# ------------------------------------------------------------------ DFT
+@pytest.mark.parametrize("B,N", [(1, 2), (7, 3), (33, 12), (300, 16), (129, 100), (5, 250)])
+def test_dft_generic_sizes(tina, oracle, B, N):
+    import torch
+    rng = np.random.default_rng(200 + N)
+    x = ti.noise_complex(rng, B * N).reshape(B, N)
+    Z = tina.dft(_cuda(x)); Xi = tina.dft(_cuda(x), inverse=True)
+    torch.cuda.synchronize()
+    assert rel_l2_rows(Z.cpu().numpy(), oracle.dft(x)) <= TOL_FP32
+    assert rel_l2_rows(Xi.cpu().numpy(), oracle.dft(x, inverse=True)) <= TOL_FP32
+
+
+@pytest.mark.parametrize("B,N", [(1, 32), (128, 32), (130, 64), (257, 96), (1000, 128), (300, 256),
+                                 (77, 512), (140, 1024), (129, 2048)])
+@pytest.mark.parametrize("prec,tol", [(0, TOL_FP32), (1, TOL_BF16)])
+def test_dft_tensor_sizes(tina, oracle, B, N, prec, tol):
+    """N % 32 == 0: tcgen05 path; spans several M tiles and a ragged tail."""
+    import torch
+    rng = np.random.default_rng(300 + N + B)
+    x = ti.noise_complex(rng, B * N).reshape(B, N)
+    Z = tina.dft(_cuda(x), prec=prec); Xi = tina.dft(_cuda(x), inverse=True, prec=prec)
+    torch.cuda.synchronize()
+    assert rel_l2_rows(Z.cpu().numpy(), oracle.dft(x)) <= tol
+    assert rel_l2_rows(Xi.cpu().numpy(), oracle.dft(x, inverse=True)) <= tol
+
+
+def test_dft_unit_impulse_and_tone(tina):
+    import torch
+    N = 256
+    x = np.zeros((2, N), np.complex64)
+    x[0, 0] = 1
+    x[1] = np.exp(2j * np.pi * ((17 * np.arange(N)) % N) / N)
+    Z = tina.dft(_cuda(x)); torch.cuda.synchronize()
+    Z = Z.cpu().numpy()
+    assert np.allclose(Z[0], 1, atol=1e-5)
+    want = np.zeros(N, np.complex128); want[17] = N
+    assert np.linalg.norm(Z[1] - want) / N <= TOL_FP32
+
+
+def test_config2_dft_roundtrip_full(tina, oracle):
+    """c2: B=65536, N=256 forward then inverse; oracle on a seeded row sample."""
+    import torch
+    x = ti.config2()
+    xd = _cuda(x)
+    Z = tina.dft(xd)
+    xb = tina.dft(Z, inverse=True)
+    torch.cuda.synchronize()
+    rows = ti.sample_frames(x.shape[0], 480, ti.SEED_BASE + 2)
+    assert rel_l2_rows(Z.cpu().numpy()[rows], oracle.dft(x[rows])) <= TOL_FP32
+    xb = xb.cpu().numpy()
+    assert rel_l2_rows(xb, x.astype(np.complex128)) <= 2 * TOL_FP32          # two transforms
+    ref_rt = oracle.dft(oracle.dft(x[rows]), inverse=True)
+    assert rel_l2_rows(xb[rows], ref_rt) <= 2 * TOL_FP32
+
+
+# ------------------------------------------------------------------ PFB
+@pytest.mark.parametrize("P,M,F,real", [
+    (2, 1, 1, False), (4, 3, 5, False), (16, 4, 100, False), (10, 2, 33, True), (24, 5, 17, False),
+    (32, 4, 300, False), (64, 8, 200, False), (64, 8, 129, True), (128, 16, 257, False),
+    (256, 3, 140, True), (96, 2, 131, False), (192, 4, 70, True), (1024, 16, 130, False),
+    (2048, 2, 129, True), (32, 1, 128, False), (64, 64, 40, False)])
+def test_pfb_parity_small(tina, oracle, P, M, F, real):
+    rng = np.random.default_rng(400 + P + M)
+    case = ti.pfb_case(P, M, F, real=real, seed=401 + P, window=ti.random_taps(rng, P * M))
+    got = _run_pfb(tina, case)
+    ref = oracle.pfb(case.x[0], P, M, case.window)
+    assert got.shape[1:] == ref.shape
+    assert rel_l2_rows(got[0], ref) <= TOL_FP32
+
+
+@pytest.mark.parametrize("P,M,F,real", [(64, 4, 200, False), (128, 8, 150, True), (1024, 16, 130, False)])
+def test_pfb_bf16_small(tina, oracle, P, M, F, real):
+    case = ti.pfb_case(P, M, F, real=real, seed=500 + P)
+    got = _run_pfb(tina, case, prec=1)
+    ref = oracle.pfb(case.x[0], P, M, case.window)
+    assert rel_l2_rows(got[0], ref) <= TOL_BF16
+
+
+def test_pfb_batched_streams_and_tail(tina, oracle):
+    """S streams in one launch; n_samples not a multiple of P (tail ignored, reading R8)."""
+    P, M, F, S = 64, 4, 140, 3
+    case = ti.pfb_case(P, M, F, streams=S, seed=600)
+    x = np.concatenate([case.x, np.ones((S, 6), np.complex64)], axis=1)     # ragged tail
+    case.x = np.ascontiguousarray(x)
+    got = _run_pfb(tina, case)
+    assert got.shape == (S, F, P)
+    for s in range(S):
+        assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
+
+
+def test_pfb_m1_rect_is_blocked_dft(tina, oracle):
+    import torch
+    P, F = 128, 256
+    case = ti.pfb_case(P, 1, F, seed=700, window=np.ones(P, np.float32))
+    got = _run_pfb(tina, case)[0]
+    blocks = _cuda(case.x[0].reshape(F, P))
+    Z = tina.dft(blocks); torch.cuda.synchronize()
+    assert np.array_equal(got, Z.cpu().numpy())
+    assert rel_l2_rows(got, oracle.dft(case.x[0].reshape(F, P))) <= TOL_FP32
+
+
+def test_config1_pfb_full(tina, oracle):
+    case = ti.config1()
+    got = _run_pfb(tina, case)
+    ref = oracle.pfb(case.x[0], case.P, case.M, case.window)
+    assert got.shape == (1, 4096, 16)
+    assert rel_l2_rows(got[0], ref) <= TOL_FP32
+
+
+def test_pfb_fir_only(tina, oracle):
+    import torch
+    for real in (False, True):
+        P, M, F = 64, 16, 100
+        rng = np.random.default_rng(800)
+        case = ti.pfb_case(P, M, F, real=real, streams=2, seed=801, window=ti.random_taps(rng, P * M))
+        y = tina.pfb_fir(_cuda(case.x), P, M, _cuda(case.window)); torch.cuda.synchronize()
+        y = y.cpu().numpy()
+        for s in range(2):
+            _, yref = oracle.pfb(case.x[s], P, M, case.window, return_subfiltered=True)
+            assert rel_l2_rows(y[s], yref) <= TOL_FP32
+
+
+def test_error_paths(tina):
+    import torch
+    x = torch.zeros(64, dtype=torch.complex64, device="cuda")
+    w = torch.ones(64, dtype=torch.float32, device="cuda")
+    with pytest.raises(tina.TinaError) as e:
+        tina.pfb(x, 16, 4, w)                    # 4 blocks, M=4 -> F=1 OK ... make it too short:
+        tina.pfb(x[:48], 16, 4, w)
+    assert e.value.status == 2
+    with pytest.raises(tina.TinaError) as e:
+        tina.pfb(torch.zeros(10, dtype=torch.float32, device="cuda"), 5, 1,
+                 torch.ones(5, dtype=torch.float32, device="cuda"))       # odd P, real kind
+    assert e.value.status == 2
+    with pytest.raises(tina.TinaError) as e:
+        tina.dft(torch.zeros((1, 16384), dtype=torch.complex64, device="cuda"))
+    assert e.value.status == 3
