@@ -55,7 +55,7 @@ static tina_status pfb_validate(const void* x, int S, long long n_samples, int P
                                 const float* window, tina_kind kind, const void* out,
                                 const char* who, long long* F_out)
 {
-    if (!x || !window || !out) return fail(TINA_ERR_NULL_POINTER, "%s: null pointer", who);
+    if (!x || !window) return fail(TINA_ERR_NULL_POINTER, "%s: null pointer", who);
     if (kind != TINA_COMPLEX && kind != TINA_REAL) return fail(TINA_ERR_BAD_SHAPE, "%s: bad kind", who);
     if (S < 1 || P < 2 || M < 1 || n_samples < 1) return fail(TINA_ERR_BAD_SHAPE, "%s: S, M >= 1 and P >= 2 required", who);
     if (kind == TINA_REAL && (P & 1)) return fail(TINA_ERR_BAD_SHAPE, "%s: P must be even for the real kind", who);
@@ -63,6 +63,7 @@ static tina_status pfb_validate(const void* x, int S, long long n_samples, int P
     if (M > kMaxTapsPfb) return fail(TINA_ERR_UNSUPPORTED, "%s: M > %d", who, kMaxTapsPfb);
     const long long F = n_samples / P - M + 1;
     if (F < 1) return fail(TINA_ERR_BAD_SHAPE, "%s: n_samples too short (F = %lld)", who, F);
+    if (!out) return fail(TINA_ERR_NULL_POINTER, "%s: null output pointer", who);
     if (x == out) return fail(TINA_ERR_BAD_SHAPE, "%s: in-place not supported", who);
     if (!aligned16(x) || !aligned16(out) || !aligned16(window))
         return fail(TINA_ERR_ALIGNMENT, "%s: x, window, out must be 16-byte aligned", who);

@@ -206,8 +206,7 @@ def test_error_paths(tina):
     x = torch.zeros(64, dtype=torch.complex64, device="cuda")
     w = torch.ones(64, dtype=torch.float32, device="cuda")
     with pytest.raises(tina.TinaError) as e:
-        tina.pfb(x, 16, 4, w)                    # 4 blocks, M=4 -> F=1 OK ... make it too short:
-        tina.pfb(x[:48], 16, 4, w)
+        tina.pfb(x[:48], 16, 4, w)               # 3 blocks, M=4 -> F=0: too short
     assert e.value.status == 2
     with pytest.raises(tina.TinaError) as e:
         tina.pfb(torch.zeros(10, dtype=torch.float32, device="cuda"), 5, 1,
