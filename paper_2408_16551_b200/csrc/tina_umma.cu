@@ -41,6 +41,7 @@ constexpr int NB_RING = 4;
 constexpr int UMMA_THREADS = 512;
 constexpr int PROD_WARP0 = 8, N_PROD_WARPS = 8, FPW = BM / N_PROD_WARPS;   // 16 frames per producer warp
 constexpr int EPI_WARP0 = 4;
+constexpr int KSPLIT_MAX = 1024;            // longest accumulation chain kept in TMEM (K elements)
 
 struct SmemCtl {
     uint64_t a_full[4], a_empty[4];
@@ -61,6 +62,7 @@ struct UmmaParams {
     int P, M;
     int tiles_per_stream, n_passes, total_work;
     int parts;                 // 2: bf16x3 (hi+lo), 1: single bf16 pass
+    int k_splits, kc_per_split; // accumulation chains per tile
 };
 
 // =====================================================================================
@@ -244,10 +246,12 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm
             const int n0 = (w % prm.n_passes) * NT_MAX;
             const int nt = min(NT_MAX, N - n0);
             const int n_sub = (nt + NSUB - 1) / NSUB;
+            for (int ks = 0; ks < prm.k_splits; ++ks) {
             mbar_wait(smem_u32(&ctl->t_empty[t.idx]), t.phase ^ 1);
             tc_fence_after();
             const uint32_t d_base = tmem_base + t.idx * 256;
-            for (int kc = 0; kc < n_kc; ++kc) {
+            const int kc_begin = ks * prm.kc_per_split, kc_end = min(n_kc, kc_begin + prm.kc_per_split);
+            for (int kc = kc_begin; kc < kc_end; ++kc) {
                 mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
                 tc_fence_after();
                 const uint32_t a_hi = smem_u32(a_ring + a.idx * a_slot_bytes);
@@ -261,7 +265,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm
                     tc_fence_after();
                     if (lane == 0) {
                         const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * B_ENTRY_BYTES));
-                        uint32_t acc = kc > 0;
+                        uint32_t acc = kc > kc_begin;
                         if (parts > 1) {
                             const uint64_t ad = smem_desc_sw128(a_lo);
 #pragma unroll
@@ -291,12 +295,13 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm
                 }
                 if (lane == 0) {
                     umma_commit(smem_u32(&ctl->a_empty[a.idx]));
-                    if (kc == n_kc - 1) umma_commit(smem_u32(&ctl->t_full[t.idx]));
+                    if (kc == kc_end - 1) umma_commit(smem_u32(&ctl->t_full[t.idx]));
                 }
                 __syncwarp();
                 a.advance(n_a);
             }
             t.advance(n_acc);
+            }
         }
     } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
         // ============================ epilogue: TMEM -> global ==============================
@@ -310,37 +315,63 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm
             const long long row = (long long)(tile % prm.tiles_per_stream) * BM + q * 32 + lane;
             const bool valid = row < prm.F;
             float* orow = prm.out + ((long long)s * prm.F + row) * prm.out_row;
-            mbar_wait(smem_u32(&ctl->t_full[t.idx]), t.phase);
-            tc_fence_after();
-            const uint32_t taddr = tmem_base + t.idx * 256 + ((uint32_t)(q * 32) << 16);
-            for (int cb = 0; cb < nt; cb += 32) {
-                uint32_t r[32];
-                tmem_ld32(taddr + cb, r);
-                tmem_ld_wait();
-                if (valid) {
-                    const int n = n0 + cb;
-                    if (REAL) {
-                        float2* o2 = reinterpret_cast<float2*>(orow + n);
+            for (int ks = 0; ks < prm.k_splits; ++ks) {
+                mbar_wait(smem_u32(&ctl->t_full[t.idx]), t.phase);
+                tc_fence_after();
+                const uint32_t taddr = tmem_base + t.idx * 256 + ((uint32_t)(q * 32) << 16);
+                for (int cb = 0; cb < nt; cb += 32) {
+                    uint32_t r[32];
+                    tmem_ld32(taddr + cb, r);
+                    tmem_ld_wait();
+                    if (valid) {
+                        const int n = n0 + cb;
+                        float4* o4 = reinterpret_cast<float4*>(orow + n);     // complex rows are 16-byte aligned
+                        float2* o2 = reinterpret_cast<float2*>(orow + n);     // real rows only 8-byte aligned
+                        if (ks > 0) {
+                            // later accumulation chains: out += chain (fp32 round-to-nearest add)
+                            if (REAL) {
 #pragma unroll
-                        for (int j = 0; j < 16; ++j)
-                            o2[j] = make_float2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
-                        if (n == 0) {   // columns 0 / 1 carry Re X[0] and Re X[P/2]; both bins are real
-                            o2[0] = make_float2(__uint_as_float(r[0]), 0.f);
-                            *reinterpret_cast<float2*>(orow + prm.P) = make_float2(__uint_as_float(r[1]), 0.f);
+                                for (int j = 0; j < 16; ++j) {
+                                    const float2 o = o2[j];
+                                    r[2 * j] = __float_as_uint(o.x + __uint_as_float(r[2 * j]));
+                                    r[2 * j + 1] = __float_as_uint(o.y + __uint_as_float(r[2 * j + 1]));
+                                }
+                            } else {
+#pragma unroll
+                                for (int j = 0; j < 8; ++j) {
+                                    const float4 o = o4[j];
+                                    r[4 * j] = __float_as_uint(o.x + __uint_as_float(r[4 * j]));
+                                    r[4 * j + 1] = __float_as_uint(o.y + __uint_as_float(r[4 * j + 1]));
+                                    r[4 * j + 2] = __float_as_uint(o.z + __uint_as_float(r[4 * j + 2]));
+                                    r[4 * j + 3] = __float_as_uint(o.w + __uint_as_float(r[4 * j + 3]));
+                                }
+                            }
                         }
-                    } else {
-                        float4* o4 = reinterpret_cast<float4*>(orow + n);
+                        if (REAL) {
+                            if (n == 0) {
+                                // columns 0 / 1 carry Re X[0] and Re X[P/2]; both bins are purely real
+                                float2* ny = reinterpret_cast<float2*>(orow + prm.P);
+                                float nyq = __uint_as_float(r[1]);
+                                if (ks > 0) nyq += ny->x;                     // out[1] == 0 was added above: r[1] is still the chain value
+                                *ny = make_float2(nyq, 0.f);
+                                r[1] = 0u;
+                            }
 #pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            o4[j] = make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
-                                                __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
+                            for (int j = 0; j < 16; ++j)
+                                o2[j] = make_float2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < 8; ++j)
+                                o4[j] = make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
+                                                    __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
+                        }
                     }
                 }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->t_empty[t.idx]));
+                t.advance(n_acc);
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(&ctl->t_empty[t.idx]));
-            t.advance(n_acc);
         }
     } else if (warp >= PROD_WARP0) {
         // ============================ FIR producers =========================================
@@ -489,6 +520,8 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     if (total > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: too many tiles");
     prm.total_work = (int)total;
     prm.parts = parts;
+    prm.k_splits = (K + KSPLIT_MAX - 1) / KSPLIT_MAX;
+    prm.kc_per_split = ((K / KC) + prm.k_splits - 1) / prm.k_splits;
 
     static int n_sm = 0;
     if (!n_sm) {
