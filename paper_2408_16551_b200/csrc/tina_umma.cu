@@ -175,14 +175,107 @@ void umma_clear_plans()
 }
 
 // =====================================================================================
-// The fused kernel.  MT = compile-time tap count the sliding window is unrolled for
-// (taps m >= M are zero; MT == 0: no window, y = x, i.e. a plain DFT batch).
+// FIR producer: one warp computes FPW (16) consecutive frames x 64 scalar columns of the
+// subfiltered signal (Eq. (20)) and writes them, split into bf16 hi / lo, into an A-ring slot
+// in the canonical K-major SWIZZLE_128B layout.  Each lane owns two adjacent scalar columns
+// (one complex sample, or two real branches); the last MT input rows live in a rotating
+// register window, so every input sample is loaded once per warp and every output costs MT
+// packed FMAs (fma.rn.f32x2).  All global loads are issued before the wait on the slot.
 // =====================================================================================
 struct RingPos {
     uint32_t idx = 0, phase = 0;
     __device__ __forceinline__ void advance(uint32_t n) { if (++idx == n) { idx = 0; phase ^= 1; } }
 };
 
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
+{
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return d;
+}
+__device__ __forceinline__ float2 fmul2(float2 a, float2 b)
+{
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+        "mul.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return d;
+}
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ float2 ldg_f2(const float* p)
+{
+    return __ldg(reinterpret_cast<const float2*>(p));
+}
+
+template <int MT, bool REAL, bool CHECK>
+__device__ __forceinline__ void fir_chunk(const UmmaParams& prm, const float* __restrict__ xc, int c0, long long f0,
+                                          uint32_t a_ring_s, uint32_t a_slot_bytes, const uint32_t (&swz)[8],
+                                          SmemCtl* ctl, const RingPos& a, bool split)
+{
+    constexpr int WA = MT > 0 ? MT : 1;
+    const int M = prm.M;
+    const long long K = prm.K;
+    float2 tap[WA], row[WA - 1 + FPW];
+    // ---- all global loads first (taps, then the FPW + WA - 1 input rows this warp touches)
+    if (MT > 0) {
+#pragma unroll
+        for (int m = 0; m < WA; ++m) {
+            if (m < M) {
+                if (REAL) tap[m] = ldg_f2(prm.window + (long long)m * prm.P + c0);
+                else { const float h = __ldg(prm.window + (long long)m * prm.P + (c0 >> 1)); tap[m] = make_float2(h, h); }
+            } else tap[m] = make_float2(0.f, 0.f);
+        }
+    }
+    {
+        const long long r0 = f0 + M - WA;                 // first row of the window of frame f0
+        const float* p = xc + r0 * K;
+#pragma unroll
+        for (int j = 0; j < WA - 1 + FPW; ++j) {
+            if (CHECK) {
+                const long long r = r0 + j;
+                row[j] = (r >= 0 && r < prm.NBLK) ? ldg_f2(p) : make_float2(0.f, 0.f);
+            } else {
+                row[j] = ldg_f2(p);
+            }
+            p += K;
+        }
+    }
+    mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
+    const uint32_t slot = a_ring_s + a.idx * a_slot_bytes;
+    // ---- frame i uses rows i .. i + WA - 1 (row i + WA - 1 - m pairs with tap m)
+#pragma unroll
+    for (int i = 0; i < FPW; ++i) {
+        float2 y;
+        if (MT > 0) {
+            y = fmul2(tap[0], row[i + WA - 1]);
+#pragma unroll
+            for (int m = 1; m < WA; ++m) y = ffma2(tap[m], row[i + WA - 1 - m], y);
+        } else {
+            y = row[i];
+        }
+        const __nv_bfloat162 hi = __floats2bfloat162_rn(y.x, y.y);
+        const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
+        const uint32_t addr = slot + swz[i & 7] + (uint32_t)i * 128u;
+        sts32(addr, hb);
+        if (split) {
+            const float lx = y.x - __uint_as_float(hb << 16);
+            const float ly = y.y - __uint_as_float(hb & 0xffff0000u);
+            const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
+            sts32(addr + A_PART_BYTES, *reinterpret_cast<const uint32_t*>(&lo));
+        }
+    }
+    fence_proxy_async();
+}
+
+// =====================================================================================
+// The fused kernel.  MT = compile-time tap count the sliding window is unrolled for
+// (taps m >= M are zero; MT == 0: no window, y = x, i.e. a plain DFT batch).
+// =====================================================================================
 template <int MT, bool REAL>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm)
@@ -375,72 +468,30 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm
         }
     } else if (warp >= PROD_WARP0) {
         // ============================ FIR producers =========================================
-        constexpr int W = MT > 0 ? MT : FPW;     // frames per unrolled group
-        constexpr int WA = MT > 0 ? MT : 1;      // window / tap registers
         const int pw = warp - PROD_WARP0;
-        const int M = prm.M;
+        const uint32_t a_ring_s = smem_u32(a_ring);
+        // byte offset of this lane's 4-byte cell in row 0 of an A tile, for each swizzle phase (row & 7):
+        // row r, 16-byte chunk (lane >> 2) is stored at chunk position (lane >> 2) ^ (r & 7)
+        uint32_t swz[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            swz[j] = (uint32_t)(pw * FPW) * 128u + ((((uint32_t)lane >> 2) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 3u) * 4u;
         RingPos a;
         for (int w = blockIdx.x; w < prm.total_work; w += gridDim.x) {
             const int tile = w / prm.n_passes;
             const int s = tile / prm.tiles_per_stream;
             const long long f0 = (long long)(tile % prm.tiles_per_stream) * BM + pw * FPW;
-            const float* xs = prm.x + (long long)s * prm.stream_stride;
+            const float* xs = prm.x + (long long)s * prm.stream_stride + 2 * lane;
+            // rows f0 + M - WA .. f0 + FPW + M - 2 are touched; interior tiles need no bounds checks
+            constexpr int WA = MT > 0 ? MT : 1;
+            const bool interior = (f0 + prm.M - WA >= 0) && (f0 + FPW + prm.M - 1 <= prm.NBLK);
             for (int kc = 0; kc < n_kc; ++kc) {
-                const int c0 = kc * KC + 2 * lane;
-                const float* xc = xs + c0;
-                float2 tap[WA], win[WA];
-                if (MT > 0) {
-#pragma unroll
-                    for (int m = 0; m < WA; ++m) {
-                        if (m < M) {
-                            if (REAL) tap[m] = __ldg(reinterpret_cast<const float2*>(prm.window + (long long)m * prm.P + c0));
-                            else { const float h = __ldg(prm.window + (long long)m * prm.P + (c0 >> 1)); tap[m] = make_float2(h, h); }
-                        } else tap[m] = make_float2(0.f, 0.f);
-                    }
-                    // window slots 0..W-2 <- input rows f0 + M - W + j
-#pragma unroll
-                    for (int j = 0; j < WA - 1; ++j) {
-                        const long long r = f0 + M - WA + j;
-                        win[j] = (r >= 0 && r < prm.NBLK) ? __ldg(reinterpret_cast<const float2*>(xc + r * prm.K))
-                                                           : make_float2(0.f, 0.f);
-                    }
-                }
-                mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
-                uint8_t* slot = a_ring + a.idx * a_slot_bytes;
-#pragma unroll
-                for (int fb = 0; fb < FPW; fb += W) {
-#pragma unroll
-                    for (int u = 0; u < W; ++u) {
-                        const int fl = pw * FPW + fb + u;                 // frame row within the tile
-                        const long long r = f0 + fb + u + M - 1;          // newest input row of this frame
-                        const float2 v = (r < prm.NBLK) ? __ldg(reinterpret_cast<const float2*>(xc + r * prm.K))
-                                                        : make_float2(0.f, 0.f);
-                        float2 y;
-                        if (MT > 0) {
-                            win[(u + WA - 1) % WA] = v;
-                            y = make_float2(0.f, 0.f);
-#pragma unroll
-                            for (int m = 0; m < WA; ++m) {
-                                const float2 xv = win[(u + WA - 1 - m + WA) % WA];
-                                y.x = fmaf(tap[m].x, xv.x, y.x);
-                                y.y = fmaf(tap[m].y, xv.y, y.y);
-                            }
-                        } else {
-                            y = v;
-                        }
-                        const __nv_bfloat162 hi = __floats2bfloat162_rn(y.x, y.y);
-                        const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
-                        const uint32_t off = (uint32_t)fl * 128u + ((((uint32_t)lane >> 2) ^ ((uint32_t)fl & 7u)) << 4) + ((uint32_t)lane & 3u) * 4u;
-                        *reinterpret_cast<uint32_t*>(slot + off) = hb;
-                        if (parts > 1) {
-                            const float lx = y.x - __uint_as_float(hb << 16);
-                            const float ly = y.y - __uint_as_float(hb & 0xffff0000u);
-                            const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
-                            *reinterpret_cast<uint32_t*>(slot + A_PART_BYTES + off) = *reinterpret_cast<const uint32_t*>(&lo);
-                        }
-                    }
-                }
-                fence_proxy_async();
+                if (interior)
+                    fir_chunk<MT, REAL, false>(prm, xs + kc * KC, kc * KC + 2 * lane, f0, a_ring_s, a_slot_bytes, swz,
+                                               ctl, a, parts > 1);
+                else
+                    fir_chunk<MT, REAL, true>(prm, xs + kc * KC, kc * KC + 2 * lane, f0, a_ring_s, a_slot_bytes, swz,
+                                              ctl, a, parts > 1);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[a.idx]));
                 a.advance(n_a);
