@@ -198,6 +198,7 @@ def run_ours(args, w):
     import torch
     import torch.distributed as dist
     import paper_2408_16551_b200 as tina
+    from paper_2408_16551_b200 import shard
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -262,10 +263,7 @@ def run_ours(args, w):
     launches = tina.launch_count() - launches0
     total_ms = e0.elapsed_time(e1)
     kern_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(total_ms, device="cuda")
     ms_per_step = total_ms / args.steps
     value = world * samples / (ms_per_step * 1e-3) / 1e9
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
@@ -283,10 +281,7 @@ def run_ours(args, w):
             tina.pfb_host(xp, w["P"], w["M"], wp, prec=w["prec"], out=outp)  # synchronous call
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = shard.max_over_ranks(dt, device="cuda")
         e2e = {"value": world * samples / dt / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": int(xp.numel() * xp.element_size() + wp.numel() * 4),
                "d2h_bytes_per_step": int(outp.numel() * 8), "ms_per_step": dt * 1e3, "steps": n_e2e}
