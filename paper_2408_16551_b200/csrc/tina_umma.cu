@@ -22,9 +22,12 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 
+#include <cstdlib>
+#include <cstring>
 #include <map>
 #include <mutex>
 #include <tuple>
+#include <vector>
 
 namespace tina {
 
@@ -35,21 +38,28 @@ constexpr int KC = 64;                   // K elements per pipeline chunk (one 1
 constexpr int NSUB = 256;                // columns per MMA instruction / B ring entry
 constexpr int NT_MAX = 512;              // accumulator columns per pass (all of TMEM)
 constexpr int A_PART_BYTES = BM * KC * 2;        // 16 KB
-constexpr int A_RING_BYTES = 64 * 1024;
+constexpr int A_RING_BYTES = 96 * 1024;      // 3 slots of hi+lo tiles (6 of hi only)
 constexpr int B_ENTRY_BYTES = NSUB * KC * 2;     // 32 KB
-constexpr int NB_RING = 4;
+constexpr int B_RING_BYTES = 96 * 1024;      // 6 half-tiles of 16 KB with cta_group::2: 1.5 chunks of twiddles in flight
 constexpr int UMMA_THREADS = 512;
-constexpr int PROD_WARP0 = 8, N_PROD_WARPS = 8, FPW = BM / N_PROD_WARPS;   // 16 frames per producer warp
-constexpr int EPI_WARP0 = 4;
+// Warp roles.  The SM's issue arbiter favours higher warp ids, so the latency-critical single-thread
+// roles (TMA, MMA) sit at the top and the throughput-bound FIR producers at the bottom.
+constexpr int PROD_WARP0 = 0, N_PROD_WARPS = 8, FPW = BM / N_PROD_WARPS;   // 16 frames per producer warp
+constexpr int EPI_WARP0 = 8;                // 4 warps; warp % 4 selects the TMEM lane quarter
+constexpr int TMA_WARP = 12, MMA_WARP = 13, ALLOC_WARP = 14;
+constexpr int UMMA_CG = 2;                  // CTAs per tcgen05 cta_group (2: CTA pair, M = 256 per MMA)
 constexpr int KSPLIT_MAX = 1024;            // longest accumulation chain kept in TMEM (K elements)
 
 struct SmemCtl {
-    uint64_t a_full[4], a_empty[4];
-    uint64_t b_full[NB_RING], b_empty[NB_RING];
+    uint64_t a_full[8], a_empty[8];
+    uint64_t b_full[8], b_empty[8];
     uint64_t t_full[2], t_empty[2];
     uint32_t tmem_base;
 };
-constexpr size_t UMMA_SMEM_BYTES = 1024 + A_RING_BYTES + NB_RING * B_ENTRY_BYTES + sizeof(SmemCtl);
+constexpr int EPI_LD = 36;                  // padded row length (floats) of the epilogue transpose tiles
+constexpr int EPI_STAGE_BYTES = 8192;        // per epilogue warp: two swizzled 32x32 fp32 tiles (TMA store) or one padded tile
+constexpr size_t UMMA_SMEM_BYTES = 1024 + A_RING_BYTES + B_RING_BYTES + 4 * EPI_STAGE_BYTES + sizeof(SmemCtl);
+static_assert(UMMA_SMEM_BYTES <= 232448, "exceeds the 227 KB shared memory opt-in limit");
 
 struct UmmaParams {
     const float* x;            // [S][stream_stride] floats
@@ -62,6 +72,9 @@ struct UmmaParams {
     int P, M;
     int tiles_per_stream, n_passes, total_work;
     int parts;                 // 2: bf16x3 (hi+lo), 1: single bf16 pass
+    unsigned long long* prof;  // optional [grid][16] cycle counters (TINA_PROF=1, diagnostics only)
+    int stagger;               // 1: delay cluster i by i/n of a chain period (desynchronises the TMEM drains)
+    int debug;                 // TINA_DEBUG_SKIP bits (1: no FIR work, 2: no epilogue global traffic, 4: no MMAs, 8: no TMA)
     int k_splits, kc_per_split; // accumulation chains per tile
 };
 
@@ -156,7 +169,7 @@ static tina_status get_plan(int P, bool real, bool inverse, int parts, cudaStrea
     if (!enc) { cudaFree(pl.tt); return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found"); }
     const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)parts * N};       // innermost (K) first
     const cuuint64_t strides[1] = {(cuuint64_t)N * sizeof(__nv_bfloat16)};
-    const cuuint32_t box[2] = {(cuuint32_t)KC, (cuuint32_t)(N < NSUB ? N : NSUB)};
+    const cuuint32_t box[2] = {(cuuint32_t)KC, (cuuint32_t)((N < NSUB ? N : NSUB) / UMMA_CG)};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(&pl.tmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, pl.tt, dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -207,188 +220,277 @@ __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v)
 {
     asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
 __device__ __forceinline__ float2 ldg_f2(const float* p)
 {
     return __ldg(reinterpret_cast<const float2*>(p));
 }
 
+template <int MT>
+struct FirRegs {
+    static constexpr int WA = MT > 0 ? MT : 1;
+    float2 tap[WA];
+    float2 row[WA - 1 + FPW];
+};
+
+// Issue every global load of one chunk: MT tap pairs and the FPW + MT - 1 input rows the warp touches.
 template <int MT, bool REAL, bool CHECK>
-__device__ __forceinline__ void fir_chunk(const UmmaParams& prm, const float* __restrict__ xc, int c0, long long f0,
-                                          uint32_t a_ring_s, uint32_t a_slot_bytes, const uint32_t (&swz)[8],
-                                          SmemCtl* ctl, const RingPos& a, bool split)
+__device__ __forceinline__ void fir_load(FirRegs<MT>& rg, const float* __restrict__ window, int P, int M,
+                                         long long K, long long nblk, const float* __restrict__ xc, int c0, long long f0)
 {
-    constexpr int WA = MT > 0 ? MT : 1;
-    const int M = prm.M;
-    const long long K = prm.K;
-    float2 tap[WA], row[WA - 1 + FPW];
-    // ---- all global loads first (taps, then the FPW + WA - 1 input rows this warp touches)
+    constexpr int WA = FirRegs<MT>::WA;
     if (MT > 0) {
+        const float* wp = window + (REAL ? c0 : (c0 >> 1));
 #pragma unroll
         for (int m = 0; m < WA; ++m) {
             if (m < M) {
-                if (REAL) tap[m] = ldg_f2(prm.window + (long long)m * prm.P + c0);
-                else { const float h = __ldg(prm.window + (long long)m * prm.P + (c0 >> 1)); tap[m] = make_float2(h, h); }
-            } else tap[m] = make_float2(0.f, 0.f);
+                if (REAL) rg.tap[m] = ldg_f2(wp);
+                else { const float h = __ldg(wp); rg.tap[m] = make_float2(h, h); }
+            } else rg.tap[m] = make_float2(0.f, 0.f);
+            wp += P;
         }
     }
-    {
-        const long long r0 = f0 + M - WA;                 // first row of the window of frame f0
-        const float* p = xc + r0 * K;
+    const long long r0 = f0 + M - WA;                 // first row of the window of frame f0
+    const float* p = xc + r0 * K;
 #pragma unroll
-        for (int j = 0; j < WA - 1 + FPW; ++j) {
-            if (CHECK) {
-                const long long r = r0 + j;
-                row[j] = (r >= 0 && r < prm.NBLK) ? ldg_f2(p) : make_float2(0.f, 0.f);
-            } else {
-                row[j] = ldg_f2(p);
-            }
-            p += K;
-        }
-    }
-    mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
-    const uint32_t slot = a_ring_s + a.idx * a_slot_bytes;
-    // ---- frame i uses rows i .. i + WA - 1 (row i + WA - 1 - m pairs with tap m)
-#pragma unroll
-    for (int i = 0; i < FPW; ++i) {
-        float2 y;
-        if (MT > 0) {
-            y = fmul2(tap[0], row[i + WA - 1]);
-#pragma unroll
-            for (int m = 1; m < WA; ++m) y = ffma2(tap[m], row[i + WA - 1 - m], y);
+    for (int j = 0; j < WA - 1 + FPW; ++j) {
+        if (CHECK) {
+            const long long r = r0 + j;
+            rg.row[j] = (r >= 0 && r < nblk) ? ldg_f2(p) : make_float2(0.f, 0.f);
         } else {
-            y = row[i];
+            rg.row[j] = ldg_f2(p);
         }
-        const __nv_bfloat162 hi = __floats2bfloat162_rn(y.x, y.y);
-        const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
-        const uint32_t addr = slot + swz[i & 7] + (uint32_t)i * 128u;
-        sts32(addr, hb);
-        if (split) {
-            const float lx = y.x - __uint_as_float(hb << 16);
-            const float ly = y.y - __uint_as_float(hb & 0xffff0000u);
-            const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
-            sts32(addr + A_PART_BYTES, *reinterpret_cast<const uint32_t*>(&lo));
+        p += K;
+    }
+}
+
+// Polyphase MAC of the FPW frames held in registers, split into bf16 hi / lo, swizzled store.
+// Frame i uses rows i .. i + WA - 1 (row i + WA - 1 - m pairs with tap m).  Four frames are
+// advanced together so that four independent FMA chains are in flight.
+template <int MT>
+__device__ __forceinline__ void fir_compute_store(const FirRegs<MT>& rg, uint32_t slot, const uint32_t (&swz)[8], bool split)
+{
+    constexpr int WA = FirRegs<MT>::WA;
+    constexpr int FG = 8;                  // frames advanced together (independent FMA chains in flight)
+#pragma unroll
+    for (int i0 = 0; i0 < FPW; i0 += FG) {
+        float2 y[FG];
+        if (MT > 0) {
+#pragma unroll
+            for (int g = 0; g < FG; ++g) y[g] = fmul2(rg.tap[0], rg.row[i0 + g + WA - 1]);
+#pragma unroll
+            for (int m = 1; m < WA; ++m)
+#pragma unroll
+                for (int g = 0; g < FG; ++g) y[g] = ffma2(rg.tap[m], rg.row[i0 + g + WA - 1 - m], y[g]);
+        } else {
+#pragma unroll
+            for (int g = 0; g < FG; ++g) y[g] = rg.row[i0 + g];
+        }
+#pragma unroll
+        for (int g = 0; g < FG; ++g) {
+            const int i = i0 + g;
+            const __nv_bfloat162 hi = __floats2bfloat162_rn(y[g].x, y[g].y);
+            const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
+            const uint32_t addr = slot + swz[i & 7] + (uint32_t)i * 128u;
+            sts32(addr, hb);
+            if (split) {
+                const float lx = y[g].x - __uint_as_float(hb << 16);
+                const float ly = y[g].y - __uint_as_float(hb & 0xffff0000u);
+                const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
+                sts32(addr + A_PART_BYTES, *reinterpret_cast<const uint32_t*>(&lo));
+            }
         }
     }
-    fence_proxy_async();
+}
+
+// tcgen05.commit: arrive on `bar` in this CTA (cta_group::1) or in both CTAs of the pair (::2)
+template <int CG>
+__device__ __forceinline__ void commit_cg(uint32_t bar)
+{
+    if (CG == 1) umma_commit(bar); else umma_commit_mc(bar, (uint16_t)3);
+}
+// arrive on a barrier the leader CTA waits on (remote arrive from the peer of a cta_group::2 pair)
+template <int CG>
+__device__ __forceinline__ void arrive_leader(uint32_t bar, uint32_t rank)
+{
+    if (CG == 1 || rank == 0) mbar_arrive(bar); else mbar_arrive_cluster(bar, 0);
 }
 
 // =====================================================================================
 // The fused kernel.  MT = compile-time tap count the sliding window is unrolled for
 // (taps m >= M are zero; MT == 0: no window, y = x, i.e. a plain DFT batch).
 // =====================================================================================
-template <int MT, bool REAL>
+template <int MT, bool REAL, int CG>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
-pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm)
+pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_out,
+                const UmmaParams prm)
 {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     uint8_t* a_ring = smem;
     uint8_t* b_ring = smem + A_RING_BYTES;
-    SmemCtl* ctl = reinterpret_cast<SmemCtl*>(b_ring + NB_RING * B_ENTRY_BYTES);
+    uint8_t* stage = b_ring + B_RING_BYTES;                         // 4 epilogue warps x EPI_STAGE_BYTES (1024-aligned)
+    SmemCtl* ctl = reinterpret_cast<SmemCtl*>(stage + 4 * EPI_STAGE_BYTES);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int parts = prm.parts;
     const uint32_t a_slot_bytes = A_PART_BYTES * parts;
-    const uint32_t n_a = A_RING_BYTES / a_slot_bytes;            // 2 (bf16x3) or 4 (single pass)
+    const uint32_t n_a = A_RING_BYTES / a_slot_bytes;            // 4 (bf16x3) or 8 (single pass)
     const int N = prm.K;
     const int n_kc = prm.K / KC;
     const int nt_max = N < NT_MAX ? N : NT_MAX;
     const uint32_t n_acc = nt_max <= 256 ? 2 : 1;                 // TMEM accumulator stages
-    const uint32_t b_box_bytes = (uint32_t)(N < NSUB ? N : NSUB) * KC * 2;
+    // cta_group::2: the CTA pair shares every twiddle tile (each CTA stages half of its N rows) and
+    // the leader (rank 0) issues M=256 MMAs over both CTAs' A tiles; barriers the leader waits on
+    // live in the leader's shared memory and are signalled remotely by the peer.
+    const uint32_t rank = CG == 2 ? cluster_ctarank() : 0;
+    const int cl = blockIdx.x / CG, n_cl = gridDim.x / CG;      // cluster id / number of clusters
+    constexpr uint32_t B_ENTRY = B_ENTRY_BYTES / CG;             // bytes per B ring entry in this CTA
+    constexpr uint32_t N_B = B_RING_BYTES / B_ENTRY;              // ring entries
+    const uint32_t b_box_bytes = (uint32_t)(N < NSUB ? N : NSUB) / CG * KC * 2;   // bytes one TMA box delivers
 
-    if (warp == 0 && lane == 0) {
+    if (warp == TMA_WARP && lane == 0) {
         prefetch_tmap(&tmap_b);
-        for (int i = 0; i < 4; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS); mbar_init(smem_u32(&ctl->a_empty[i]), 1); }
-        for (int i = 0; i < NB_RING; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4); }
+        if (!REAL) prefetch_tmap(&tmap_out);
+        // a_full: this CTA's 8 producer warps (+ in the leader one forwarded arrival from the peer's warp 1)
+        for (int i = 0; i < 8; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), 1); }
+        for (int i = 0; i < (int)N_B; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
         fence_mbar_init();
     }
-    if (warp == 2) {
-        tmem_alloc<1>(smem_u32(&ctl->tmem_base), 512);
-        tmem_relinquish<1>();
+    if (warp == ALLOC_WARP) {
+        tmem_alloc<CG>(smem_u32(&ctl->tmem_base), 512);
+        tmem_relinquish<CG>();
     }
     tc_fence_before();
-    __syncthreads();
+    if (CG == 2) cluster_sync(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = ctl->tmem_base;
 
-    if (warp == 0) {
+    if (warp == TMA_WARP) {
         // ============================ TMA producer: twiddle tiles ============================
         if (lane == 0) {
             RingPos b;
-            for (int w = blockIdx.x; w < prm.total_work; w += gridDim.x) {
+            for (int w = cl; w < prm.total_work; w += n_cl) {
                 const int n0 = (w % prm.n_passes) * NT_MAX;
                 const int nt = min(NT_MAX, N - n0);
                 const int n_sub = (nt + NSUB - 1) / NSUB;
                 for (int kc = 0; kc < n_kc; ++kc)
-                    for (int nh = 0; nh < n_sub; ++nh)
+                    for (int nh = 0; nh < n_sub; ++nh) {
+                        const int nw = min(NSUB, nt - nh * NSUB);
                         for (int part = 0; part < parts; ++part) {
                             mbar_wait(smem_u32(&ctl->b_empty[b.idx]), b.phase ^ 1);
                             const uint32_t bar = smem_u32(&ctl->b_full[b.idx]);
-                            mbar_expect_tx(bar, b_box_bytes);
-                            tma_load_2d(smem_u32(b_ring + b.idx * B_ENTRY_BYTES), &tmap_b, bar,
-                                        kc * KC, part * N + n0 + nh * NSUB);
-                            b.advance(NB_RING);
+                            const uint32_t dst = smem_u32(b_ring + b.idx * B_ENTRY);
+                            const int row = part * N + n0 + nh * NSUB + (int)rank * (nw / CG);
+                            if (prm.debug & 8) { if (rank == 0) mbar_arrive(bar); }
+                            else if (CG == 1) {
+                                mbar_expect_tx(bar, b_box_bytes);
+                                tma_load_2d(dst, &tmap_b, bar, kc * KC, row);
+                            } else {
+                                if (rank == 0) mbar_expect_tx(bar, 2 * b_box_bytes);
+                                tma_load_2d_cg2(dst, &tmap_b, mapa_u32(bar, 0), kc * KC, row);
+                            }
+                            b.advance(N_B);
                         }
+                    }
             }
         }
-    } else if (warp == 1) {
+    } else if (warp == MMA_WARP) {
         // ============================ MMA issuer ============================================
+        // (cta_group::2: only the leader CTA issues; the peer's warp 1 forwards "my A tile is ready"
+        //  to the leader's barrier, one remote arrive per chunk instead of one per producer warp)
+        if (CG == 2 && rank != 0) {
+            RingPos a;
+            for (int w = cl; w < prm.total_work; w += n_cl)
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                    if (lane == 0) mbar_arrive_cluster(smem_u32(&ctl->a_full[a.idx]), 0);
+                    __syncwarp();
+                    a.advance(n_a);
+                }
+        }
+        if (CG == 1 || rank == 0) {
         RingPos a, b, t;
-        for (int w = blockIdx.x; w < prm.total_work; w += gridDim.x) {
+        long long pf_a = 0, pf_b = 0, pf_t = 0, pf_tot = clock64(), pf_c;
+        // Stagger the clusters across one accumulation-chain period.  Every cluster does identical
+        // work, so without this all 148 SMs drain their TMEM tiles (38 MB + the read-modify-write
+        // traffic) in the same few microseconds and the epilogue becomes HBM-burst bound.
+        if (prm.stagger) {
+            const int n_sub_max = (nt_max + NSUB - 1) / NSUB;
+            const long long chain = (long long)prm.kc_per_split * n_sub_max * (KC / 16) * (parts > 1 ? 3 : 1) * 128;
+            const long long delay = chain * cl / n_cl;
+            const long long t0 = clock64();
+            while (clock64() - t0 < delay) { }
+        }
+#define PF_BEGIN() (pf_c = clock64())
+#define PF_END(acc) (acc += clock64() - pf_c)
+        uint32_t te_bits = 0;                                  // phase bit per 256-column TMEM block
+        for (int w = cl; w < prm.total_work; w += n_cl) {
             const int n0 = (w % prm.n_passes) * NT_MAX;
             const int nt = min(NT_MAX, N - n0);
             const int n_sub = (nt + NSUB - 1) / NSUB;
             for (int ks = 0; ks < prm.k_splits; ++ks) {
-            mbar_wait(smem_u32(&ctl->t_empty[t.idx]), t.phase ^ 1);
-            tc_fence_after();
-            const uint32_t d_base = tmem_base + t.idx * 256;
+            const uint32_t blk0 = n_acc == 2 ? t.idx : 0;          // first 256-column TMEM block of this chain
+            const uint32_t d_base = tmem_base + blk0 * 256;
             const int kc_begin = ks * prm.kc_per_split, kc_end = min(n_kc, kc_begin + prm.kc_per_split);
             for (int kc = kc_begin; kc < kc_end; ++kc) {
-                mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                PF_BEGIN(); mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase); PF_END(pf_a);
                 tc_fence_after();
                 const uint32_t a_hi = smem_u32(a_ring + a.idx * a_slot_bytes);
                 const uint32_t a_lo = a_hi + A_PART_BYTES;
                 for (int nh = 0; nh < n_sub; ++nh) {
                     const int nw = min(NSUB, nt - nh * NSUB);
-                    const uint32_t idesc = idesc_bf16(BM, nw);
+                    const uint32_t idesc = idesc_bf16(BM * CG, nw);
                     const uint32_t d = d_base + nh * NSUB;
+                    if (kc == kc_begin) {
+                        // first write into this TMEM block: wait until the epilogue has drained it
+                        PF_BEGIN(); mbar_wait(smem_u32(&ctl->t_empty[blk0 + nh]), ((te_bits >> (blk0 + nh)) & 1u) ^ 1u); PF_END(pf_t);
+                        te_bits ^= 1u << (blk0 + nh);
+                        tc_fence_after();
+                    }
                     // ---- B_hi: (A_lo x B_hi) then (A_hi x B_hi)
-                    mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase);
+                    PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); PF_END(pf_b);
                     tc_fence_after();
                     if (lane == 0) {
-                        const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * B_ENTRY_BYTES));
+                        const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * B_ENTRY));
                         uint32_t acc = kc > kc_begin;
+                        if (prm.debug & 4) { } else
                         if (parts > 1) {
                             const uint64_t ad = smem_desc_sw128(a_lo);
 #pragma unroll
-                            for (int k = 0; k < KC / 16; ++k) { umma_bf16<1>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                            for (int k = 0; k < KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
                         }
                         const uint64_t ad = smem_desc_sw128(a_hi);
+                        if (!(prm.debug & 4))
 #pragma unroll
-                        for (int k = 0; k < KC / 16; ++k) { umma_bf16<1>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
-                        umma_commit(smem_u32(&ctl->b_empty[b.idx]));
+                        for (int k = 0; k < KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                        commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]));
                     }
                     __syncwarp();
-                    b.advance(NB_RING);
+                    b.advance(N_B);
                     // ---- B_lo: (A_hi x B_lo)
                     if (parts > 1) {
-                        mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase);
+                        PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); PF_END(pf_b);
                         tc_fence_after();
                         if (lane == 0) {
-                            const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * B_ENTRY_BYTES));
+                            const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * B_ENTRY));
                             const uint64_t ad = smem_desc_sw128(a_hi);
+                            if (!(prm.debug & 4))
 #pragma unroll
-                            for (int k = 0; k < KC / 16; ++k) umma_bf16<1>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
-                            umma_commit(smem_u32(&ctl->b_empty[b.idx]));
+                            for (int k = 0; k < KC / 16; ++k) umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
+                            commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]));
                         }
                         __syncwarp();
-                        b.advance(NB_RING);
+                        b.advance(N_B);
                     }
                 }
                 if (lane == 0) {
-                    umma_commit(smem_u32(&ctl->a_empty[a.idx]));
-                    if (kc == kc_end - 1) umma_commit(smem_u32(&ctl->t_full[t.idx]));
+                    commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]));
+                    if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[t.idx]));
                 }
                 __syncwarp();
                 a.advance(n_a);
@@ -396,78 +498,163 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm
             t.advance(n_acc);
             }
         }
+        if (prm.prof && lane == 0) {
+            unsigned long long* pp = prm.prof + blockIdx.x * 16;
+            pp[0] = clock64() - pf_tot; pp[1] = pf_a; pp[2] = pf_b; pp[3] = pf_t;
+        }
+        }
     } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
-        // ============================ epilogue: TMEM -> global ==============================
+        // ============================ epilogue: TMEM -> smem transpose -> global =============
+        // tcgen05.ld hands each lane one accumulator ROW; a row-per-lane global store touches 32
+        // cache lines per instruction.  Each warp therefore bounces its 32x32 block through a
+        // padded shared-memory tile and stores it with 128-byte-contiguous row segments
+        // (4 rows x 128 B per float4 instruction; 2 rows x 128 B per float2 for the real kind,
+        // whose rows are only 8-byte aligned).  Later accumulation chains add into the output.
         const int q = warp - EPI_WARP0;
+        float* stg = reinterpret_cast<float*>(stage + q * EPI_STAGE_BYTES);
+        const uint32_t sbuf = smem_u32(stg);
         RingPos t;
-        for (int w = blockIdx.x; w < prm.total_work; w += gridDim.x) {
+        long long pe_w = 0, pe_tot = clock64(), pe_x, pe_ld = 0, pe_sts = 0, pe_st = 0, pe_fo = 0, pe_sy = 0;
+        for (int w = cl; w < prm.total_work; w += n_cl) {
             const int tile = w / prm.n_passes;
             const int n0 = (w % prm.n_passes) * NT_MAX;
             const int nt = min(NT_MAX, N - n0);
             const int s = tile / prm.tiles_per_stream;
-            const long long row = (long long)(tile % prm.tiles_per_stream) * BM + q * 32 + lane;
-            const bool valid = row < prm.F;
-            float* orow = prm.out + ((long long)s * prm.F + row) * prm.out_row;
+            const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + q * 32;
+            float* obase = prm.out + ((long long)s * prm.F + row0) * prm.out_row + n0;
+            const int rows_valid = (prm.debug & 2) ? 0 : (int)min(32LL, prm.F - row0);   // <= 0: nothing to store
             for (int ks = 0; ks < prm.k_splits; ++ks) {
-                mbar_wait(smem_u32(&ctl->t_full[t.idx]), t.phase);
+                pe_x = clock64(); mbar_wait(smem_u32(&ctl->t_full[t.idx]), t.phase); pe_w += clock64() - pe_x;
                 tc_fence_after();
-                const uint32_t taddr = tmem_base + t.idx * 256 + ((uint32_t)(q * 32) << 16);
-                for (int cb = 0; cb < nt; cb += 32) {
+                const uint32_t blk0 = n_acc == 2 ? t.idx : 0;
+                const uint32_t taddr = tmem_base + blk0 * 256 + ((uint32_t)(q * 32) << 16);
+                if (!REAL) {
+                    // Complex kind: rows are 16-byte aligned, so the tile leaves through the TMA engine.
+                    // Each 32x32 block is written (bank-conflict free, 128-byte swizzle) into one of two
+                    // 4 KB staging tiles and stored -- or, for later accumulation chains, add-reduced in
+                    // fp32 at L2 -- by one bulk tensor instruction; rows >= F are clipped by the tensor map.
+                    if (ks > 0 && lane == 0) bulk_wait<0>();     // the previous chain's stores to this tile are complete
                     uint32_t r[32];
-                    tmem_ld32(taddr + cb, r);
-                    tmem_ld_wait();
-                    if (valid) {
-                        const int n = n0 + cb;
-                        float4* o4 = reinterpret_cast<float4*>(orow + n);     // complex rows are 16-byte aligned
-                        float2* o2 = reinterpret_cast<float2*>(orow + n);     // real rows only 8-byte aligned
-                        if (ks > 0) {
-                            // later accumulation chains: out += chain (fp32 round-to-nearest add)
-                            if (REAL) {
+                    tmem_ld32(taddr, r);
+                    uint32_t buf = 0;
+                    for (int cb = 0; cb < nt; cb += 32) {
+                        tmem_ld_wait();
+                        if (lane == 0) bulk_wait_read<1>();      // the tile issued two blocks ago has been read
+                        __syncwarp();
+                        const uint32_t tile_s = sbuf + buf * 4096u;
+                        const uint32_t dst = tile_s + (uint32_t)lane * 128u;
 #pragma unroll
-                                for (int j = 0; j < 16; ++j) {
-                                    const float2 o = o2[j];
-                                    r[2 * j] = __float_as_uint(o.x + __uint_as_float(r[2 * j]));
-                                    r[2 * j + 1] = __float_as_uint(o.y + __uint_as_float(r[2 * j + 1]));
-                                }
-                            } else {
-#pragma unroll
-                                for (int j = 0; j < 8; ++j) {
-                                    const float4 o = o4[j];
-                                    r[4 * j] = __float_as_uint(o.x + __uint_as_float(r[4 * j]));
-                                    r[4 * j + 1] = __float_as_uint(o.y + __uint_as_float(r[4 * j + 1]));
-                                    r[4 * j + 2] = __float_as_uint(o.z + __uint_as_float(r[4 * j + 2]));
-                                    r[4 * j + 3] = __float_as_uint(o.w + __uint_as_float(r[4 * j + 3]));
-                                }
-                            }
+                        for (int j = 0; j < 8; ++j)
+                            sts128(dst + (((uint32_t)j ^ ((uint32_t)lane & 7u)) << 4), r[4 * j], r[4 * j + 1], r[4 * j + 2], r[4 * j + 3]);
+                        if (cb + 32 < nt) tmem_ld32(taddr + cb + 32, r);
+                        fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0 && !(prm.debug & 2)) {
+                            if (ks == 0) tma_store_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
+                            else         tma_reduce_add_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
+                            bulk_commit();
                         }
-                        if (REAL) {
-                            if (n == 0) {
-                                // columns 0 / 1 carry Re X[0] and Re X[P/2]; both bins are purely real
-                                float2* ny = reinterpret_cast<float2*>(orow + prm.P);
-                                float nyq = __uint_as_float(r[1]);
-                                if (ks > 0) nyq += ny->x;                     // out[1] == 0 was added above: r[1] is still the chain value
-                                *ny = make_float2(nyq, 0.f);
-                                r[1] = 0u;
-                            }
-#pragma unroll
-                            for (int j = 0; j < 16; ++j)
-                                o2[j] = make_float2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
-                        } else {
-#pragma unroll
-                            for (int j = 0; j < 8; ++j)
-                                o4[j] = make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
-                                                    __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
+                        buf ^= 1u;
+                        if ((cb & 255) == 224 || cb + 32 >= nt) {
+                            if ((cb & 255) == 224 && cb + 32 < nt) tmem_ld_wait();
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[blk0 + (cb >> 8)]), rank);
                         }
                     }
+                    t.advance(n_acc);
+                    continue;
                 }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&ctl->t_empty[t.idx]));
+                // lane -> (row, column) of the transposed (coalesced) global access pattern
+                constexpr int NV = REAL ? 16 : 8;                     // accesses per lane per 32-column block
+                constexpr int RSTEP = REAL ? 2 : 4;
+                const int c = REAL ? 2 * (lane & 15) : 4 * (lane & 7);
+                const int rbase = REAL ? (lane >> 4) : (lane >> 3);
+                float* const gp0 = obase + (long long)rbase * prm.out_row + c;
+                const long long gstep = (long long)RSTEP * prm.out_row;
+                float4 o4[REAL ? 1 : 8];
+                float2 o2[REAL ? 16 : 1];
+                float nyq_old[REAL ? 16 : 1];
+                // later chains: the running sums of a block are fetched one block ahead
+                auto fetch_old = [&](int cb) {
+                    const bool special = REAL && (n0 + cb == 0) && c == 0;
+#pragma unroll
+                    for (int i = 0; i < NV; ++i) {
+                        if (rbase + RSTEP * i < rows_valid) {
+                            const float* g = gp0 + cb + i * gstep;
+                            if (REAL) {
+                                o2[i] = *reinterpret_cast<const float2*>(g);
+                                if (special) nyq_old[i] = *(g + prm.P);
+                            } else {
+                                o4[i] = *reinterpret_cast<const float4*>(g);
+                            }
+                        }
+                    }
+                };
+                uint32_t r[32];
+                if (ks > 0) fetch_old(0);
+                tmem_ld32(taddr, r);
+                for (int cb = 0; cb < nt; cb += 32) {
+                    const bool special = REAL && (n0 + cb == 0) && c == 0;   // columns 0 / 1 = Re X[0], Re X[P/2]
+                    pe_x = clock64(); tmem_ld_wait(); pe_ld += clock64() - pe_x; pe_x = clock64();
+#pragma unroll
+                    for (int j = 0; j < 8; ++j)
+                        *reinterpret_cast<float4*>(stg + lane * EPI_LD + 4 * j) =
+                            make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
+                                        __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
+                    // the next block's TMEM read overlaps this block's transpose and stores
+                    if (cb + 32 < nt) tmem_ld32(taddr + cb + 32, r);
+                    __syncwarp();
+                    pe_sts += clock64() - pe_x; pe_x = clock64();
+#pragma unroll
+                    for (int i = 0; i < NV; ++i) {
+                        const int rr = rbase + RSTEP * i;
+                        if (rr < rows_valid) {
+                            float* g = gp0 + cb + i * gstep;
+                            if (REAL) {
+                                float2 v = *reinterpret_cast<const float2*>(stg + rr * EPI_LD + c);
+                                if (special) {
+                                    if (ks > 0) { v.x += o2[i].x; v.y += nyq_old[i]; }
+                                    *reinterpret_cast<float2*>(g + prm.P) = make_float2(v.y, 0.f);   // out[P], out[P+1]
+                                    v.y = 0.f;
+                                } else if (ks > 0) {
+                                    v.x += o2[i].x; v.y += o2[i].y;
+                                }
+                                *reinterpret_cast<float2*>(g) = v;
+                            } else {
+                                float4 v = *reinterpret_cast<const float4*>(stg + rr * EPI_LD + c);
+                                if (ks > 0) { v.x += o4[i].x; v.y += o4[i].y; v.z += o4[i].z; v.w += o4[i].w; }
+                                *reinterpret_cast<float4*>(g) = v;
+                            }
+                        }
+                    }
+                    pe_st += clock64() - pe_x; pe_x = clock64();
+                    if (ks > 0 && cb + 32 < nt) fetch_old(cb + 32);
+                    pe_fo += clock64() - pe_x; pe_x = clock64();
+                    __syncwarp();
+                    pe_sy += clock64() - pe_x;
+                    if ((cb & 255) == 224 || cb + 32 >= nt) {
+                        // a 256-column TMEM block has been read out (the read of the following block,
+                        // if any, is already in flight): hand it back to the MMA warp
+                        if ((cb & 255) == 224 && cb + 32 < nt) tmem_ld_wait();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[blk0 + (cb >> 8)]), rank);
+                    }
+                }
                 t.advance(n_acc);
             }
         }
-    } else if (warp >= PROD_WARP0) {
+        if (!REAL && lane == 0) bulk_wait<0>();                  // staging tiles must outlive their TMA reads
+        if (prm.prof && q == 0 && lane == 0) {
+            unsigned long long* pp = prm.prof + blockIdx.x * 16;
+            pp[8] = clock64() - pe_tot; pp[9] = pe_w; pp[10] = pe_ld; pp[11] = pe_sts; pp[12] = pe_st; pp[13] = pe_fo; pp[14] = pe_sy;
+        }
+    } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ FIR producers =========================================
+        // Software pipeline over the flattened (work item, K chunk) sequence: the loads of chunk
+        // c+1 are issued right after the arithmetic of chunk c and before its fence / arrive, so
+        // their latency (and the fence's) overlaps the hand-off and the wait for the next slot.
         const int pw = warp - PROD_WARP0;
         const uint32_t a_ring_s = smem_u32(a_ring);
         // byte offset of this lane's 4-byte cell in row 0 of an A tile, for each swizzle phase (row & 7):
@@ -476,32 +663,61 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const UmmaParams prm
 #pragma unroll
         for (int j = 0; j < 8; ++j)
             swz[j] = (uint32_t)(pw * FPW) * 128u + ((((uint32_t)lane >> 2) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 3u) * 4u;
+        constexpr int WA = MT > 0 ? MT : 1;
+        const float* const window = prm.window;
+        const int P = prm.P, M = prm.M;
+        const long long K = prm.K, nblk = prm.NBLK;
+        const bool split = parts > 1;
+        FirRegs<MT> rg;
         RingPos a;
-        for (int w = blockIdx.x; w < prm.total_work; w += gridDim.x) {
-            const int tile = w / prm.n_passes;
+        int w = cl, kc = 0;
+        const float* xs = nullptr;
+        long long f0 = 0;
+        bool interior = false;
+        auto set_tile = [&](int ww) {
+            const int tile = ww / prm.n_passes;
             const int s = tile / prm.tiles_per_stream;
-            const long long f0 = (long long)(tile % prm.tiles_per_stream) * BM + pw * FPW;
-            const float* xs = prm.x + (long long)s * prm.stream_stride + 2 * lane;
+            f0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + pw * FPW;
+            xs = prm.x + (long long)s * prm.stream_stride + 2 * lane;
             // rows f0 + M - WA .. f0 + FPW + M - 2 are touched; interior tiles need no bounds checks
-            constexpr int WA = MT > 0 ? MT : 1;
-            const bool interior = (f0 + prm.M - WA >= 0) && (f0 + FPW + prm.M - 1 <= prm.NBLK);
-            for (int kc = 0; kc < n_kc; ++kc) {
-                if (interior)
-                    fir_chunk<MT, REAL, false>(prm, xs + kc * KC, kc * KC + 2 * lane, f0, a_ring_s, a_slot_bytes, swz,
-                                               ctl, a, parts > 1);
-                else
-                    fir_chunk<MT, REAL, true>(prm, xs + kc * KC, kc * KC + 2 * lane, f0, a_ring_s, a_slot_bytes, swz,
-                                              ctl, a, parts > 1);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[a.idx]));
-                a.advance(n_a);
+            interior = (f0 + M - WA >= 0) && (f0 + FPW + M - 1 <= nblk);
+        };
+        auto load = [&](int kk) {
+            if (prm.debug & 1) return;
+            if (interior) fir_load<MT, REAL, false>(rg, window, P, M, K, nblk, xs + kk * KC, kk * KC + 2 * lane, f0);
+            else          fir_load<MT, REAL, true>(rg, window, P, M, K, nblk, xs + kk * KC, kk * KC + 2 * lane, f0);
+        };
+        long long pq_w = 0, pq_c = 0, pq_f = 0, pq_tot = clock64(), pq_x;
+        bool have = w < prm.total_work;
+        if (have) { set_tile(w); load(0); }
+        while (have) {
+            int w2 = w, kc2 = kc + 1;
+            if (kc2 == n_kc) { kc2 = 0; w2 += n_cl; }
+            const bool have2 = w2 < prm.total_work;
+            pq_x = clock64(); mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1); pq_w += clock64() - pq_x;
+            pq_x = clock64();
+            if (!(prm.debug & 1)) fir_compute_store<MT>(rg, a_ring_s + a.idx * a_slot_bytes, swz, split);
+            if (have2) {
+                if (kc2 == 0) set_tile(w2);
+                load(kc2);
             }
+            pq_c += clock64() - pq_x; pq_x = clock64();
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[a.idx]));
+            pq_f += clock64() - pq_x;
+            a.advance(n_a);
+            w = w2; kc = kc2; have = have2;
+        }
+        if (prm.prof && pw == 0 && lane == 0) {
+            unsigned long long* pp = prm.prof + blockIdx.x * 16;
+            pp[4] = clock64() - pq_tot; pp[5] = pq_w; pp[6] = pq_c; pp[7] = pq_f;
         }
     }
 
     tc_fence_before();
-    __syncthreads();
-    if (warp == 2) tmem_dealloc<1>(tmem_base, 512);
+    if (CG == 2) cluster_sync(); else __syncthreads();   // the peer's smem / barriers stay live until both are done
+    if (warp == ALLOC_WARP) tmem_dealloc<CG>(tmem_base, 512);
 }
 
 // =====================================================================================
@@ -514,18 +730,45 @@ bool umma_supported(int P, bool real)
 }
 
 template <int MT, bool REAL>
-static tina_status launch_umma(const CUtensorMap& tmap, const UmmaParams& prm, int grid, cudaStream_t st)
+static tina_status launch_umma(const CUtensorMap& tmap, const CUtensorMap& tmap_out, const UmmaParams& prm, int grid,
+                               cudaStream_t st)
 {
+    auto kern = pfb_umma_kernel<MT, REAL, UMMA_CG>;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(pfb_umma_kernel<MT, REAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)UMMA_SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UMMA_SMEM_BYTES);
         if (e != cudaSuccess) return check_cuda(e, "cudaFuncSetAttribute(pfb_umma_kernel)");
         attr_done = true;
     }
-    pfb_umma_kernel<MT, REAL><<<grid, UMMA_THREADS, UMMA_SMEM_BYTES, st>>>(tmap, prm);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(UMMA_THREADS);
+    cfg.dynamicSmemBytes = UMMA_SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = UMMA_CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    UmmaParams prm2 = prm;
+    const bool prof = getenv("TINA_PROF") != nullptr;
+    if (prof) { cudaMalloc(&prm2.prof, (size_t)grid * 16 * 8); cudaMemsetAsync(prm2.prof, 0, (size_t)grid * 16 * 8, st); }
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tmap, tmap_out, prm2);
+    if (prof) {
+        std::vector<unsigned long long> h((size_t)grid * 16);
+        cudaStreamSynchronize(st);
+        cudaMemcpy(h.data(), prm2.prof, h.size() * 8, cudaMemcpyDeviceToHost);
+        cudaFree(prm2.prof);
+        double acc[16] = {0};
+        for (int b = 0; b < grid; b += UMMA_CG) for (int i = 0; i < 16; ++i) acc[i] += (double)h[(size_t)b * 16 + i] / (grid / UMMA_CG);
+        fprintf(stderr, "[tina prof] leader CTA mean cycles: mma tot %.0f a_full %.0f b_full %.0f t_empty %.0f | prod tot %.0f a_empty %.0f work %.0f fence %.0f | epi tot %.0f t_full %.0f ldwait %.0f sts %.0f lds+stg %.0f fetch %.0f sync %.0f\n",
+                acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], acc[7], acc[8], acc[9], acc[10], acc[11], acc[12], acc[13], acc[14]);
+    }
     count_launch();
     g_last_path = kPathUmma;
+    if (e != cudaSuccess) return check_cuda(e, "pfb_umma_kernel launch");
     return check_cuda(cudaGetLastError(), "pfb_umma_kernel launch");
 }
 
@@ -565,13 +808,16 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     prm.K = K;
     prm.P = P;
     prm.M = M;
-    prm.tiles_per_stream = (int)((F + BM - 1) / BM);
+    prm.tiles_per_stream = (int)((F + BM * UMMA_CG - 1) / (BM * UMMA_CG));
     prm.n_passes = (K + NT_MAX - 1) / NT_MAX;
     const long long total = (long long)S * prm.tiles_per_stream * prm.n_passes;
     if (total > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: too many tiles");
     prm.total_work = (int)total;
     prm.parts = parts;
-    prm.k_splits = (K + KSPLIT_MAX - 1) / KSPLIT_MAX;
+    prm.prof = nullptr;
+    { const char* sg = getenv("TINA_STAGGER"); prm.stagger = sg ? atoi(sg) : 1; }
+    { const char* dbg = getenv("TINA_DEBUG_SKIP"); prm.debug = dbg ? atoi(dbg) : 0; }
+    { const char* ksm = getenv("TINA_KSPLIT"); const int kmax = ksm ? atoi(ksm) : KSPLIT_MAX; prm.k_splits = (K + kmax - 1) / kmax; }
     prm.kc_per_split = ((K / KC) + prm.k_splits - 1) / prm.k_splits;
 
     static int n_sm = 0;
@@ -581,10 +827,27 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
         cudaError_t e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "cudaDeviceGetAttribute(SM count)"); }
     }
-    const int grid = prm.total_work < n_sm ? prm.total_work : n_sm;
+    const int n_cl = n_sm / UMMA_CG;
+    const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
+
+    // Output tensor map for the TMA-store epilogue (complex kind only: its rows are 16-byte aligned).
+    CUtensorMap tmap_out;
+    memset(&tmap_out, 0, sizeof(tmap_out));
+    if (!real) {
+        EncodeTiledFn enc = encode_fn();
+        if (!enc) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+        const cuuint64_t dims[3] = {(cuuint64_t)K, (cuuint64_t)F, (cuuint64_t)S};
+        const cuuint64_t strides[2] = {(cuuint64_t)K * sizeof(float), (cuuint64_t)F * K * sizeof(float)};
+        const cuuint32_t box[3] = {32, 32, 1};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = enc(&tmap_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(out) failed (%d)", (int)r);
+    }
 
 #define TINA_LAUNCH(MT_)                                                                           \
-    (real ? launch_umma<MT_, true>(plan->tmap, prm, grid, st) : launch_umma<MT_, false>(plan->tmap, prm, grid, st))
+    (real ? launch_umma<MT_, true>(plan->tmap, tmap_out, prm, grid, st) : launch_umma<MT_, false>(plan->tmap, tmap_out, prm, grid, st))
     if (!window) return TINA_LAUNCH(0);
     if (M <= 4) return TINA_LAUNCH(4);
     if (M <= 8) return TINA_LAUNCH(8);
