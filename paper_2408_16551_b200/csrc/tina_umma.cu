@@ -73,6 +73,7 @@ struct UmmaParams {
     int tiles_per_stream, n_passes, total_work;
     int parts;                 // 2: bf16x3 (hi+lo), 1: single bf16 pass
     unsigned long long* prof;  // optional [grid][16] cycle counters (TINA_PROF=1, diagnostics only)
+    int out_tma;               // 1: epilogue leaves through TMA tensor stores (always for the complex kind)
     int stagger;               // 1: delay cluster i by i/n of a chain period (desynchronises the TMEM drains)
     int debug;                 // TINA_DEBUG_SKIP bits (1: no FIR work, 2: no epilogue global traffic, 4: no MMAs, 8: no TMA)
     int k_splits, kc_per_split; // accumulation chains per tile
@@ -326,7 +327,7 @@ __device__ __forceinline__ void arrive_leader(uint32_t bar, uint32_t rank)
 template <int MT, bool REAL, int CG>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_out,
-                const UmmaParams prm)
+                const __grid_constant__ CUtensorMap tmap_out2, const UmmaParams prm)
 {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -354,7 +355,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
 
     if (warp == TMA_WARP && lane == 0) {
         prefetch_tmap(&tmap_b);
-        if (!REAL) prefetch_tmap(&tmap_out);
+        if (prm.out_tma) { prefetch_tmap(&tmap_out); if (REAL) prefetch_tmap(&tmap_out2); }
         // a_full: this CTA's 8 producer warps (+ in the leader one forwarded arrival from the peer's warp 1)
         for (int i = 0; i < 8; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), 1); }
         for (int i = 0; i < (int)N_B; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 1); }
@@ -528,30 +529,70 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 tc_fence_after();
                 const uint32_t blk0 = n_acc == 2 ? t.idx : 0;
                 const uint32_t taddr = tmem_base + blk0 * 256 + ((uint32_t)(q * 32) << 16);
-                if (!REAL) {
-                    // Complex kind: rows are 16-byte aligned, so the tile leaves through the TMA engine.
-                    // Each 32x32 block is written (bank-conflict free, 128-byte swizzle) into one of two
-                    // 4 KB staging tiles and stored -- or, for later accumulation chains, add-reduced in
-                    // fp32 at L2 -- by one bulk tensor instruction; rows >= F are clipped by the tensor map.
+                if (prm.out_tma) {
+                    // The tile leaves through the TMA engine.  Each 32x32 block is written (bank-conflict
+                    // free, 128-byte swizzle) into one of two 4 KB staging tiles and stored -- or, for later
+                    // accumulation chains, add-reduced in fp32 at L2 -- by bulk tensor instructions; rows
+                    // >= F are clipped by the tensor map.  Complex kind: one 32-row box.  Real kind: rows
+                    // are only 8-byte aligned, but PAIRS of rows have a 16-byte-multiple pitch, so even
+                    // and odd rows go out as two 16-row boxes through two maps over row pairs.
                     if (ks > 0 && lane == 0) bulk_wait<0>();     // the previous chain's stores to this tile are complete
                     uint32_t r[32];
                     tmem_ld32(taddr, r);
                     uint32_t buf = 0;
+                    const uint32_t rr = REAL ? ((uint32_t)lane >> 1) : (uint32_t)lane;       // row within the staged box
+                    const bool odd = REAL && (lane & 1);
+                    float* const orow = obase + (long long)lane * prm.out_row;               // this lane's output row
                     for (int cb = 0; cb < nt; cb += 32) {
                         tmem_ld_wait();
+                        if (REAL && lane < rows_valid && !(prm.debug & 2)) {
+                            if (n0 + cb == 0) {
+                                // columns 0 / 1 carry Re X[0] and Re X[P/2]; Im X[0] = Im X[P/2] = 0
+                                float2* ny = reinterpret_cast<float2*>(orow + prm.P);
+                                float nyq = __uint_as_float(r[1]);
+                                if (ks > 0) nyq += ny->x;
+                                *ny = make_float2(nyq, 0.f);
+                                r[1] = 0u;
+                            }
+                            if (odd) {
+                                // odd rows start 8 bytes off a 16-byte boundary: their TMA box covers columns
+                                // cb+2 .. cb+29; the two edge pairs are stored from registers
+                                float2* e0 = reinterpret_cast<float2*>(orow + cb);           // (obase already points at column n0)
+                                float2* e1 = reinterpret_cast<float2*>(orow + cb + 30);
+                                float2 a = make_float2(__uint_as_float(r[0]), __uint_as_float(r[1]));
+                                float2 b = make_float2(__uint_as_float(r[30]), __uint_as_float(r[31]));
+                                if (ks > 0) { const float2 oa = *e0, ob = *e1; a.x += oa.x; a.y += oa.y; b.x += ob.x; b.y += ob.y; }
+                                *e0 = a; *e1 = b;
+                            }
+                        } else if (REAL && n0 + cb == 0) {
+                            r[1] = 0u;
+                        }
                         if (lane == 0) bulk_wait_read<1>();      // the tile issued two blocks ago has been read
                         __syncwarp();
                         const uint32_t tile_s = sbuf + buf * 4096u;
-                        const uint32_t dst = tile_s + (uint32_t)lane * 128u;
+                        if (!odd) {
+                            const uint32_t dst = tile_s + rr * 128u;
 #pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            sts128(dst + (((uint32_t)j ^ ((uint32_t)lane & 7u)) << 4), r[4 * j], r[4 * j + 1], r[4 * j + 2], r[4 * j + 3]);
+                            for (int j = 0; j < 8; ++j)
+                                sts128(dst + (((uint32_t)j ^ (rr & 7u)) << 4), r[4 * j], r[4 * j + 1], r[4 * j + 2], r[4 * j + 3]);
+                        } else {
+                            const uint32_t dst = tile_s + 2048u + rr * 112u;                 // dense 16 x 28 floats
+#pragma unroll
+                            for (int j = 0; j < 7; ++j)
+                                sts128(dst + 16u * j, r[4 * j + 2], r[4 * j + 3], r[4 * j + 4], r[4 * j + 5]);
+                        }
                         if (cb + 32 < nt) tmem_ld32(taddr + cb + 32, r);
                         fence_proxy_async();
                         __syncwarp();
                         if (lane == 0 && !(prm.debug & 2)) {
-                            if (ks == 0) tma_store_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
-                            else         tma_reduce_add_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
+                            if (!REAL) {
+                                if (ks == 0) tma_store_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
+                                else         tma_reduce_add_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
+                            } else {
+                                const int pr = (int)(row0 >> 1), c_odd = prm.P + 2 + n0 + cb + 2;
+                                if (ks == 0) { tma_store_3d(&tmap_out, tile_s, n0 + cb, pr, s); tma_store_3d(&tmap_out2, tile_s + 2048u, c_odd, pr, s); }
+                                else { tma_reduce_add_3d(&tmap_out, tile_s, n0 + cb, pr, s); tma_reduce_add_3d(&tmap_out2, tile_s + 2048u, c_odd, pr, s); }
+                            }
                             bulk_commit();
                         }
                         buf ^= 1u;
@@ -645,7 +686,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 t.advance(n_acc);
             }
         }
-        if (!REAL && lane == 0) bulk_wait<0>();                  // staging tiles must outlive their TMA reads
+        if (prm.out_tma && lane == 0) bulk_wait<0>();            // staging tiles must outlive their TMA reads
         if (prm.prof && q == 0 && lane == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
             pp[8] = clock64() - pe_tot; pp[9] = pe_w; pp[10] = pe_ld; pp[11] = pe_sts; pp[12] = pe_st; pp[13] = pe_fo; pp[14] = pe_sy;
@@ -730,8 +771,8 @@ bool umma_supported(int P, bool real)
 }
 
 template <int MT, bool REAL>
-static tina_status launch_umma(const CUtensorMap& tmap, const CUtensorMap& tmap_out, const UmmaParams& prm, int grid,
-                               cudaStream_t st)
+static tina_status launch_umma(const CUtensorMap& tmap, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
+                               const UmmaParams& prm, int grid, cudaStream_t st)
 {
     auto kern = pfb_umma_kernel<MT, REAL, UMMA_CG>;
     static bool attr_done = false;
@@ -755,7 +796,7 @@ static tina_status launch_umma(const CUtensorMap& tmap, const CUtensorMap& tmap_
     UmmaParams prm2 = prm;
     const bool prof = getenv("TINA_PROF") != nullptr;
     if (prof) { cudaMalloc(&prm2.prof, (size_t)grid * 16 * 8); cudaMemsetAsync(prm2.prof, 0, (size_t)grid * 16 * 8, st); }
-    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tmap, tmap_out, prm2);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tmap, tmap_out, tmap_out2, prm2);
     if (prof) {
         std::vector<unsigned long long> h((size_t)grid * 16);
         cudaStreamSynchronize(st);
@@ -830,24 +871,52 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     const int n_cl = n_sm / UMMA_CG;
     const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
 
-    // Output tensor map for the TMA-store epilogue (complex kind only: its rows are 16-byte aligned).
-    CUtensorMap tmap_out;
+    // Output tensor maps for the TMA-store epilogue.  Complex kind: [S][F][2P] floats, 32x32 boxes.
+    // Real kind: a row is P+2 floats (8-byte aligned only), so the maps run over row PAIRS, whose
+    // pitch (2P+4 floats) is a multiple of 16 bytes: one map sees the even rows (extent P+2 in x,
+    // ceil(F/2) pairs), the other the whole pair (extent 2P+4, floor(F/2) pairs) and is addressed at
+    // x >= P+2 for the odd rows.  Needs a 16-byte-multiple stream pitch (S == 1 or F even) and F >= 2;
+    // other real shapes use the register/shared-memory store path.
+    CUtensorMap tmap_out, tmap_out2;
     memset(&tmap_out, 0, sizeof(tmap_out));
-    if (!real) {
+    memset(&tmap_out2, 0, sizeof(tmap_out2));
+    prm.out_tma = real ? ((S == 1 || F % 2 == 0) && F >= 2) : 1;
+    if (getenv("TINA_NO_OUT_TMA") && real) prm.out_tma = 0;
+    if (prm.out_tma) {
         EncodeTiledFn enc = encode_fn();
         if (!enc) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
-        const cuuint64_t dims[3] = {(cuuint64_t)K, (cuuint64_t)F, (cuuint64_t)S};
-        const cuuint64_t strides[2] = {(cuuint64_t)K * sizeof(float), (cuuint64_t)F * K * sizeof(float)};
-        const cuuint32_t box[3] = {32, 32, 1};
         const cuuint32_t estr[3] = {1, 1, 1};
-        CUresult r = enc(&tmap_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                         CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        CUresult r;
+        if (!real) {
+            const cuuint64_t dims[3] = {(cuuint64_t)K, (cuuint64_t)F, (cuuint64_t)S};
+            const cuuint64_t strides[2] = {(cuuint64_t)K * sizeof(float), (cuuint64_t)F * K * sizeof(float)};
+            const cuuint32_t box[3] = {32, 32, 1};
+            r = enc(&tmap_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        } else {
+            const cuuint64_t row = (cuuint64_t)P + 2;
+            const cuuint64_t pitch2 = 2 * row * sizeof(float);
+            const cuuint64_t spitch = S > 1 ? (cuuint64_t)F * row * sizeof(float) : pitch2 * (cuuint64_t)((F + 1) / 2);
+            const cuuint64_t strides[2] = {pitch2, spitch};
+            const cuuint32_t box[3] = {32, 16, 1};
+            const cuuint64_t dims_e[3] = {row, (cuuint64_t)((F + 1) / 2), (cuuint64_t)S};
+            const cuuint64_t dims_o[3] = {2 * row, (cuuint64_t)(F / 2), (cuuint64_t)S};
+            r = enc(&tmap_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims_e, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            const cuuint32_t box_o[3] = {28, 16, 1};      // odd rows: columns +2 .. +29 of each block (16-byte aligned start)
+            if (r == CUDA_SUCCESS)
+                r = enc(&tmap_out2, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims_o, strides, box_o, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                        CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        }
         if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(out) failed (%d)", (int)r);
     }
 
 #define TINA_LAUNCH(MT_)                                                                           \
-    (real ? launch_umma<MT_, true>(plan->tmap, tmap_out, prm, grid, st) : launch_umma<MT_, false>(plan->tmap, tmap_out, prm, grid, st))
+    (real ? launch_umma<MT_, true>(plan->tmap, tmap_out, tmap_out2, prm, grid, st)                 \
+          : launch_umma<MT_, false>(plan->tmap, tmap_out, tmap_out2, prm, grid, st))
     if (!window) return TINA_LAUNCH(0);
     if (M <= 4) return TINA_LAUNCH(4);
     if (M <= 8) return TINA_LAUNCH(8);

@@ -169,6 +169,30 @@ def test_pfb_batched_streams_and_tail(tina, oracle):
         assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
 
 
+@pytest.mark.parametrize("P,M,F,S", [(128, 4, 130, 2), (128, 4, 129, 2), (2048, 2, 258, 2), (1024, 3, 131, 3)])
+def test_pfb_real_batched_epilogue_paths(tina, oracle, P, M, F, S):
+    """Real kind, several streams: even F takes the TMA-store epilogue (row-pair tensor maps), odd F
+    with S > 1 the register/shared-memory store path; P >= 1024 adds several accumulation chains
+    (read-modify-write of the output) and several column passes."""
+    case = ti.pfb_case(P, M, F, real=True, streams=S, seed=650 + P + F)
+    got = _run_pfb(tina, case)
+    assert got.shape == (S, F, P // 2 + 1)
+    for s in range(S):
+        ref = oracle.pfb(case.x[s], P, M, case.window)
+        assert rel_l2_rows(got[s], ref) <= TOL_FP32
+        assert np.all(got[s][:, 0].imag == 0) and np.all(got[s][:, P // 2].imag == 0)
+
+
+def test_pfb_complex_multichain_batched(tina, oracle):
+    """Complex kind, K = 4096: four accumulation chains (TMA add-reduce epilogue), 8 column passes,
+    ragged last tile, 2 streams."""
+    P, M, F, S = 2048, 2, 300, 2
+    case = ti.pfb_case(P, M, F, streams=S, seed=660)
+    got = _run_pfb(tina, case)
+    for s in range(S):
+        assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
+
+
 def test_pfb_m1_rect_is_blocked_dft(tina, oracle):
     import torch
     P, F = 128, 256
