@@ -46,7 +46,7 @@ constexpr int UMMA_THREADS = 512;
 // roles (TMA, MMA) sit at the top and the throughput-bound FIR producers at the bottom.
 constexpr int PROD_WARP0 = 0, N_PROD_WARPS = 8, FPW = BM / N_PROD_WARPS;   // 16 frames per producer warp
 constexpr int EPI_WARP0 = 8;                // 4 warps; warp % 4 selects the TMEM lane quarter
-constexpr int TMA_WARP = 12, MMA_WARP = 13, ALLOC_WARP = 14;
+constexpr int TMA_WARP = 12, MMA_WARP = 13, ALLOC_WARP = 14, MMA_WARP2 = 15;
 constexpr int UMMA_CG = 2;                  // CTAs per tcgen05 cta_group (2: CTA pair, M = 256 per MMA)
 constexpr int KSPLIT_MAX = 1024;            // longest accumulation chain kept in TMEM (K elements)
 
@@ -357,9 +357,9 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         prefetch_tmap(&tmap_b);
         if (prm.out_tma) { prefetch_tmap(&tmap_out); if (REAL) prefetch_tmap(&tmap_out2); }
         // a_full: this CTA's 8 producer warps (+ in the leader one forwarded arrival from the peer's warp 1)
-        for (int i = 0; i < 8; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), 1); }
+        for (int i = 0; i < 8; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), 2); }
         for (int i = 0; i < (int)N_B; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
+        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 2); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
         fence_mbar_init();
     }
     if (warp == ALLOC_WARP) {
@@ -400,11 +400,17 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     }
             }
         }
-    } else if (warp == MMA_WARP) {
-        // ============================ MMA issuer ============================================
-        // (cta_group::2: only the leader CTA issues; the peer's warp 1 forwards "my A tile is ready"
-        //  to the leader's barrier, one remote arrive per chunk instead of one per producer warp)
-        if (CG == 2 && rank != 0) {
+    } else if (warp == MMA_WARP || warp == MMA_WARP2) {
+        // ============================ MMA issuers ===========================================
+        // Two issuing warps, one per 256-column half of the accumulator tile (warp MMA_WARP: columns
+        // 0-255, MMA_WARP2: 256-511).  tcgen05.mma issue blocks on a short queue and every barrier
+        // wait / commit costs the issuing thread ~70-100 cycles in which it queues nothing; with two
+        // threads the tensor pipe always has the other half's MMAs to run.  Both wait on the same A
+        // slot, each consumes its own twiddle entries, and a_empty / t_full take one commit from each.
+        // (cta_group::2: only the leader CTA issues; the peer's MMA_WARP forwards "my A tile is ready"
+        //  to the leader's barrier, one remote arrive per chunk instead of one per producer warp.)
+        const int h = warp == MMA_WARP ? 0 : 1;
+        if (CG == 2 && rank != 0 && h == 0) {
             RingPos a;
             for (int w = cl; w < prm.total_work; w += n_cl)
                 for (int kc = 0; kc < n_kc; ++kc) {
@@ -415,18 +421,9 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 }
         }
         if (CG == 1 || rank == 0) {
-        RingPos a, b, t;
+        RingPos a, t;
+        uint32_t g = 0;                                        // twiddle entries produced before this chunk
         long long pf_a = 0, pf_b = 0, pf_t = 0, pf_tot = clock64(), pf_c;
-        // Stagger the clusters across one accumulation-chain period.  Every cluster does identical
-        // work, so without this all 148 SMs drain their TMEM tiles (38 MB + the read-modify-write
-        // traffic) in the same few microseconds and the epilogue becomes HBM-burst bound.
-        if (prm.stagger) {
-            const int n_sub_max = (nt_max + NSUB - 1) / NSUB;
-            const long long chain = (long long)prm.kc_per_split * n_sub_max * (KC / 16) * (parts > 1 ? 3 : 1) * 128;
-            const long long delay = chain * cl / n_cl;
-            const long long t0 = clock64();
-            while (clock64() - t0 < delay) { }
-        }
 #define PF_BEGIN() (pf_c = clock64())
 #define PF_END(acc) (acc += clock64() - pf_c)
         uint32_t te_bits = 0;                                  // phase bit per 256-column TMEM block
@@ -434,30 +431,32 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             const int n0 = (w % prm.n_passes) * NT_MAX;
             const int nt = min(NT_MAX, N - n0);
             const int n_sub = (nt + NSUB - 1) / NSUB;
+            const bool active = h < n_sub;                     // this warp's column half exists in this pass
+            const int nw = active ? min(NSUB, nt - h * NSUB) : 0;
+            const uint32_t idesc = idesc_bf16(BM * CG, nw);
             for (int ks = 0; ks < prm.k_splits; ++ks) {
-            const uint32_t blk0 = n_acc == 2 ? t.idx : 0;          // first 256-column TMEM block of this chain
-            const uint32_t d_base = tmem_base + blk0 * 256;
+            const uint32_t blk = (n_acc == 2 ? t.idx : 0) + h;   // this warp's 256-column TMEM block
+            const uint32_t d = tmem_base + blk * 256;
             const int kc_begin = ks * prm.kc_per_split, kc_end = min(n_kc, kc_begin + prm.kc_per_split);
             for (int kc = kc_begin; kc < kc_end; ++kc) {
                 PF_BEGIN(); mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase); PF_END(pf_a);
                 tc_fence_after();
                 const uint32_t a_hi = smem_u32(a_ring + a.idx * a_slot_bytes);
                 const uint32_t a_lo = a_hi + A_PART_BYTES;
-                for (int nh = 0; nh < n_sub; ++nh) {
-                    const int nw = min(NSUB, nt - nh * NSUB);
-                    const uint32_t idesc = idesc_bf16(BM * CG, nw);
-                    const uint32_t d = d_base + nh * NSUB;
+                if (active) {
                     if (kc == kc_begin) {
                         // first write into this TMEM block: wait until the epilogue has drained it
-                        PF_BEGIN(); mbar_wait(smem_u32(&ctl->t_empty[blk0 + nh]), ((te_bits >> (blk0 + nh)) & 1u) ^ 1u); PF_END(pf_t);
-                        te_bits ^= 1u << (blk0 + nh);
+                        PF_BEGIN(); mbar_wait(smem_u32(&ctl->t_empty[blk]), ((te_bits >> blk) & 1u) ^ 1u); PF_END(pf_t);
+                        te_bits ^= 1u << blk;
                         tc_fence_after();
                     }
                     // ---- B_hi: (A_lo x B_hi) then (A_hi x B_hi)
-                    PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); PF_END(pf_b);
+                    uint32_t e = g + (uint32_t)h * (uint32_t)parts;
+                    uint32_t bi = e % N_B, bp = (e / N_B) & 1u;
+                    PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); PF_END(pf_b);
                     tc_fence_after();
                     if (lane == 0) {
-                        const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * B_ENTRY));
+                        const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + bi * B_ENTRY));
                         uint32_t acc = kc > kc_begin;
                         if (prm.debug & 4) { } else
                         if (parts > 1) {
@@ -469,26 +468,26 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                         if (!(prm.debug & 4))
 #pragma unroll
                         for (int k = 0; k < KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
-                        commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]));
+                        commit_cg<CG>(smem_u32(&ctl->b_empty[bi]));
                     }
                     __syncwarp();
-                    b.advance(N_B);
                     // ---- B_lo: (A_hi x B_lo)
                     if (parts > 1) {
-                        PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); PF_END(pf_b);
+                        ++e; bi = e % N_B; bp = (e / N_B) & 1u;
+                        PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); PF_END(pf_b);
                         tc_fence_after();
                         if (lane == 0) {
-                            const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * B_ENTRY));
+                            const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + bi * B_ENTRY));
                             const uint64_t ad = smem_desc_sw128(a_hi);
                             if (!(prm.debug & 4))
 #pragma unroll
                             for (int k = 0; k < KC / 16; ++k) umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
-                            commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]));
+                            commit_cg<CG>(smem_u32(&ctl->b_empty[bi]));
                         }
                         __syncwarp();
-                        b.advance(N_B);
                     }
                 }
+                g += (uint32_t)(n_sub * parts);
                 if (lane == 0) {
                     commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]));
                     if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[t.idx]));
@@ -499,7 +498,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             t.advance(n_acc);
             }
         }
-        if (prm.prof && lane == 0) {
+        if (prm.prof && lane == 0 && h == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
             pp[0] = clock64() - pf_tot; pp[1] = pf_a; pp[2] = pf_b; pp[3] = pf_t;
         }
@@ -549,9 +548,9 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             if (n0 + cb == 0) {
                                 // columns 0 / 1 carry Re X[0] and Re X[P/2]; Im X[0] = Im X[P/2] = 0
                                 float2* ny = reinterpret_cast<float2*>(orow + prm.P);
-                                float nyq = __uint_as_float(r[1]);
-                                if (ks > 0) nyq += ny->x;
-                                *ny = make_float2(nyq, 0.f);
+                                const float nyq = __uint_as_float(r[1]);
+                                if (ks > 0) atomicAdd(&ny->x, nyq);           // fire-and-forget fp32 add at L2
+                                else *ny = make_float2(nyq, 0.f);
                                 r[1] = 0u;
                             }
                             if (odd) {
@@ -561,8 +560,8 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                                 float2* e1 = reinterpret_cast<float2*>(orow + cb + 30);
                                 float2 a = make_float2(__uint_as_float(r[0]), __uint_as_float(r[1]));
                                 float2 b = make_float2(__uint_as_float(r[30]), __uint_as_float(r[31]));
-                                if (ks > 0) { const float2 oa = *e0, ob = *e1; a.x += oa.x; a.y += oa.y; b.x += ob.x; b.y += ob.y; }
-                                *e0 = a; *e1 = b;
+                                if (ks > 0) { atomicAdd(e0, a); atomicAdd(e1, b); }   // red.global.add.v2.f32, no round trip
+                                else { *e0 = a; *e1 = b; }
                             }
                         } else if (REAL && n0 + cb == 0) {
                             r[1] = 0u;
