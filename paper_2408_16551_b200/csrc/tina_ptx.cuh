@@ -69,13 +69,15 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
     return ok != 0;
 }
 // Bounded wait: a protocol bug traps (kernel aborts with an error) instead of hanging the GPU.
-template <bool CLUSTER = false>
+// SLEEP_NS > 0: back off between polls (for roles that wait long and must not steal issue slots).
+template <int SLEEP_NS = 0>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    if (CLUSTER ? mbar_try_wait_cluster(bar, parity) : mbar_try_wait(bar, parity)) return;
+    if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
     uint32_t spins = 0;
-    while (!(CLUSTER ? mbar_try_wait_cluster(bar, parity) : mbar_try_wait(bar, parity))) {
+    while (!mbar_try_wait(bar, parity)) {
+        if (SLEEP_NS > 0) __nanosleep(SLEEP_NS);
         if ((++spins & 0xfff) == 0 && clock64() - t0 > 4000000000LL) __trap();
     }
 }

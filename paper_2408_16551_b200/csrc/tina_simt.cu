@@ -8,61 +8,152 @@
 namespace tina {
 
 // =====================================================================================
-// FIR: y[c][j] = sum_k a[k] x[c][j + M-1-k] = sum_i a[M-1-i] x[c][j+i]
-// One CTA computes FIR_TILE consecutive outputs of one channel.  Each thread owns 8
-// consecutive outputs and slides an 8-register window over the staged input, so the hot
-// loop is 64 FFMA per 8 LDS(x) + 2 broadcast LDS.128 (taps).  The staged input uses a
-// 9-words-per-8 skew so that the stride-8 per-thread walk is bank-conflict free.
+// FIR: y[c][j] = sum_k a[k] x[c][j + M-1-k] = sum_i ta[i] x[c][j+i],  ta[i] = a[M-1-i]
+// One CTA computes FIR_TILE consecutive outputs of one channel; each thread owns 16
+// consecutive outputs and slides a 16-register window over the staged input, so the hot loop
+// is 256 FFMA per 16 LDS.32 (window) + 4 broadcast LDS.128 (taps).  The input tile is staged
+// TRANSPOSED -- element e lives at [e % 16][e / 16] with a row pitch = 2 (mod 32) -- so that
+// both the coalesced fill (consecutive e per lane) and the per-thread walk (lane t reads
+// element 16 t + m: row m % 16, column t + m / 16) are bank-conflict free.  Results leave
+// through the same tile for fully coalesced stores.
 // =====================================================================================
+__device__ __forceinline__ float2 ffma2s(float2 a, float2 b, float2 c)
+{
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return d;
+}
+
 constexpr int FIR_THREADS = 256;
-constexpr int FIR_PER_THREAD = 8;
-constexpr int FIR_TILE = FIR_THREADS * FIR_PER_THREAD;  // 2048 outputs per CTA
+constexpr int FIR_PER_THREAD = 16;
+constexpr int FIR_TILE = FIR_THREADS * FIR_PER_THREAD;  // 4096 outputs per CTA
 
-__device__ __forceinline__ int skew(int e) { return e + (e >> 3); }
+// Row pitch of the transposed tile: compile-time (immediate address offsets in the hot loop), = 2 mod 32.
+constexpr int FIR_LD_SMALL = 290;    // M <= 512  (needs 256 + Mp/16 + 1 columns)
+constexpr int FIR_LD_LARGE = 514;    // M <= 4096
 
+// Shared-memory load the compiler may not merge with another load of the same word: the E and O
+// windows both hold every sample, and a register move instead of the second LDS would cost an
+// FMA-pipe slot (IMAD.MOV) in a loop that is bound by that pipe.
+__device__ __forceinline__ float lds_nomerge(const float* p)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"((unsigned)__cvta_generic_to_shared(p)));
+    return v;
+}
+
+// two unmerged 32-bit shared loads straight into the halves of one 64-bit register pair
+__device__ __forceinline__ unsigned long long lds_pair(const float* plo, const float* phi)
+{
+    unsigned long long v;
+    asm volatile("{\n\t.reg .f32 lo, hi;\n\tld.volatile.shared.f32 lo, [%1];\n\tld.volatile.shared.f32 hi, [%2];\n\tmov.b64 %0, {lo, hi};\n\t}"
+                 : "=l"(v) : "r"((unsigned)__cvta_generic_to_shared(plo)), "r"((unsigned)__cvta_generic_to_shared(phi)));
+    return v;
+}
+// d = (a, a) * b + c on packed fp32 pairs held in 64-bit registers
+__device__ __forceinline__ unsigned long long ffma2_bcast(float a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("{\n\t.reg .b64 ra;\n\tmov.b64 ra, {%1, %1};\n\tfma.rn.f32x2 %0, ra, %2, %3;\n\t}" : "=l"(d) : "f"(a), "l"(b), "l"(c));
+    return d;
+}
+
+__device__ __forceinline__ void cp_async4(float* dst_smem, const float* src, bool valid)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    const int sz = valid ? 4 : 0;                      // src-size 0: the 4 bytes are zero-filled
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+}
+
+// Persistent: each CTA walks tiles blockIdx.x, + gridDim.x, ...; the next tile is staged with
+// cp.async (LDGSTS) into the other buffer while the current one is being filtered.
+template <int LD>
 __global__ void __launch_bounds__(FIR_THREADS)
 fir_kernel(const float* __restrict__ x, const float* __restrict__ taps, float* __restrict__ y,
-           long long L, int M, long long Lo, int tiles_per_chan)
+           long long L, int M, long long Lo, int tiles_per_chan, int total_tiles)
 {
     extern __shared__ __align__(16) float smem[];
-    const int Mp = (M + 7) & ~7;                       // taps padded to a multiple of 8
+    const int Mp = (M + 15) & ~15;                     // taps padded to a multiple of 16 (zeros)
     float* s_taps = smem;                              // [Mp]  reversed: s_taps[i] = a[M-1-i]
-    float* s_x = smem + Mp;                            // skewed [FIR_TILE + Mp + 8]
+    float* s_buf0 = smem + Mp;                         // 2 x [16][LD] input tiles, then [16][LD] output tile
+    float* s_out = s_buf0 + 2 * 16 * LD;
+    const int n_stage = FIR_TILE + Mp;                 // elements the walk may touch
 
-    const int c = blockIdx.x / tiles_per_chan;
-    const long long j0 = (long long)(blockIdx.x % tiles_per_chan) * FIR_TILE;
-    const float* xc = x + (long long)c * L;
-    const int n_out = (int)min((long long)FIR_TILE, Lo - j0);
-    const int n_in = n_out + M - 1;
-    const int n_stage = FIR_TILE + Mp + 8;
+    auto stage = [&](int tile, float* dst) {
+        const int c = tile / tiles_per_chan;
+        const long long j0 = (long long)(tile % tiles_per_chan) * FIR_TILE;
+        const float* xc = x + (long long)c * L + j0;
+        const int n_in = (int)min((long long)FIR_TILE, Lo - j0) + M - 1;
+        for (int e = threadIdx.x; e < n_stage; e += FIR_THREADS)
+            cp_async4(dst + (e & 15) * LD + (e >> 4), xc + (e < n_in ? e : 0), e < n_in);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
 
-    for (int i = threadIdx.x; i < Mp; i += FIR_THREADS) s_taps[i] = (i < M) ? taps[M - 1 - i] : 0.f;
-    for (int e = threadIdx.x; e < n_stage; e += FIR_THREADS)
-        s_x[skew(e)] = (e < n_in) ? __ldg(xc + j0 + e) : 0.f;
-    __syncthreads();
+    for (int i = threadIdx.x; i < Mp; i += FIR_THREADS) s_taps[i] = (i < M) ? __ldg(taps + (M - 1 - i)) : 0.f;
+    int tile = blockIdx.x, buf = 0;
+    if (tile < total_tiles) stage(tile, s_buf0);
+    for (; tile < total_tiles; tile += gridDim.x, buf ^= 1) {
+    float* s_x = s_buf0 + buf * 16 * LD;
+    const int nxt = tile + gridDim.x;
+    if (nxt < total_tiles) { stage(nxt, s_buf0 + (buf ^ 1) * 16 * LD); asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+    else asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();                                   // tile `tile` (and the taps) are visible to every thread
 
-    const int t0 = threadIdx.x * FIR_PER_THREAD;
-    float acc[8], xr[8];
+    // Packed arithmetic (fma.rn.f32x2): the 16 outputs are 8 accumulator pairs (y[2q], y[2q+1]); tap i
+    // multiplies the input pair (x[2q+i], x[2q+i+1]).  64-bit operands must be aligned register
+    // pairs, so two windows are kept: E[m] = (x[2m], x[2m+1]) for even taps, O[m] = (x[2m+1], x[2m+2])
+    // for odd taps (8 pairs each, refreshed with two LDS.32 per pair as the walk advances).
+    const int t = threadIdx.x;
+    unsigned long long acc[8], E[8], O[8];             // packed fp32 pairs
+    const float* c0 = s_x + t;                         // element 16 t + m lives at c0[(m & 15) * LD + (m >> 4)]
 #pragma unroll
-    for (int r = 0; r < 8; ++r) { acc[r] = 0.f; xr[r] = s_x[skew(t0 + r)]; }
-
-    for (int i0 = 0; i0 < Mp; i0 += 8) {
-        const float4 ta = *reinterpret_cast<const float4*>(s_taps + i0);
-        const float4 tb = *reinterpret_cast<const float4*>(s_taps + i0 + 4);
-        const float tp[8] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+    for (int q = 0; q < 8; ++q) {
+        acc[q] = 0ull;
+        E[q] = lds_pair(c0 + (2 * q) * LD, c0 + (2 * q + 1) * LD);
+        O[q] = lds_pair(c0 + (2 * q + 1) * LD, q < 7 ? c0 + (2 * q + 2) * LD : c0 + 1);
+    }
+    const float* col = s_x + t + 1;                    // column of element 16 t + 16 + i0 + (row)
+    for (int i0 = 0; i0 < Mp; i0 += 16, ++col) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
+        for (int u4 = 0; u4 < 16; u4 += 4) {
+            const float4 tq = *reinterpret_cast<const float4*>(s_taps + i0 + u4);
+            const float tp[4] = {tq.x, tq.y, tq.z, tq.w};
 #pragma unroll
-            for (int r = 0; r < 8; ++r) acc[r] = fmaf(tp[u], xr[(r + u) & 7], acc[r]);
-            xr[u] = s_x[skew(t0 + i0 + u + 8)];       // slot u held x[t0+i0+u], no longer needed
+            for (int v = 0; v < 4; ++v) {
+                const int u = u4 + v;                  // tap i = i0 + u
+                if ((u & 1) == 0) {
+                    // pairs (x[2q+i], x[2q+i+1]) = E[q + i/2]; slot (q + u/2) & 7
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) acc[q] = ffma2_bcast(tp[v], E[(q + u / 2) & 7], acc[q]);
+                    // slot (u/2) & 7 held E[i/2]; it next holds E[i/2 + 8] = (x[i+16], x[i+17])
+                    E[(u / 2) & 7] = lds_pair(col + u * LD, col + (u + 1) * LD);
+                } else {
+                    // pairs = O[q + (i-1)/2]
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) acc[q] = ffma2_bcast(tp[v], O[(q + u / 2) & 7], acc[q]);
+                    // O[(i-1)/2 + 8] = (x[i+16], x[i+17]); row of x[i+17] wraps to the next column at u = 15
+                    O[(u / 2) & 7] = lds_pair(col + u * LD, u < 15 ? col + (u + 1) * LD : col + 1);
+                }
+            }
         }
     }
-    __syncthreads();                                   // everyone done reading s_x
+    // results leave through their own transposed tile (conflict-free writes, coalesced stores)
 #pragma unroll
-    for (int r = 0; r < 8; ++r) s_x[skew(t0 + r)] = acc[r];
-    __syncthreads();
-    float* yc = y + (long long)c * Lo + j0;
-    for (int e = threadIdx.x; e < n_out; e += FIR_THREADS) yc[e] = s_x[skew(e)];
+    for (int q = 0; q < 8; ++q) {
+        s_out[(2 * q) * LD + t] = __uint_as_float((unsigned)(acc[q] & 0xffffffffull));
+        s_out[(2 * q + 1) * LD + t] = __uint_as_float((unsigned)(acc[q] >> 32));
+    }
+    __syncthreads();                                   // also: everyone is done reading s_x before it is restaged
+    {
+        const int c = tile / tiles_per_chan;
+        const long long j0 = (long long)(tile % tiles_per_chan) * FIR_TILE;
+        const int n_out = (int)min((long long)FIR_TILE, Lo - j0);
+        float* yc = y + (long long)c * Lo + j0;
+        for (int e = threadIdx.x; e < n_out; e += FIR_THREADS) yc[e] = s_out[(e & 15) * LD + (e >> 4)];
+    }
+    }
 }
 
 tina_status simt_fir(const float* x, const float* taps, float* y, int C, long long L, int M,
@@ -71,16 +162,25 @@ tina_status simt_fir(const float* x, const float* taps, float* y, int C, long lo
     const long long Lo = L - M + 1;
     const long long tiles = (Lo + FIR_TILE - 1) / FIR_TILE;
     if (tiles * C > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_fir: C*L too large for one grid");
-    const int Mp = (M + 7) & ~7;
-    const int n_stage = FIR_TILE + Mp + 8;
-    const size_t smem = sizeof(float) * (Mp + n_stage + (n_stage >> 3) + 8);
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(fir_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-        if (e != cudaSuccess) return check_cuda(e, "cudaFuncSetAttribute(fir_kernel)");
-        attr_done = true;
+    const int Mp = (M + 15) & ~15;
+    const bool small = Mp <= 512;
+    const size_t smem = sizeof(float) * ((size_t)Mp + 3 * 16 * (size_t)(small ? FIR_LD_SMALL : FIR_LD_LARGE));
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaError_t e = cudaFuncSetAttribute(fir_kernel<FIR_LD_LARGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fir_kernel<FIR_LD_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "fir_kernel setup"); }
     }
-    fir_kernel<<<(unsigned)(tiles * C), FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles);
+    const long long total = tiles * C;
+    const int per_sm = small ? 4 : 1;                  // resident CTAs per SM (registers / shared memory)
+    const unsigned grid = (unsigned)(total < (long long)n_sm * per_sm ? total : (long long)n_sm * per_sm);
+    if (small)
+        fir_kernel<FIR_LD_SMALL><<<grid, FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles, (int)total);
+    else
+        fir_kernel<FIR_LD_LARGE><<<grid, FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles, (int)total);
     count_launch();
     g_last_path = kPathSimt;
     return check_cuda(cudaGetLastError(), "fir_kernel launch");

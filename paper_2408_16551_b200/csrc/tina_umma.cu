@@ -383,7 +383,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     for (int nh = 0; nh < n_sub; ++nh) {
                         const int nw = min(NSUB, nt - nh * NSUB);
                         for (int part = 0; part < parts; ++part) {
-                            mbar_wait(smem_u32(&ctl->b_empty[b.idx]), b.phase ^ 1);
+                            mbar_wait<64>(smem_u32(&ctl->b_empty[b.idx]), b.phase ^ 1);
                             const uint32_t bar = smem_u32(&ctl->b_full[b.idx]);
                             const uint32_t dst = smem_u32(b_ring + b.idx * B_ENTRY);
                             const int row = part * N + n0 + nh * NSUB + (int)rank * (nw / CG);
@@ -524,7 +524,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             float* obase = prm.out + ((long long)s * prm.F + row0) * prm.out_row + n0;
             const int rows_valid = (prm.debug & 2) ? 0 : (int)min(32LL, prm.F - row0);   // <= 0: nothing to store
             for (int ks = 0; ks < prm.k_splits; ++ks) {
-                pe_x = clock64(); mbar_wait(smem_u32(&ctl->t_full[t.idx]), t.phase); pe_w += clock64() - pe_x;
+                pe_x = clock64(); mbar_wait<256>(smem_u32(&ctl->t_full[t.idx]), t.phase); pe_w += clock64() - pe_x;
                 tc_fence_after();
                 const uint32_t blk0 = n_acc == 2 ? t.idx : 0;
                 const uint32_t taddr = tmem_base + blk0 * 256 + ((uint32_t)(q * 32) << 16);
