@@ -132,6 +132,8 @@ tina_status tina_pfb_fir_batched(const void* x, int S, long long n_samples, int 
     long long F;
     tina_status st = pfb_validate(x, S, n_samples, P, M, window, kind, y, "tina_pfb_fir", &F);
     if (st != TINA_OK) return st;
+    tina_status fs = TINA_OK;
+    if (umma_pfb_fir(x, S, n_samples, P, M, window, kind == TINA_REAL, y, (cudaStream_t)stream, &fs)) return fs;
     return simt_pfb_fir(x, S, n_samples, P, M, window, kind == TINA_REAL, y, (cudaStream_t)stream);
 }
 

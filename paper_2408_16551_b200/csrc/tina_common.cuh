@@ -40,5 +40,8 @@ bool umma_supported(int P, bool real);
 tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window,
                      bool real, bool inverse, tina_precision prec, void* out, cudaStream_t st);
 void umma_clear_plans();
+// subfilter stage only with the register-window kernel; false = shape not covered (use simt_pfb_fir)
+bool umma_pfb_fir(const void* x, int S, long long n_samples, int P, int M, const float* window, bool real,
+                  void* y, cudaStream_t st, tina_status* status);
 
 }  // namespace tina

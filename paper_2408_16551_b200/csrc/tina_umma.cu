@@ -924,3 +924,76 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
 }
 
 }  // namespace tina
+
+// =====================================================================================
+// Subfilter stage only (Eq. (20); Fig. 3 left column): the FIR producer's register
+// sliding window with a direct global store.  One CTA = 128 frames x 64 scalar columns (8 warps x
+// 16 frames); HBM-bound: every input sample is read once from HBM (the (M-1)-row halo between
+// neighbouring warps / CTAs comes from L1 / L2), every output written once.
+// =====================================================================================
+namespace tina {
+
+template <int MT, bool REAL>
+__global__ void __launch_bounds__(256)
+pfb_fir_win_kernel(const float* __restrict__ x, long long stream_stride, const float* __restrict__ window,
+                   float* __restrict__ y, long long F, long long NBLK, int K, int P, int M, int tiles_per_stream)
+{
+    constexpr int WA = MT;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int kc = blockIdx.x;                                   // 64-column chunk
+    const int tile = blockIdx.y;
+    const int s = tile / tiles_per_stream;
+    const long long f0 = (long long)(tile % tiles_per_stream) * BM + warp * FPW;
+    if (f0 >= F) return;
+    const int c0 = kc * KC + 2 * lane;
+    const float* xs = x + (long long)s * stream_stride + c0;
+    const bool interior = (f0 + M - WA >= 0) && (f0 + FPW + M - 1 <= NBLK);
+    FirRegs<MT> rg;
+    if (interior) fir_load<MT, REAL, false>(rg, window, P, M, K, NBLK, xs, c0, f0);
+    else          fir_load<MT, REAL, true>(rg, window, P, M, K, NBLK, xs, c0, f0);
+    float* yo = y + ((long long)s * F + f0) * K + c0;
+#pragma unroll
+    for (int i0 = 0; i0 < FPW; i0 += 8) {
+        float2 acc[8];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) acc[g] = fmul2(rg.tap[0], rg.row[i0 + g + WA - 1]);
+#pragma unroll
+        for (int m = 1; m < WA; ++m)
+#pragma unroll
+            for (int g = 0; g < 8; ++g) acc[g] = ffma2(rg.tap[m], rg.row[i0 + g + WA - 1 - m], acc[g]);
+#pragma unroll
+        for (int g = 0; g < 8; ++g)
+            if (f0 + i0 + g < F) *reinterpret_cast<float2*>(yo + (long long)(i0 + g) * K) = acc[g];
+    }
+}
+
+// true if the windowed-register kernel handled the call
+bool umma_pfb_fir(const void* x, int S, long long n_samples, int P, int M, const float* window, bool real,
+                  void* y, cudaStream_t st, tina_status* status)
+{
+    const int K = real ? P : 2 * P;
+    if (K % KC != 0 || M > 16) return false;
+    const long long NBLK = n_samples / P, F = NBLK - M + 1;
+    const int tiles_per_stream = (int)((F + BM - 1) / BM);
+    const long long tiles = (long long)S * tiles_per_stream;
+    if (tiles > 65535) return false;
+    const dim3 grid((unsigned)(K / KC), (unsigned)tiles);
+    const long long stride = real ? n_samples : 2 * n_samples;
+    const float* xf = static_cast<const float*>(x);
+    float* yf = static_cast<float*>(y);
+#define TINA_FIRWIN(MT_)                                                                                        \
+    do {                                                                                                        \
+        if (real) pfb_fir_win_kernel<MT_, true><<<grid, 256, 0, st>>>(xf, stride, window, yf, F, NBLK, K, P, M, tiles_per_stream); \
+        else      pfb_fir_win_kernel<MT_, false><<<grid, 256, 0, st>>>(xf, stride, window, yf, F, NBLK, K, P, M, tiles_per_stream); \
+    } while (0)
+    if (M <= 4) TINA_FIRWIN(4);
+    else if (M <= 8) TINA_FIRWIN(8);
+    else TINA_FIRWIN(16);
+#undef TINA_FIRWIN
+    count_launch();
+    g_last_path = kPathSimt;
+    *status = check_cuda(cudaGetLastError(), "pfb_fir_win_kernel launch");
+    return true;
+}
+
+}  // namespace tina

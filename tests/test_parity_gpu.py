@@ -225,6 +225,20 @@ def test_pfb_fir_only(tina, oracle):
             assert rel_l2_rows(y[s], yref) <= TOL_FP32
 
 
+@pytest.mark.parametrize("P,M,F,real,S", [(128, 3, 131, False, 2), (256, 8, 257, True, 1), (96, 5, 40, False, 1), (24, 4, 50, True, 2)])
+def test_pfb_fir_only_shapes(tina, oracle, P, M, F, real, S):
+    """Subfilter-only output over the register-window kernel (K % 64 == 0, M <= 16) and the generic one."""
+    import torch
+    rng = np.random.default_rng(810 + P)
+    case = ti.pfb_case(P, M, F, real=real, streams=S, seed=811 + P, window=ti.random_taps(rng, P * M))
+    y = tina.pfb_fir(_cuda(case.x), P, M, _cuda(case.window)); torch.cuda.synchronize()
+    y = y.cpu().numpy()
+    assert y.shape == (S, F, P)
+    for s in range(S):
+        _, yref = oracle.pfb(case.x[s], P, M, case.window, return_subfiltered=True)
+        assert rel_l2_rows(y[s], yref) <= TOL_FP32
+
+
 def test_error_paths(tina):
     import torch
     x = torch.zeros(64, dtype=torch.complex64, device="cuda")
