@@ -46,6 +46,32 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t cta)
                  "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}"
                  ::"r"(bar), "r"(cta) : "memory");
 }
+// same, ordering this thread's earlier (remote) shared-memory writes before the arrival at cluster scope
+__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t bar, uint32_t cta)
+{
+    asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\t"
+                 "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t}"
+                 ::"r"(bar), "r"(cta) : "memory");
+}
+// arm a barrier in CTA `cta` of the cluster: one arrival + `bytes` expected transaction bytes
+__device__ __forceinline__ void mbar_expect_tx_cluster(uint32_t bar, uint32_t cta, uint32_t bytes)
+{
+    asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\t"
+                 "mbarrier.arrive.expect_tx.shared::cluster.b64 _, [ra], %2;\n\t}"
+                 ::"r"(bar), "r"(cta), "r"(bytes) : "memory");
+}
+// bulk copy this CTA's shared memory -> shared memory of another CTA of the cluster (async proxy);
+// completion is signalled as transaction bytes on a barrier of the destination CTA
+__device__ __forceinline__ void bulk_copy_to_cluster(uint32_t dst_cluster_addr, uint32_t src_cta_addr, uint32_t bytes,
+                                                     uint32_t bar_cluster_addr)
+{
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_cluster_addr), "r"(src_cta_addr), "r"(bytes), "r"(bar_cluster_addr) : "memory");
+}
+__device__ __forceinline__ void sts32_cluster(uint32_t cluster_addr, uint32_t v)
+{
+    asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+}
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
@@ -82,6 +108,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     }
 }
 
+// generic-proxy writes (local and remote shared memory) -> visible to the async proxy (UMMA / TMA)
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

@@ -193,6 +193,17 @@ def test_pfb_complex_multichain_batched(tina, oracle):
         assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
 
 
+def test_pfb_shared_fir_clusters(tina, oracle, monkeypatch):
+    """Opt-in SHARE mode (TINA_SHARE=1): clusters of four CTAs compute the subfilter stage once per two
+    column passes and exchange the A tiles with bulk shared-memory-to-shared-memory copies."""
+    monkeypatch.setenv("TINA_SHARE", "1")
+    for (P, M, F, real, S) in [(1024, 16, 300, False, 2), (2048, 4, 259, True, 1), (512, 8, 700, False, 1)]:
+        case = ti.pfb_case(P, M, F, real=real, streams=S, seed=670 + P)
+        got = _run_pfb(tina, case)
+        for s in range(S):
+            assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
+
+
 def test_pfb_m1_rect_is_blocked_dft(tina, oracle):
     import torch
     P, F = 128, 256
