@@ -98,10 +98,14 @@ tina_status tina_pfb_batched(const void* x, int S, long long n_samples, int P, i
 tina_status tina_pfb_fir_batched(const void* x, int S, long long n_samples, int P, int M,
                                  const float* window, tina_kind kind, void* y, void* stream);
 
-/* Host-buffer convenience wrappers (the end-to-end path timed as `e2e` by bench.py):
- * x_host / window_host / out_host are HOST pointers (pinned memory recommended); the call
- * allocates device staging buffers on first use (cached, grown as needed), copies in on
- * `stream`, runs the device path, copies the result back and SYNCHRONISES the stream.      */
+/* Host-buffer entry point (the end-to-end path timed as `e2e` by bench.py):
+ * x_host / window_host / out_host are HOST pointers (pinned memory recommended; pageable memory
+ * works but copies synchronously).  The call allocates device staging buffers on first use (cached,
+ * grown as needed), cuts the batch into pieces (whole streams, or frame ranges of a stream with
+ * their (M-1)-block halo) and pipelines host->device copy, the device path and device->host copy of
+ * successive pieces on three internal streams ordered after `stream`; it returns after the last
+ * result byte has landed in out_host (SYNCHRONOUS).  Results are bit-identical to the device call.
+ * Not re-entrant (the staging buffers are shared; concurrent calls serialise on a mutex).       */
 tina_status tina_pfb_batched_host(const void* x_host, int S, long long n_samples, int P, int M,
                                   const float* window_host, tina_kind kind, tina_precision prec,
                                   void* out_host, void* stream);

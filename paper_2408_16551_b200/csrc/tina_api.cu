@@ -155,12 +155,66 @@ tina_status tina_pfb_batched_host(const void* x_host, int S, long long n_samples
     if ((st = stage_reserve(1, wb)) != TINA_OK) return st;
     if ((st = stage_reserve(2, ob)) != TINA_OK) return st;
     cudaStream_t cs = (cudaStream_t)stream;
-    cudaError_t e = cudaMemcpyAsync(g_stage[0].p, x_host, xb, cudaMemcpyHostToDevice, cs);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(g_stage[1].p, window_host, wb, cudaMemcpyHostToDevice, cs);
-    if (e != cudaSuccess) return check_cuda(e, "H2D copy");
-    st = tina_pfb_batched(g_stage[0].p, S, n_samples, P, M, (const float*)g_stage[1].p, kind, prec, g_stage[2].p, stream);
-    if (st != TINA_OK) return st;
-    e = cudaMemcpyAsync(out_host, g_stage[2].p, ob, cudaMemcpyDeviceToHost, cs);
+    cudaError_t e = cudaMemcpyAsync(g_stage[1].p, window_host, wb, cudaMemcpyHostToDevice, cs);
+    if (e != cudaSuccess) return check_cuda(e, "H2D copy (window)");
+
+    // Pipeline: the batch is cut into pieces (whole streams, or frame ranges of a stream with their
+    // (M-1)-block halo); piece i+1 is copied in and piece i-1 copied out while piece i is computed
+    // (PCIe is full duplex), on three internal streams chained by events.
+    const size_t row_in = (size_t)P * esz, row_out = nk * 8;
+    int pieces_per_stream = 1;
+    if (row_in % 16 == 0 && F >= 1024) {
+        pieces_per_stream = (int)((16 + S - 1) / S);
+        while (pieces_per_stream > 1 && F / pieces_per_stream < 512) --pieces_per_stream;
+    }
+    long long fpp = (F + pieces_per_stream - 1) / pieces_per_stream;
+    fpp = (fpp + 255) / 256 * 256;                                   // even frame counts keep real-kind rows 16-byte aligned
+    const int n_pieces_max = 64;
+    static cudaStream_t s_in = nullptr, s_cmp = nullptr, s_out = nullptr;
+    static cudaEvent_t ev_start = nullptr, ev_in[n_pieces_max], ev_cmp[n_pieces_max];
+    if (!s_in) {
+        e = cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s_cmp, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming);
+        for (int i = 0; i < n_pieces_max && e == cudaSuccess; ++i) {
+            e = cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_cmp[i], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) { s_in = nullptr; return check_cuda(e, "tina_pfb_batched_host: stream / event setup"); }
+    }
+    e = cudaEventRecord(ev_start, cs);                                // everything follows the caller's stream
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_in, ev_start, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_cmp, ev_start, 0);
+    if (e != cudaSuccess) return check_cuda(e, "tina_pfb_batched_host: stream ordering");
+    int piece = 0;
+    for (int sidx = 0; sidx < S; ++sidx) {
+        for (long long f_lo = 0; f_lo < F; f_lo += fpp, ++piece) {
+            const long long nf = (F - f_lo) < fpp ? (F - f_lo) : fpp;
+            const int ei = piece % n_pieces_max;
+            const size_t in_off = ((size_t)sidx * n_samples + (size_t)f_lo * P) * esz;
+            // last piece of a stream also carries the ignored tail samples (< P of them): not needed
+            const size_t in_bytes = (size_t)(nf + M - 1) * row_in;
+            const size_t out_off = ((size_t)sidx * F + f_lo) * row_out, out_bytes = (size_t)nf * row_out;
+            e = cudaMemcpyAsync((char*)g_stage[0].p + in_off, (const char*)x_host + in_off, in_bytes, cudaMemcpyHostToDevice, s_in);
+            if (e == cudaSuccess) e = cudaEventRecord(ev_in[ei], s_in);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s_cmp, ev_in[ei], 0);
+            if (e != cudaSuccess) return check_cuda(e, "H2D copy");
+            st = tina_pfb_batched((char*)g_stage[0].p + in_off, 1, (nf + M - 1) * (long long)P, P, M, (const float*)g_stage[1].p,
+                                  kind, prec, (char*)g_stage[2].p + out_off, s_cmp);
+            if (st != TINA_OK) { cudaDeviceSynchronize(); return st; }
+            e = cudaEventRecord(ev_cmp[ei], s_cmp);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s_out, ev_cmp[ei], 0);
+            if (e == cudaSuccess) e = cudaMemcpyAsync((char*)out_host + out_off, (char*)g_stage[2].p + out_off, out_bytes, cudaMemcpyDeviceToHost, s_out);
+            if (e != cudaSuccess) return check_cuda(e, "D2H copy");
+            if (piece + 1 >= n_pieces_max && (piece + 1) % n_pieces_max == 0) {
+                // event pool wraps: drain before reusing the events
+                e = cudaStreamSynchronize(s_out);
+                if (e != cudaSuccess) return check_cuda(e, "tina_pfb_batched_host: synchronize");
+            }
+        }
+    }
+    e = cudaStreamSynchronize(s_out);
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     return check_cuda(e, "D2H copy / synchronize");
 }

@@ -71,6 +71,7 @@ struct UmmaParams {
     int K;                     // floats per input row = GEMM K = GEMM N
     int P, M;
     int tiles_per_stream, n_passes, total_work;
+    int nt_pass;               // accumulator columns per pass
     int parts;                 // 2: bf16x3 (hi+lo), 1: single bf16 pass
     unsigned long long* prof;  // optional [grid][16] cycle counters (TINA_PROF=1, diagnostics only)
     int out_tma;               // 1: epilogue leaves through TMA tensor stores (always for the complex kind)
@@ -346,7 +347,8 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
     const uint32_t n_a = A_RING_BYTES / a_slot_bytes;            // 4 (bf16x3) or 8 (single pass)
     const int N = prm.K;
     const int n_kc = prm.K / KC;
-    const int nt_max = N < NT_MAX ? N : NT_MAX;
+    const int NTP = prm.nt_pass;                                  // accumulator columns per pass (256 or 512)
+    const int nt_max = N < NTP ? N : NTP;
     const uint32_t n_acc = nt_max <= 256 ? 2 : 1;                 // TMEM accumulator stages
     // cta_group::2: the CTA pair shares every twiddle tile (each CTA stages half of its N rows) and
     // the leader (rank 0) issues M=256 MMAs over both CTAs' A tiles; barriers the leader waits on
@@ -392,8 +394,8 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         if (lane == 0) {
             RingPos b;
             for (int w = cl; w < prm.total_work; w += n_cl) {
-                const int n0 = TINA_PASS(w) * NT_MAX;
-                const int nt = min(NT_MAX, N - n0);
+                const int n0 = TINA_PASS(w) * NTP;
+                const int nt = min(NTP, N - n0);
                 const int n_sub = (nt + NSUB - 1) / NSUB;
                 for (int kc = 0; kc < n_kc; ++kc)
                     for (int nh = 0; nh < n_sub; ++nh) {
@@ -444,8 +446,8 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
 #define PF_END(acc) (acc += clock64() - pf_c)
         uint32_t te_bits = 0;                                  // phase bit per 256-column TMEM block
         for (int w = cl; w < prm.total_work; w += n_cl) {
-            const int n0 = TINA_PASS(w) * NT_MAX;
-            const int nt = min(NT_MAX, N - n0);
+            const int n0 = TINA_PASS(w) * NTP;
+            const int nt = min(NTP, N - n0);
             const int n_sub = (nt + NSUB - 1) / NSUB;
             const bool active = h < n_sub;                     // this warp's column half exists in this pass
             const int nw = active ? min(NSUB, nt - h * NSUB) : 0;
@@ -533,8 +535,8 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         long long pe_w = 0, pe_tot = clock64(), pe_x, pe_ld = 0, pe_sts = 0, pe_st = 0, pe_fo = 0, pe_sy = 0;
         for (int w = cl; w < prm.total_work; w += n_cl) {
             const int tile = w / npg;
-            const int n0 = TINA_PASS(w) * NT_MAX;
-            const int nt = min(NT_MAX, N - n0);
+            const int n0 = TINA_PASS(w) * NTP;
+            const int nt = min(NTP, N - n0);
             const int s = tile / prm.tiles_per_stream;
             const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + q * 32;
             float* obase = prm.out + ((long long)s * prm.F + row0) * prm.out_row + n0;
@@ -887,7 +889,10 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     prm.P = P;
     prm.M = M;
     prm.tiles_per_stream = (int)((F + BM * UMMA_CG - 1) / (BM * UMMA_CG));
-    prm.n_passes = (K + NT_MAX - 1) / NT_MAX;
+    // Column pass width: all 512 TMEM columns (one accumulator stage, both MMA-issuing warps busy).  256-column
+    // passes (two TMEM stages, epilogue overlapped) measured slower at config 2 because only one warp issues.
+    prm.nt_pass = getenv("TINA_NT256") ? 256 : NT_MAX;
+    prm.n_passes = (K + prm.nt_pass - 1) / prm.nt_pass;
     // SHARE (clusters of four, FIR computed once per two column passes) needs an even number of passes
     static int n_sm = 0;
     if (!n_sm) {

@@ -250,6 +250,22 @@ def test_pfb_fir_only_shapes(tina, oracle, P, M, F, real, S):
         assert rel_l2_rows(y[s], yref) <= TOL_FP32
 
 
+@pytest.mark.parametrize("P,M,F,real,S", [(64, 4, 300, False, 3), (128, 8, 2500, True, 1), (256, 4, 3000, False, 2),
+                                           (16, 4, 1500, False, 1), (10, 2, 77, True, 2)])
+def test_pfb_host_pipeline_matches_device_call(tina, oracle, P, M, F, real, S):
+    """tina_pfb_batched_host (host buffers; pieces pipelined over copy / compute / copy streams) returns
+    exactly what the device-pointer call returns, and that matches the oracle."""
+    import torch
+    case = ti.pfb_case(P, M, F, real=real, streams=S, seed=900 + P + F)
+    xh = torch.from_numpy(case.x).pin_memory()
+    wh = torch.from_numpy(case.window).pin_memory()
+    got_h = tina.pfb_host(xh, P, M, wh).numpy()
+    got_d = _run_pfb(tina, case)
+    assert np.array_equal(got_h, got_d)
+    ref = oracle.pfb(case.x[S - 1], P, M, case.window)
+    assert rel_l2_rows(got_h[S - 1], ref) <= TOL_FP32
+
+
 def test_error_paths(tina):
     import torch
     x = torch.zeros(64, dtype=torch.complex64, device="cuda")
