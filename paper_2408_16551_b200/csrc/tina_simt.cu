@@ -175,7 +175,15 @@ tina_status simt_fir(const float* x, const float* taps, float* y, int C, long lo
         if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "fir_kernel setup"); }
     }
     const long long total = tiles * C;
-    const int per_sm = small ? 4 : 1;                  // resident CTAs per SM (registers / shared memory)
+    // resident CTAs per SM (registers / shared memory): a persistent grid must not exceed one wave
+    static int occ_small = 0, occ_large = 0;
+    int& occ = small ? occ_small : occ_large;
+    if (!occ) {
+        cudaError_t e = small ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fir_kernel<FIR_LD_SMALL>, FIR_THREADS, smem)
+                              : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fir_kernel<FIR_LD_LARGE>, FIR_THREADS, smem);
+        if (e != cudaSuccess || occ < 1) { occ = 0; return check_cuda(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor(fir_kernel)"); }
+    }
+    const int per_sm = occ;
     const unsigned grid = (unsigned)(total < (long long)n_sm * per_sm ? total : (long long)n_sm * per_sm);
     if (small)
         fir_kernel<FIR_LD_SMALL><<<grid, FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles, (int)total);
