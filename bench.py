@@ -181,7 +181,7 @@ def run_reference(args, w):
         return
     flops, byts, samples, frames = useful_flops_and_bytes(w)
     rates, secs = [], []
-    budget = max(2.0, min(15.0, 120.0 / max(args.steps + args.warmup, 1)))
+    budget = max(0.3, min(15.0, 100.0 / max(args.steps + args.warmup, 1)))   # whole run: about two minutes
     for i in range(args.warmup + args.steps):
         r, cores, sample, dt = cpu_oracle_rate(w, budget_s=budget)
         if i >= args.warmup:
