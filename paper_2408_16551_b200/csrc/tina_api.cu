@@ -88,6 +88,8 @@ tina_status tina_fir(const float* x, const float* taps, float* y, int C, long lo
     if (M > kMaxTapsFir) return fail(TINA_ERR_UNSUPPORTED, "tina_fir: M > %d", kMaxTapsFir);
     if ((const void*)x == (const void*)y) return fail(TINA_ERR_BAD_SHAPE, "tina_fir: in-place not supported");
     if (!aligned16(x) || !aligned16(y)) return fail(TINA_ERR_ALIGNMENT, "tina_fir: x, y must be 16-byte aligned");
+    tina_status fs = TINA_OK;
+    if (umma_fir(x, taps, y, C, L, M, (cudaStream_t)stream, &fs)) return fs;
     return simt_fir(x, taps, y, C, L, M, (cudaStream_t)stream);
 }
 

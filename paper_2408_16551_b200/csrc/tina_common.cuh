@@ -40,6 +40,9 @@ bool umma_supported(int P, bool real);
 tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window,
                      bool real, bool inverse, tina_precision prec, void* out, cudaStream_t st);
 void umma_clear_plans();
+// standalone FIR as a Toeplitz contraction on the tensor cores; false = shape not covered (use simt_fir)
+bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, int M, cudaStream_t st,
+              tina_status* status);
 // subfilter stage only with the register-window kernel; false = shape not covered (use simt_pfb_fir)
 bool umma_pfb_fir(const void* x, int S, long long n_samples, int P, int M, const float* window, bool real,
                   void* y, cudaStream_t st, tina_status* status);

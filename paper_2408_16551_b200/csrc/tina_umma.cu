@@ -22,6 +22,7 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 
+#include <atomic>
 #include <cstdlib>
 #include <cstring>
 #include <map>
@@ -56,6 +57,7 @@ struct SmemCtl {
     uint64_t t_full[2], t_empty[2];
     uint32_t tmem_base;
 };
+constexpr int FIR_PITCH = 132;               // staged row pitch (floats) of the Toeplitz-FIR epilogue (N = 128 columns)
 constexpr int EPI_LD = 36;                  // padded row length (floats) of the epilogue transpose tiles
 constexpr int EPI_STAGE_BYTES = 4608;        // per epilogue warp: one padded 32 x EPI_LD tile; the TMA path uses 4096-byte tiles at q * 4096
 constexpr size_t UMMA_SMEM_BYTES = A_RING_BYTES + B_RING_BYTES + 4 * EPI_STAGE_BYTES + sizeof(SmemCtl);
@@ -68,7 +70,14 @@ struct UmmaParams {
     long long stream_stride;   // floats between streams of x
     long long F, NBLK;         // frames per stream, input blocks per stream
     long long out_row;         // floats per output row (complex: 2P, real: P+2)
-    int K;                     // floats per input row = GEMM K = GEMM N
+    long long out_stream_stride; // floats between streams of out (F * out_row; FIR: L - M + 1)
+    int K;                     // GEMM K: floats of one A row (multiple of 64)
+    int N;                     // GEMM N: output columns (= K for the PFB / DFT; block length for the Toeplitz FIR)
+    long long x_row_stride;    // floats between consecutive A rows (= K for the PFB / DFT; block length for the FIR)
+    long long x_len;           // 0, or number of valid floats per stream: elements beyond it read as zero (FIR)
+    long long out_len;         // (scalar store mode) valid output floats per stream
+    int a_ring_bytes, b_ring_bytes, stage_bytes;   // shared-memory carve-up (defaults A_RING_BYTES / B_RING_BYTES / EPI_STAGE_BYTES)
+    int out_scalar;            // 1: epilogue stores rows of N contiguous floats, 4-byte aligned, clipped at out_len (FIR)
     int P, M;
     int tiles_per_stream, n_passes, total_work;
     int nt_pass;               // accumulator columns per pass
@@ -241,8 +250,11 @@ struct FirRegs {
 // Issue every global load of one chunk: MT tap pairs and the FPW + MT - 1 input rows the warp touches.
 template <int MT, bool REAL, bool CHECK>
 __device__ __forceinline__ void fir_load(FirRegs<MT>& rg, const float* __restrict__ window, int P, int M,
-                                         long long K, long long nblk, const float* __restrict__ xc, int c0, long long f0)
+                                         long long K, long long nblk, const float* __restrict__ xc, int c0, long long f0,
+                                         long long x_len = 0)
 {
+    // K here is the distance between consecutive rows (prm.x_row_stride); x_len != 0 (CHECK only): element
+    // index row * K + c0 (+1) must stay below x_len, anything beyond reads as zero (overlapping FIR rows)
     constexpr int WA = FirRegs<MT>::WA;
     if (MT > 0) {
         const float* wp = window + (REAL ? c0 : (c0 >> 1));
@@ -261,7 +273,16 @@ __device__ __forceinline__ void fir_load(FirRegs<MT>& rg, const float* __restric
     for (int j = 0; j < WA - 1 + FPW; ++j) {
         if (CHECK) {
             const long long r = r0 + j;
-            rg.row[j] = (r >= 0 && r < nblk) ? ldg_f2(p) : make_float2(0.f, 0.f);
+            float2 v = make_float2(0.f, 0.f);
+            if (r >= 0 && r < nblk) {
+                if (x_len == 0) v = ldg_f2(p);
+                else {
+                    const long long e = r * K + c0;
+                    if (e + 1 < x_len) v = ldg_f2(p);
+                    else if (e < x_len) v.x = __ldg(p);
+                }
+            }
+            rg.row[j] = v;
         } else {
             rg.row[j] = ldg_f2(p);
         }
@@ -337,15 +358,15 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
     extern __shared__ __align__(1024) uint8_t smem[];           // dynamic shared memory starts 1024-byte aligned (checked below)
     if ((smem_u32(smem) & 1023u) != 0) __trap();                // the swizzled tiles need 1024-byte alignment
     uint8_t* a_ring = smem;
-    uint8_t* b_ring = smem + A_RING_BYTES;
-    uint8_t* stage = b_ring + B_RING_BYTES;                         // 4 epilogue warps x EPI_STAGE_BYTES (1024-aligned)
-    SmemCtl* ctl = reinterpret_cast<SmemCtl*>(stage + 4 * EPI_STAGE_BYTES);
+    uint8_t* b_ring = smem + prm.a_ring_bytes;
+    uint8_t* stage = b_ring + prm.b_ring_bytes;                         // 4 epilogue warps x EPI_STAGE_BYTES (1024-aligned)
+    SmemCtl* ctl = reinterpret_cast<SmemCtl*>(stage + 4 * prm.stage_bytes);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int parts = prm.parts;
     const uint32_t a_slot_bytes = A_PART_BYTES * parts;
-    const uint32_t n_a = A_RING_BYTES / a_slot_bytes;            // 4 (bf16x3) or 8 (single pass)
-    const int N = prm.K;
+    const uint32_t n_a = (uint32_t)prm.a_ring_bytes / a_slot_bytes;            // 4 (bf16x3) or 8 (single pass)
+    const int N = prm.N;
     const int n_kc = prm.K / KC;
     const int NTP = prm.nt_pass;                                  // accumulator columns per pass (256 or 512)
     const int nt_max = N < NTP ? N : NTP;
@@ -368,7 +389,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
     const int npg = SHARE ? prm.n_passes / 2 : prm.n_passes;     // column passes per work item group
 #define TINA_PASS(w) (SHARE ? 2 * ((w) % npg) + (int)pr : (w) % npg)
     constexpr uint32_t B_ENTRY = B_ENTRY_BYTES / CG;             // bytes per B ring entry in this CTA
-    constexpr uint32_t N_B = B_RING_BYTES / B_ENTRY;              // ring entries
+    const uint32_t N_B = (uint32_t)prm.b_ring_bytes / B_ENTRY;    // ring entries (<= 8)
     const uint32_t b_box_bytes = (uint32_t)(N < NSUB ? N : NSUB) / CG * KC * 2;   // bytes one TMA box delivers
 
     if (warp == TMA_WARP && lane == 0) {
@@ -529,7 +550,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         // (4 rows x 128 B per float4 instruction; 2 rows x 128 B per float2 for the real kind,
         // whose rows are only 8-byte aligned).  Later accumulation chains add into the output.
         const int q = warp - EPI_WARP0;
-        float* stg = reinterpret_cast<float*>(stage + q * EPI_STAGE_BYTES);   // register / shared-memory store path
+        float* stg = reinterpret_cast<float*>(stage + q * prm.stage_bytes);   // register / shared-memory store path
         const uint32_t sbuf = smem_u32(stage) + q * 4096u;                    // TMA path: 1024-byte aligned swizzled tile
         RingPos t;
         long long pe_w = 0, pe_tot = clock64(), pe_x, pe_ld = 0, pe_sts = 0, pe_st = 0, pe_fo = 0, pe_sy = 0;
@@ -539,7 +560,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             const int nt = min(NTP, N - n0);
             const int s = tile / prm.tiles_per_stream;
             const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + q * 32;
-            float* obase = prm.out + ((long long)s * prm.F + row0) * prm.out_row + n0;
+            float* obase = prm.out + (long long)s * prm.out_stream_stride + row0 * prm.out_row + n0;
             const int rows_valid = (prm.debug & 2) ? 0 : (int)min(32LL, prm.F - row0);   // <= 0: nothing to store
             for (int ks = 0; ks < prm.k_splits; ++ks) {
                 pe_x = clock64(); mbar_wait<256>(smem_u32(&ctl->t_full[t.idx]), t.phase); pe_w += clock64() - pe_x;
@@ -618,6 +639,48 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[blk0 + (cb >> 8)]), rank, leader);
                         }
                     }
+                    t.advance(n_acc);
+                    continue;
+                }
+                if (prm.out_scalar) {
+                    // Toeplitz FIR: the warp's 32 rows x N columns are ONE contiguous run of 32 N floats of a
+                    // [C][L-M+1] array that is only 4-byte aligned.  Misaligned 128-byte row segments leave
+                    // partially written sectors behind (measured 4.5x slower), so the whole sub-tile is staged
+                    // (row pitch FIR_PITCH), TMEM is handed back at once, and the run is written as 16-byte
+                    // aligned float4 with scalar head / tail.
+                    uint32_t r[32];
+                    tmem_ld32(taddr, r);
+                    for (int cb = 0; cb < nt; cb += 32) {
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            *reinterpret_cast<float4*>(stg + lane * FIR_PITCH + cb + 4 * j) =
+                                make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
+                                            __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
+                        if (cb + 32 < nt) tmem_ld32(taddr + cb + 32, r);
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[blk0]), rank, leader);
+                    // linear element l of the run <-> staged [l / nt][l % nt]; stream index e0 + l
+                    const long long e0 = row0 * prm.out_row + n0;
+                    long long n_run = prm.out_len - e0;                        // valid elements of the run
+                    if (n_run > 32LL * 128) n_run = 32LL * 128;
+                    if (n_run > 0 && !(prm.debug & 2)) {
+                        float* g = obase;                                        // address of l = 0
+                        const int run = (int)n_run;
+                        const int head = min(run, (int)(((16u - ((uint32_t)(uintptr_t)g & 15u)) & 15u) >> 2));
+                        const int nv4 = (run - head) >> 2;                       // aligned float4 stores
+                        auto at = [&](int l) { return stg[(l >> 7) * FIR_PITCH + (l & 127)]; };   // nt == 128 in this mode
+                        if (lane < head) g[lane] = at(lane);
+                        for (int v = lane; v < nv4; v += 32) {
+                            const int l = head + 4 * v;
+                            *reinterpret_cast<float4*>(g + l) = make_float4(at(l), at(l + 1), at(l + 2), at(l + 3));
+                        }
+                        const int tail0 = head + 4 * nv4;
+                        if (tail0 + lane < run) g[tail0 + lane] = at(tail0 + lane);
+                    }
+                    __syncwarp();
                     t.advance(n_acc);
                     continue;
                 }
@@ -722,7 +785,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         constexpr int WA = MT > 0 ? MT : 1;
         const float* const window = prm.window;
         const int P = prm.P, M = prm.M;
-        const long long K = prm.K, nblk = prm.NBLK;
+        const long long K = prm.x_row_stride, nblk = prm.NBLK, x_len = prm.x_len;
         const bool split = parts > 1;
         FirRegs<MT> rg;
         const uint32_t r_ring_s = SHARE ? mapa_u32(a_ring_s, sib) : 0;   // the sibling's A ring (cluster address)
@@ -737,12 +800,13 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             f0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + pw * FPW;
             xs = prm.x + (long long)s * prm.stream_stride + 2 * lane;
             // rows f0 + M - WA .. f0 + FPW + M - 2 are touched; interior tiles need no bounds checks
-            interior = (f0 + M - WA >= 0) && (f0 + FPW + M - 1 <= nblk);
+            interior = (f0 + M - WA >= 0) && (f0 + FPW + M - 1 <= nblk) &&
+                       (x_len == 0 || (f0 + FPW + M - 2) * K + prm.K <= x_len);
         };
         auto load = [&](int kk) {
             if (prm.debug & 1) return;
             if (interior) fir_load<MT, REAL, false>(rg, window, P, M, K, nblk, xs + kk * KC, kk * KC + 2 * lane, f0);
-            else          fir_load<MT, REAL, true>(rg, window, P, M, K, nblk, xs + kk * KC, kk * KC + 2 * lane, f0);
+            else          fir_load<MT, REAL, true>(rg, window, P, M, K, nblk, xs + kk * KC, kk * KC + 2 * lane, f0, x_len);
         };
         // next chunk of the sequence that this CTA produces (SHARE: chunks alternate between the siblings)
         auto advance = [&](int& ww, int& kk, uint32_t& nn) {
@@ -885,7 +949,14 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     prm.F = F;
     prm.NBLK = NBLK;
     prm.out_row = real ? P + 2 : 2 * P;
+    prm.out_stream_stride = F * prm.out_row;
     prm.K = K;
+    prm.N = K;
+    prm.x_row_stride = K;
+    prm.x_len = 0;
+    prm.out_len = 0;
+    prm.out_scalar = 0;
+    prm.a_ring_bytes = A_RING_BYTES; prm.b_ring_bytes = B_RING_BYTES; prm.stage_bytes = EPI_STAGE_BYTES;
     prm.P = P;
     prm.M = M;
     prm.tiles_per_stream = (int)((F + BM * UMMA_CG - 1) / (BM * UMMA_CG));
@@ -1052,6 +1123,111 @@ bool umma_pfb_fir(const void* x, int S, long long n_samples, int P, int M, const
     count_launch();
     g_last_path = kPathSimt;
     *status = check_cuda(cudaGetLastError(), "pfb_fir_win_kernel launch");
+    return true;
+}
+
+}  // namespace tina
+
+// =====================================================================================
+// Standalone FIR on the tensor cores (the paper's unfolding view, Eq. (17)-(19), PAPER.md:183-202:
+// a FIR is a product of the unfolded signal with a banded Toeplitz matrix of the taps).
+// The signal of one channel is cut into blocks of T = 128 outputs; block b needs the T + M - 1
+// inputs x[bT .. bT + T + M - 2], i.e. OVERLAPPING rows of an "A" matrix with row pitch T:
+//     y[bT + n] = sum_c x[bT + c] * Tz[c][n],   Tz[c][n] = a[n + M-1 - c]  (0 outside the band)
+// This is the fused kernel with MT = 0 (A = x, split into bf16 hi / lo on the fly), the Toeplitz
+// matrix in place of the twiddles (built per call from the caller's taps, hi / lo split, K padded
+// to a multiple of 64 with zero rows) and N = T output columns.  With 64 taps 2/3 of the MMA work
+// is useful and the kernel is bound by HBM, not by the fp32 pipes (the CUDA-core kernel is
+// register-file-bandwidth bound at ~16 TFMA/s, 31 % of the HBM roofline at config 3).
+// =====================================================================================
+namespace tina {
+
+constexpr int FIR_T = 128;
+
+__global__ void toeplitz_kernel(__nv_bfloat16* __restrict__ tz, const float* __restrict__ taps, int M, int Kp)
+{
+    const int total = FIR_T * Kp;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < total; e += gridDim.x * blockDim.x) {
+        const int n = e / Kp, c = e % Kp;
+        const int k = n + M - 1 - c;
+        const float v = (k >= 0 && k < M) ? taps[k] : 0.f;
+        const __nv_bfloat16 hi = __float2bfloat16(v);
+        tz[e] = hi;
+        tz[total + e] = __float2bfloat16(v - __bfloat162float(hi));
+    }
+}
+
+bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, int M, cudaStream_t st,
+              tina_status* status)
+{
+    if (M > 193 || (L & 1) || getenv("TINA_FIR_SIMT")) return false;
+    const long long Lo = L - M + 1;
+    const int Kp = (FIR_T + M - 1 + KC - 1) / KC * KC;
+    const long long R = (Lo + FIR_T - 1) / FIR_T;                    // output blocks (A rows) per channel
+    const long long tps = (R + BM * UMMA_CG - 1) / (BM * UMMA_CG);
+    if (tps * C > 0x7fffffffLL) return false;
+
+    // Toeplitz scratch: a small ring of device buffers (the matrix is rebuilt from the caller's taps on every
+    // call, in stream order; eight calls may be in flight on different streams before a buffer is reused)
+    constexpr int kRing = 8;
+    constexpr size_t kTzBytes = (size_t)2 * FIR_T * 320 * sizeof(__nv_bfloat16);
+    static __nv_bfloat16* tz_ring = nullptr;
+    static std::atomic<unsigned> tz_next{0};
+    static int n_sm = 0;
+    {
+        std::lock_guard<std::mutex> lk(g_plan_mu);
+        if (!tz_ring) {
+            int dev = 0;
+            cudaGetDevice(&dev);
+            cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tz_ring), kRing * kTzBytes);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess) { tz_ring = nullptr; *status = check_cuda(e, "cudaMalloc(toeplitz)"); return true; }
+        }
+    }
+    __nv_bfloat16* tz = reinterpret_cast<__nv_bfloat16*>(reinterpret_cast<char*>(tz_ring) + (tz_next.fetch_add(1) % kRing) * kTzBytes);
+    toeplitz_kernel<<<(FIR_T * Kp + 255) / 256, 256, 0, st>>>(tz, taps, M, Kp);
+    count_launch();
+    CUtensorMap tmap, zero1, zero2;
+    memset(&zero1, 0, sizeof(zero1));
+    memset(&zero2, 0, sizeof(zero2));
+    EncodeTiledFn enc = encode_fn();
+    tina_status rs = TINA_OK;
+    if (!enc) rs = fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    if (rs == TINA_OK) {
+        const cuuint64_t dims[2] = {(cuuint64_t)Kp, (cuuint64_t)2 * FIR_T};
+        const cuuint64_t strides[1] = {(cuuint64_t)Kp * sizeof(__nv_bfloat16)};
+        const cuuint32_t box[2] = {(cuuint32_t)KC, (cuuint32_t)(FIR_T / UMMA_CG)};
+        const cuuint32_t estr[2] = {1, 1};
+        CUresult r = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, tz, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) rs = fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(toeplitz) failed (%d)", (int)r);
+    }
+    if (rs == TINA_OK) {
+        UmmaParams prm;
+        memset(&prm, 0, sizeof(prm));
+        prm.x = x; prm.window = nullptr; prm.out = y;
+        prm.stream_stride = L;
+        prm.F = R; prm.NBLK = R;
+        prm.out_row = FIR_T; prm.out_stream_stride = Lo;
+        prm.K = Kp; prm.N = FIR_T;
+        prm.x_row_stride = FIR_T; prm.x_len = L; prm.out_len = Lo; prm.out_scalar = 1;
+        prm.P = FIR_T; prm.M = 1;
+        prm.tiles_per_stream = (int)tps;
+        prm.nt_pass = NT_MAX; prm.n_passes = 1;
+        prm.total_work = (int)(tps * C);
+        prm.parts = 2;
+        prm.out_tma = 0; prm.stagger = 0;
+        prm.a_ring_bytes = 2 * 2 * A_PART_BYTES;                  // 2 slots of hi+lo
+        prm.b_ring_bytes = 4 * (B_ENTRY_BYTES / UMMA_CG);         // 4 half-tile entries (only 64 rows of each are used)
+        prm.stage_bytes = 32 * FIR_PITCH * 4;                     // 32 rows x 128 columns per epilogue warp
+        prm.debug = 0;
+        prm.k_splits = 1; prm.kc_per_split = Kp / KC;
+        const int n_cl = n_sm / UMMA_CG;
+        const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
+        rs = launch_umma<0, false, false>(tmap, zero1, zero2, prm, grid, st);
+    }
+    *status = rs;
     return true;
 }
 

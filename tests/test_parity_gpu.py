@@ -61,6 +61,26 @@ def test_fir_impulse_response_is_taps(tina):
     assert np.array_equal(y.cpu().numpy()[0], a)
 
 
+@pytest.mark.parametrize("C,L,K", [(2, 128 + 192, 193), (3, 4096, 1), (1, 130, 3), (5, 33000, 129), (2, 70000, 65)])
+def test_fir_toeplitz_tensor_path(tina, oracle, C, L, K):
+    """Even L and K <= 193 run as a banded-Toeplitz contraction on the tensor cores (the paper's
+    unfolding view): ragged last block, K = 1, the largest covered K."""
+    import torch
+    rng = np.random.default_rng(150 + K)
+    x = ti.noise_real(rng, C * L).reshape(C, L)
+    a = ti.random_taps(rng, K)
+    y = tina.fir(_cuda(x), _cuda(a))
+    torch.cuda.synchronize()
+    assert tina.last_path() == 2
+    ref = oracle.fir(x, a)
+    assert y.shape == ref.shape
+    assert rel_l2_rows(y.cpu().numpy(), ref) <= TOL_FP32
+    # impulse response = taps in order (to the bf16x3 split accuracy of each tap)
+    xi = np.zeros((1, 2 * K + 2), np.float32); xi[0, K - 1] = 1
+    yi = tina.fir(_cuda(xi), _cuda(a)); torch.cuda.synchronize()
+    assert np.allclose(yi.cpu().numpy()[0, :K], a, rtol=2e-5, atol=1e-6 * np.abs(a).max())
+
+
 def test_config3_fir_full(tina, oracle):
     """c3 at full size; per-channel rel L2 and per-4096-sample-block rel L2."""
     import torch
