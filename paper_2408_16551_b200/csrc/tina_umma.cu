@@ -1,6 +1,6 @@
 // tina_umma.cu -- the fused PFB / DFT kernel of libtina on the sm_100a tensor cores.
 //
-// One persistent, warp-specialised kernel computes, per 128-frame tile,
+// One persistent, warp-specialised kernel computes, per tile of frames,
 //     y[f][c]   = sum_m w[m][c] * x[f + M-1-m][c]          (Eq. (20); CUDA cores)
 //     out[f][n] = sum_c y[f][c] * T[c][n]                   (Eq. (12)-(13); tcgen05)
 // where x is viewed as a real [NB][K] matrix (K = 2P interleaved re/im for the complex kind,
@@ -10,12 +10,19 @@
 // comes from the error-compensated product  y*T ~= y_lo*T_hi + y_hi*T_hi + y_hi*T_lo  (bf16x3,
 // fp32 accumulation in TMEM); TINA_PREC_BF16 issues the single y_hi*T_hi pass.
 //
+// Launched as clusters of two CTAs (one per SM of a TPC pair) running tcgen05.mma.cta_group::2: the
+// pair owns a 256-frame x 512-column tile, each CTA supplies its own 128 frames of A and half of every
+// twiddle tile.  Accumulation chains are kept to 1024 contraction elements (the tensor-core fp32
+// accumulator truncates: DESIGN.md section 7); later chains are added into the output in fp32.
+//
 // Warp roles (512 threads, 1 CTA per SM):
-//   warp 0      TMA producer: twiddle tiles T_hi / T_lo  -> B ring (4 x 32 KB, SWIZZLE_128B)
-//   warp 1      MMA issuer (one elected lane): tcgen05.mma kind::f16, M=128, N<=256, K=16
-//   warp 2      TMEM allocator
-//   warps 4-7   epilogue: tcgen05.ld (TMEM -> registers) -> global stores
-//   warps 8-15  FIR producers: polyphase MAC in fp32 registers -> bf16 hi/lo -> A ring
+//   warps 0-7   FIR producers: polyphase MAC in fp32 registers (fma.rn.f32x2) -> bf16 hi/lo -> A ring
+//   warps 8-11  epilogue: tcgen05.ld (TMEM -> registers) -> swizzled staging tile -> TMA store / add-reduce
+//   warp 12     TMA producer: twiddle half-tiles T_hi / T_lo -> B ring (SWIZZLE_128B), barrier on the leader
+//   warps 13,15 MMA issuers of the leader CTA, one per 256-column accumulator half (kind::f16, M=256, K=16);
+//               the peer's warp 13 forwards "A tile ready" to the leader
+//   warp 14     TMEM allocator
+// The same kernel serves the standalone DFT (no window) and the Toeplitz FIR (overlapping A rows, N != K).
 #include "tina_common.cuh"
 #include "tina_ptx.cuh"
 
