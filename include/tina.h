@@ -113,6 +113,13 @@ tina_status tina_pfb_batched_host(const void* x_host, int S, long long n_samples
                                   const float* window_host, tina_kind kind, tina_precision prec,
                                   void* out_host, void* stream);
 
+/* Unfolding, Eq. (17): Y(i, j) = X(i + j), i in [0, I-J+1), j in [0, J)
+ * -- e.g. X = [1,2,3,4], J = 2 gives [[1,2],[2,3],[3,4]] (the paper's worked example).
+ *   x [I] float32 (device), y [I-J+1][J] float32 row-major (device), must not overlap x.
+ * Supported: 1 <= J <= I.  Memory-bound gather (each output written once, coalesced; the J-fold
+ * re-reads of x are served by L1 / L2).  Errors: NULL_POINTER, BAD_SHAPE, CUDA.                  */
+tina_status tina_unfold(const float* x, float* y, long long I, int J, void* stream);
+
 /* F = floor(n_samples / P) - M + 1; <= 0 means the input is too short.                     */
 long long   tina_pfb_num_frames(long long n_samples, int P, int M);
 

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libtina.so")
 _lib = None
 
-EXPORTS = ["tina_fir", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
+EXPORTS = ["tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
            "tina_pfb_batched_host", "tina_pfb_num_frames", "tina_status_string", "tina_last_error",
            "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path"]
 
@@ -37,12 +37,13 @@ def lib() -> ctypes.CDLL:
     L = ctypes.CDLL(_LIB_PATH)
     ll, vp, ci = ctypes.c_longlong, ctypes.c_void_p, ctypes.c_int
     L.tina_fir.argtypes = [vp, vp, vp, ci, ll, ci, vp]
+    L.tina_unfold.argtypes = [vp, vp, ll, ci, vp]
     L.tina_dft.argtypes = [vp, vp, ll, ci, ci, ci, vp]
     L.tina_pfb.argtypes = [vp, ll, ci, ci, vp, ci, ci, vp, vp]
     L.tina_pfb_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, ci, vp, vp]
     L.tina_pfb_fir_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, vp, vp]
     L.tina_pfb_batched_host.argtypes = [vp, ci, ll, ci, ci, vp, ci, ci, vp, vp]
-    for f in ("tina_fir", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
+    for f in ("tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
               "tina_pfb_batched_host", "tina_clear_plan_cache", "tina_version", "tina_last_path"):
         getattr(L, f).restype = ci
     L.tina_pfb_num_frames.argtypes = [ll, ci, ci]
@@ -112,6 +113,20 @@ def fir(x, taps, out=None, stream=None):
         out = torch.empty((C, max(L - M + 1, 0)), dtype=torch.float32, device=x.device)
     _dev(out, torch.float32, "out")
     _check(lib().tina_fir(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream)))
+    return out
+
+
+def unfold(x, J: int, out=None, stream=None):
+    """tina_unfold: x [I] float32 CUDA -> y [I-J+1, J] float32, Y(i, j) = X(i + j)."""
+    import torch
+    x = _dev(x, torch.float32, "x")
+    if x.dim() != 1:
+        raise ValueError("x must be 1-D")
+    I = x.shape[0]
+    if out is None:
+        out = torch.empty((max(I - J + 1, 0), J), dtype=torch.float32, device=x.device)
+    _dev(out, torch.float32, "out")
+    _check(lib().tina_unfold(x.data_ptr(), out.data_ptr(), I, J, _stream_ptr(stream)))
     return out
 
 

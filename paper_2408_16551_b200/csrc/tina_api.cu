@@ -221,6 +221,14 @@ tina_status tina_pfb_batched_host(const void* x_host, int S, long long n_samples
     return check_cuda(e, "D2H copy / synchronize");
 }
 
+tina_status tina_unfold(const float* x, float* y, long long I, int J, void* stream)
+{
+    if (!x || !y) return fail(TINA_ERR_NULL_POINTER, "tina_unfold: null pointer");
+    if (J < 1 || I < J) return fail(TINA_ERR_BAD_SHAPE, "tina_unfold: need 1 <= J <= I");
+    if ((const void*)x == (const void*)y) return fail(TINA_ERR_BAD_SHAPE, "tina_unfold: in-place not supported");
+    return simt_unfold(x, y, I, J, (cudaStream_t)stream);
+}
+
 long long tina_pfb_num_frames(long long n_samples, int P, int M)
 {
     if (P < 1 || M < 1 || n_samples < 0) return 0;

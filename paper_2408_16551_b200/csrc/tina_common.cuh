@@ -29,6 +29,7 @@ inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 // ---- generic CUDA-core path (tina_simt.cu) ------------------------------------------
 tina_status simt_fir(const float* x, const float* taps, float* y, int C, long long L, int M,
                      cudaStream_t st);
+tina_status simt_unfold(const float* x, float* y, long long I, int J, cudaStream_t st);
 // PFB / DFT on CUDA cores: window == nullptr means M == 1 with unit taps (plain DFT).
 tina_status simt_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window,
                      bool real, bool inverse, void* out, cudaStream_t st);

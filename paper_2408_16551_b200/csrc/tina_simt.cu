@@ -393,4 +393,31 @@ tina_status simt_pfb_fir(const void* x, int S, long long n_samples, int P, int M
     return check_cuda(cudaGetLastError(), "pfb_fir_kernel launch");
 }
 
+// =====================================================================================
+// Unfolding, Eq. (17): Y(i, j) = X(i + j).  One thread per output element, flat index
+// e = i J + j: consecutive threads write consecutive addresses and read x[i + j] (stride-1 within
+// a row, rows overlap by J - 1: L1 / L2 hits).
+// =====================================================================================
+__global__ void __launch_bounds__(256)
+unfold_kernel(const float* __restrict__ x, float* __restrict__ y, long long total, int J)
+{
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (long long)gridDim.x * blockDim.x) {
+        const long long i = e / J;
+        const int j = (int)(e - i * J);
+        y[e] = __ldg(x + i + j);
+    }
+}
+
+tina_status simt_unfold(const float* x, float* y, long long I, int J, cudaStream_t st)
+{
+    const long long total = (I - J + 1) * (long long)J;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    unfold_kernel<<<(unsigned)blocks, 256, 0, st>>>(x, y, total, J);
+    count_launch();
+    g_last_path = kPathSimt;
+    return check_cuda(cudaGetLastError(), "unfold_kernel launch");
+}
+
 }  // namespace tina

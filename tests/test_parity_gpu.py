@@ -81,6 +81,18 @@ def test_fir_toeplitz_tensor_path(tina, oracle, C, L, K):
     assert np.allclose(yi.cpu().numpy()[0, :K], a, rtol=2e-5, atol=1e-6 * np.abs(a).max())
 
 
+def test_unfold_matches_oracle_and_paper_example(tina, oracle):
+    """Eq. (17); bit-exact (a gather).  Includes the paper's worked example."""
+    import torch
+    y = tina.unfold(_cuda(np.array([1, 2, 3, 4], np.float32)), 2); torch.cuda.synchronize()
+    assert np.array_equal(y.cpu().numpy(), np.array([[1, 2], [2, 3], [3, 4]], np.float32))
+    rng = np.random.default_rng(77)
+    for (I, J) in [(1, 1), (1000, 1), (1000, 1000), (70001, 64), (5000, 333)]:
+        x = ti.noise_real(rng, I)
+        y = tina.unfold(_cuda(x), J); torch.cuda.synchronize()
+        assert np.array_equal(y.cpu().numpy().astype(np.float64), oracle.unfold(x, J))
+
+
 def test_config3_fir_full(tina, oracle):
     """c3 at full size; per-channel rel L2 and per-4096-sample-block rel L2."""
     import torch
