@@ -405,7 +405,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         // a_full: this CTA's 8 producer warps (+ in the leader one forwarded arrival from the peer's warp 1)
         for (int i = 0; i < 8; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), SHARE ? 4 : 2); }
         for (int i = 0; i < (int)N_B; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 2); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
+        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
         fence_mbar_init();
     }
     if (warp == ALLOC_WARP) {
@@ -536,7 +536,9 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 g += (uint32_t)(n_sub * parts);
                 if (lane == 0) {
                     commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), SHARE ? (uint16_t)0xF : pair_mask);
-                    if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[t.idx]), pair_mask);
+                    // one "accumulator ready" barrier per 256-column TMEM block: the two halves finish (and are
+                    // drained) independently, so one half's drain overlaps the other half's MMAs
+                    if (kc == kc_end - 1 && active) commit_cg<CG>(smem_u32(&ctl->t_full[blk]), pair_mask);
                 }
                 __syncwarp();
                 a.advance(n_a);
@@ -561,6 +563,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         const uint32_t sbuf = smem_u32(stage) + q * 4096u;                    // TMA path: 1024-byte aligned swizzled tile
         RingPos t;
         long long pe_w = 0, pe_tot = clock64(), pe_x, pe_ld = 0, pe_sts = 0, pe_st = 0, pe_fo = 0, pe_sy = 0;
+        uint32_t tf_bits = 0;                                  // phase bit per TMEM block's t_full barrier
         for (int w = cl; w < prm.total_work; w += n_cl) {
             const int tile = w / npg;
             const int n0 = TINA_PASS(w) * NTP;
@@ -570,9 +573,14 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             float* obase = prm.out + (long long)s * prm.out_stream_stride + row0 * prm.out_row + n0;
             const int rows_valid = (prm.debug & 2) ? 0 : (int)min(32LL, prm.F - row0);   // <= 0: nothing to store
             for (int ks = 0; ks < prm.k_splits; ++ks) {
-                pe_x = clock64(); mbar_wait<256>(smem_u32(&ctl->t_full[t.idx]), t.phase); pe_w += clock64() - pe_x;
-                tc_fence_after();
                 const uint32_t blk0 = n_acc == 2 ? t.idx : 0;
+                // wait for the 256-column TMEM block that column cb starts (called before its first tcgen05.ld)
+                auto wait_block = [&](int cb) {
+                    const uint32_t bk = blk0 + ((uint32_t)cb >> 8);
+                    pe_x = clock64(); mbar_wait<256>(smem_u32(&ctl->t_full[bk]), (tf_bits >> bk) & 1u); pe_w += clock64() - pe_x;
+                    tf_bits ^= 1u << bk;
+                    tc_fence_after();
+                };
                 const uint32_t taddr = tmem_base + blk0 * 256 + ((uint32_t)(q * 32) << 16);
                 if (prm.out_tma) {
                     // The tile leaves through the TMA engine.  Each 32x32 block is written (bank-conflict
@@ -583,6 +591,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     // and odd rows go out as two 16-row boxes through two maps over row pairs.
                     if (ks > 0 && lane == 0) bulk_wait<0>();     // the previous chain's stores to this tile are complete
                     uint32_t r[32];
+                    wait_block(0);
                     tmem_ld32(taddr, r);
                     const uint32_t rr = REAL ? ((uint32_t)lane >> 1) : (uint32_t)lane;       // row within the staged box
                     const bool odd = REAL && (lane & 1);
@@ -625,7 +634,8 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             for (int j = 0; j < 7; ++j)
                                 sts128(dst + 16u * j, r[4 * j + 2], r[4 * j + 3], r[4 * j + 4], r[4 * j + 5]);
                         }
-                        if (cb + 32 < nt) tmem_ld32(taddr + cb + 32, r);
+                        const bool last_of_block = (cb & 255) == 224;            // next 32 columns start another TMEM block
+                        if (cb + 32 < nt && !last_of_block) tmem_ld32(taddr + cb + 32, r);
                         fence_proxy_async();
                         __syncwarp();
                         if (lane == 0 && !(prm.debug & 2)) {
@@ -639,11 +649,13 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             }
                             bulk_commit();
                         }
-                        if ((cb & 255) == 224 || cb + 32 >= nt) {
-                            if ((cb & 255) == 224 && cb + 32 < nt) tmem_ld_wait();
+                        if (last_of_block || cb + 32 >= nt) {
+                            // this TMEM block has been read out completely: hand it back, then (if there is
+                            // another block) wait for it and start reading it
                             tc_fence_before();
                             __syncwarp();
                             if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[blk0 + (cb >> 8)]), rank, leader);
+                            if (cb + 32 < nt) { wait_block(cb + 32); tmem_ld32(taddr + cb + 32, r); }
                         }
                     }
                     t.advance(n_acc);
@@ -656,6 +668,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     // (row pitch FIR_PITCH), TMEM is handed back at once, and the run is written as 16-byte
                     // aligned float4 with scalar head / tail.
                     uint32_t r[32];
+                    wait_block(0);
                     tmem_ld32(taddr, r);
                     for (int cb = 0; cb < nt; cb += 32) {
                         tmem_ld_wait();
@@ -664,7 +677,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             *reinterpret_cast<float4*>(stg + lane * FIR_PITCH + cb + 4 * j) =
                                 make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
                                             __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
-                        if (cb + 32 < nt) tmem_ld32(taddr + cb + 32, r);
+                        if (cb + 32 < nt) { if (((cb + 32) & 255) == 0) wait_block(cb + 32); tmem_ld32(taddr + cb + 32, r); }
                     }
                     tc_fence_before();
                     __syncwarp();
@@ -719,6 +732,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 };
                 uint32_t r[32];
                 if (ks > 0) fetch_old(0);
+                wait_block(0);
                 tmem_ld32(taddr, r);
                 for (int cb = 0; cb < nt; cb += 32) {
                     const bool special = REAL && (n0 + cb == 0) && c == 0;   // columns 0 / 1 = Re X[0], Re X[P/2]
@@ -729,7 +743,8 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
                                         __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
                     // the next block's TMEM read overlaps this block's transpose and stores
-                    if (cb + 32 < nt) tmem_ld32(taddr + cb + 32, r);
+                    const bool last_of_block = (cb & 255) == 224;
+                    if (cb + 32 < nt && !last_of_block) tmem_ld32(taddr + cb + 32, r);
                     __syncwarp();
                     pe_sts += clock64() - pe_x; pe_x = clock64();
 #pragma unroll
@@ -759,13 +774,13 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     pe_fo += clock64() - pe_x; pe_x = clock64();
                     __syncwarp();
                     pe_sy += clock64() - pe_x;
-                    if ((cb & 255) == 224 || cb + 32 >= nt) {
-                        // a 256-column TMEM block has been read out (the read of the following block,
-                        // if any, is already in flight): hand it back to the MMA warp
-                        if ((cb & 255) == 224 && cb + 32 < nt) tmem_ld_wait();
+                    if (last_of_block || cb + 32 >= nt) {
+                        // a 256-column TMEM block has been read out: hand it back to the MMA warp, then wait
+                        // for the next block (if any) and start reading it
                         tc_fence_before();
                         __syncwarp();
                         if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[blk0 + (cb >> 8)]), rank, leader);
+                        if (cb + 32 < nt) { wait_block(cb + 32); tmem_ld32(taddr + cb + 32, r); }
                     }
                 }
                 t.advance(n_acc);
