@@ -255,6 +255,40 @@ def test_config1_pfb_full(tina, oracle):
     assert rel_l2_rows(got[0], ref) <= TOL_FP32
 
 
+def test_config4_full_size_sampled(tina, oracle):
+    """c4 at full size, in the launch configuration bench.py times (one tina_pfb_batched call over the
+    8 streams): first 16, last 16 and 96 seeded frames of every stream against the oracle; tone bins
+    dominate (P9); error over the non-tone bins reported against the looser bound of SURVEY 8(c)."""
+    case = ti.config4()
+    got = _run_pfb(tina, case)
+    assert got.shape == (8, 8192, 1024)
+    worst, worst_nt = 0.0, 0.0
+    for s in range(8):
+        fr = ti.sample_frames(8192, 96, ti.SEED_BASE + 40 + s)
+        ref = oracle.pfb(case.x[s], 1024, 16, case.window, frames=fr)
+        g = got[s][fr]
+        worst = max(worst, rel_l2_rows(g, ref))
+        mask = np.ones(1024, bool); mask[case.tone_bins[s]] = False
+        worst_nt = max(worst_nt, rel_l2_rows(g[:, mask], ref[:, mask]))
+        top3 = np.argsort(np.abs(ref).mean(axis=0))[-3:]
+        assert set(top3.tolist()) == set(case.tone_bins[s].tolist())
+    assert worst <= TOL_FP32
+    assert worst_nt <= 1.3e-4          # 1e-5 of the frame norm, which the tones inflate ~12x (SURVEY 8(c))
+
+
+@pytest.mark.parametrize("prec,tol", [(0, TOL_FP32), (1, TOL_BF16)])
+def test_config5_full_size_sampled(tina, oracle, prec, tol):
+    """c5 at full size (2^27 real samples, P=4096, M=8): fp32-accurate and single-pass bf16 runs, first 16,
+    last 16 and 64 seeded frames against the oracle; Im X[0] = Im X[P/2] = 0."""
+    case = ti.config5()
+    got = _run_pfb(tina, case, prec=prec)[0]
+    assert got.shape == (32761, 2049)
+    fr = ti.sample_frames(32761, 64, ti.SEED_BASE + 50)
+    ref = oracle.pfb(case.x[0], 4096, 8, case.window, frames=fr)
+    assert rel_l2_rows(got[fr], ref) <= tol
+    assert np.all(got[:, 0].imag == 0) and np.all(got[:, 2048].imag == 0)
+
+
 def test_pfb_fir_only(tina, oracle):
     import torch
     for real in (False, True):
