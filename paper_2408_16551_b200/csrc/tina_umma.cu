@@ -91,7 +91,6 @@ struct UmmaParams {
     int parts;                 // 2: bf16x3 (hi+lo), 1: single bf16 pass
     unsigned long long* prof;  // optional [grid][16] cycle counters (TINA_PROF=1, diagnostics only)
     int out_tma;               // 1: epilogue leaves through TMA tensor stores (always for the complex kind)
-    int stagger;               // 1: delay cluster i by i/n of a chain period (desynchronises the TMEM drains)
     int debug;                 // TINA_DEBUG_SKIP bits (1: no FIR work, 2: no epilogue global traffic, 4: no MMAs, 8: no TMA)
     int k_splits, kc_per_split; // accumulation chains per tile
 };
@@ -353,6 +352,9 @@ __device__ __forceinline__ void arrive_leader(uint32_t bar, uint32_t rank_in_pai
     if (CG == 1 || rank_in_pair == 0) mbar_arrive(bar); else mbar_arrive_cluster(bar, leader);
 }
 
+// cycle counter for the optional in-kernel profile (TINA_PROF=1); a constant when profiling is off
+#define PF_NOW() (prm.prof ? clock64() : 0LL)
+
 // =====================================================================================
 // The fused kernel.  MT = compile-time tap count the sliding window is unrolled for
 // (taps m >= M are zero; MT == 0: no window, y = x, i.e. a plain DFT batch).
@@ -469,9 +471,9 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         if (CG == 1 || rank == 0) {
         RingPos a, t;
         uint32_t g = 0;                                        // twiddle entries produced before this chunk
-        long long pf_a = 0, pf_b = 0, pf_t = 0, pf_tot = clock64(), pf_c;
-#define PF_BEGIN() (pf_c = clock64())
-#define PF_END(acc) (acc += clock64() - pf_c)
+        long long pf_a = 0, pf_b = 0, pf_t = 0, pf_tot = PF_NOW(), pf_c;
+#define PF_BEGIN() (pf_c = PF_NOW())
+#define PF_END(acc) (acc += PF_NOW() - pf_c)
         uint32_t te_bits = 0;                                  // phase bit per 256-column TMEM block
         for (int w = cl; w < prm.total_work; w += n_cl) {
             const int n0 = TINA_PASS(w) * NTP;
@@ -548,7 +550,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         }
         if (prm.prof && lane == 0 && h == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
-            pp[0] = clock64() - pf_tot; pp[1] = pf_a; pp[2] = pf_b; pp[3] = pf_t;
+            pp[0] = PF_NOW() - pf_tot; pp[1] = pf_a; pp[2] = pf_b; pp[3] = pf_t;
         }
         }
     } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
@@ -562,7 +564,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         float* stg = reinterpret_cast<float*>(stage + q * prm.stage_bytes);   // register / shared-memory store path
         const uint32_t sbuf = smem_u32(stage) + q * 4096u;                    // TMA path: 1024-byte aligned swizzled tile
         RingPos t;
-        long long pe_w = 0, pe_tot = clock64(), pe_x, pe_ld = 0, pe_sts = 0, pe_st = 0, pe_fo = 0, pe_sy = 0;
+        long long pe_w = 0, pe_tot = PF_NOW(), pe_x, pe_ld = 0, pe_sts = 0, pe_st = 0, pe_fo = 0, pe_sy = 0;
         uint32_t tf_bits = 0;                                  // phase bit per TMEM block's t_full barrier
         for (int w = cl; w < prm.total_work; w += n_cl) {
             const int tile = w / npg;
@@ -577,7 +579,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 // wait for the 256-column TMEM block that column cb starts (called before its first tcgen05.ld)
                 auto wait_block = [&](int cb) {
                     const uint32_t bk = blk0 + ((uint32_t)cb >> 8);
-                    pe_x = clock64(); mbar_wait<256>(smem_u32(&ctl->t_full[bk]), (tf_bits >> bk) & 1u); pe_w += clock64() - pe_x;
+                    pe_x = PF_NOW(); mbar_wait<256>(smem_u32(&ctl->t_full[bk]), (tf_bits >> bk) & 1u); pe_w += PF_NOW() - pe_x;
                     tf_bits ^= 1u << bk;
                     tc_fence_after();
                 };
@@ -736,7 +738,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 tmem_ld32(taddr, r);
                 for (int cb = 0; cb < nt; cb += 32) {
                     const bool special = REAL && (n0 + cb == 0) && c == 0;   // columns 0 / 1 = Re X[0], Re X[P/2]
-                    pe_x = clock64(); tmem_ld_wait(); pe_ld += clock64() - pe_x; pe_x = clock64();
+                    pe_x = PF_NOW(); tmem_ld_wait(); pe_ld += PF_NOW() - pe_x; pe_x = PF_NOW();
 #pragma unroll
                     for (int j = 0; j < 8; ++j)
                         *reinterpret_cast<float4*>(stg + lane * EPI_LD + 4 * j) =
@@ -746,7 +748,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     const bool last_of_block = (cb & 255) == 224;
                     if (cb + 32 < nt && !last_of_block) tmem_ld32(taddr + cb + 32, r);
                     __syncwarp();
-                    pe_sts += clock64() - pe_x; pe_x = clock64();
+                    pe_sts += PF_NOW() - pe_x; pe_x = PF_NOW();
 #pragma unroll
                     for (int i = 0; i < NV; ++i) {
                         const int rr = rbase + RSTEP * i;
@@ -769,11 +771,11 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             }
                         }
                     }
-                    pe_st += clock64() - pe_x; pe_x = clock64();
+                    pe_st += PF_NOW() - pe_x; pe_x = PF_NOW();
                     if (ks > 0 && cb + 32 < nt) fetch_old(cb + 32);
-                    pe_fo += clock64() - pe_x; pe_x = clock64();
+                    pe_fo += PF_NOW() - pe_x; pe_x = PF_NOW();
                     __syncwarp();
-                    pe_sy += clock64() - pe_x;
+                    pe_sy += PF_NOW() - pe_x;
                     if (last_of_block || cb + 32 >= nt) {
                         // a 256-column TMEM block has been read out: hand it back to the MMA warp, then wait
                         // for the next block (if any) and start reading it
@@ -789,7 +791,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         if (prm.out_tma && lane == 0) bulk_wait<0>();            // staging tiles must outlive their TMA reads
         if (prm.prof && q == 0 && lane == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
-            pp[8] = clock64() - pe_tot; pp[9] = pe_w; pp[10] = pe_ld; pp[11] = pe_sts; pp[12] = pe_st; pp[13] = pe_fo; pp[14] = pe_sy;
+            pp[8] = PF_NOW() - pe_tot; pp[9] = pe_w; pp[10] = pe_ld; pp[11] = pe_sts; pp[12] = pe_st; pp[13] = pe_fo; pp[14] = pe_sy;
         }
     } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ FIR producers =========================================
@@ -837,7 +839,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 if (++kk == n_kc) { kk = 0; ww += n_cl; }
             } while (SHARE && ww < prm.total_work && (nn & 1u) != pr);
         };
-        long long pq_w = 0, pq_c = 0, pq_f = 0, pq_tot = clock64(), pq_x;
+        long long pq_w = 0, pq_c = 0, pq_f = 0, pq_tot = PF_NOW(), pq_x;
         if (SHARE && pr != 0) advance(w, kc, n);             // pair 1 starts with chunk 1
         bool have = w < prm.total_work;
         if (have) { set_tile(w); load(kc); }
@@ -847,15 +849,15 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             advance(w2, kc2, n2);
             const bool have2 = w2 < prm.total_work;
             const uint32_t slot_i = n % n_a, slot_ph = (n / n_a) & 1u;
-            pq_x = clock64(); mbar_wait(smem_u32(&ctl->a_empty[slot_i]), slot_ph ^ 1); pq_w += clock64() - pq_x;
-            pq_x = clock64();
+            pq_x = PF_NOW(); mbar_wait(smem_u32(&ctl->a_empty[slot_i]), slot_ph ^ 1); pq_w += PF_NOW() - pq_x;
+            pq_x = PF_NOW();
             if (!(prm.debug & 1))
                 fir_compute_store<MT>(rg, a_ring_s + slot_i * a_slot_bytes, swz, split);
             if (have2) {
                 if (w2 != w) set_tile(w2);
                 load(kc2);
             }
-            pq_c += clock64() - pq_x; pq_x = clock64();
+            pq_c += PF_NOW() - pq_x; pq_x = PF_NOW();
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) {
@@ -872,12 +874,12 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                                              FPW * 128u, rbar);
                 }
             }
-            pq_f += clock64() - pq_x;
+            pq_f += PF_NOW() - pq_x;
             w = w2; kc = kc2; n = n2; have = have2;
         }
         if (prm.prof && pw == 0 && lane == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
-            pp[4] = clock64() - pq_tot; pp[5] = pq_w; pp[6] = pq_c; pp[7] = pq_f;
+            pp[4] = PF_NOW() - pq_tot; pp[5] = pq_w; pp[6] = pq_c; pp[7] = pq_f;
         }
     }
 
@@ -979,6 +981,13 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     prm.out_len = 0;
     prm.out_scalar = 0;
     prm.a_ring_bytes = A_RING_BYTES; prm.b_ring_bytes = B_RING_BYTES; prm.stage_bytes = EPI_STAGE_BYTES;
+    {   // experiment knobs: ring depths (A slots of 32 KB, B half-tile entries of 16 KB)
+        const char* ea = getenv("TINA_A_SLOTS"); const char* eb = getenv("TINA_B_ENTRIES");
+        if (ea) prm.a_ring_bytes = atoi(ea) * 2 * A_PART_BYTES;
+        if (eb) prm.b_ring_bytes = atoi(eb) * (B_ENTRY_BYTES / UMMA_CG);
+        if ((size_t)prm.a_ring_bytes + prm.b_ring_bytes + 4 * prm.stage_bytes + sizeof(SmemCtl) > UMMA_SMEM_BYTES)
+            return fail(TINA_ERR_UNSUPPORTED, "ring sizes exceed shared memory");
+    }
     prm.P = P;
     prm.M = M;
     prm.tiles_per_stream = (int)((F + BM * UMMA_CG - 1) / (BM * UMMA_CG));
@@ -1002,7 +1011,6 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     prm.total_work = (int)total;
     prm.parts = parts;
     prm.prof = nullptr;
-    { const char* sg = getenv("TINA_STAGGER"); prm.stagger = sg ? atoi(sg) : 1; }
     { const char* dbg = getenv("TINA_DEBUG_SKIP"); prm.debug = dbg ? atoi(dbg) : 0; }
     { const char* ksm = getenv("TINA_KSPLIT"); const int kmax = ksm ? atoi(ksm) : KSPLIT_MAX; prm.k_splits = (K + kmax - 1) / kmax; }
     prm.kc_per_split = ((K / KC) + prm.k_splits - 1) / prm.k_splits;
@@ -1239,7 +1247,7 @@ bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, i
         prm.nt_pass = NT_MAX; prm.n_passes = 1;
         prm.total_work = (int)(tps * C);
         prm.parts = 2;
-        prm.out_tma = 0; prm.stagger = 0;
+        prm.out_tma = 0;
         prm.a_ring_bytes = 2 * 2 * A_PART_BYTES;                  // 2 slots of hi+lo
         prm.b_ring_bytes = 4 * (B_ENTRY_BYTES / UMMA_CG);         // 4 half-tile entries (only 64 rows of each are used)
         prm.stage_bytes = 32 * FIR_PITCH * 4;                     // 32 rows x 128 columns per epilogue warp
