@@ -215,6 +215,18 @@ def test_pfb_real_batched_epilogue_paths(tina, oracle, P, M, F, S):
         assert np.all(got[s][:, 0].imag == 0) and np.all(got[s][:, P // 2].imag == 0)
 
 
+@pytest.mark.parametrize("P,M,F,real,S", [(32, 1, 1, False, 1), (64, 16, 1, True, 3), (32, 4, 257, False, 5),
+                                           (4096, 2, 130, False, 1), (8192, 2, 131, True, 1), (1024, 16, 513, False, 1)])
+def test_pfb_tensor_path_edges(tina, oracle, P, M, F, real, S):
+    """Single frame, ragged pair tiles, several streams, the largest contraction lengths (K = 8192:
+    eight accumulation chains, 16 column passes)."""
+    case = ti.pfb_case(P, M, F, real=real, streams=S, seed=680 + P + F)
+    got = _run_pfb(tina, case)
+    assert tina.last_path() == 2
+    for s in range(S):
+        assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
+
+
 def test_pfb_complex_multichain_batched(tina, oracle):
     """Complex kind, K = 4096: four accumulation chains (TMA add-reduce epilogue), 8 column passes,
     ragged last tile, 2 streams."""
