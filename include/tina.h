@@ -41,7 +41,9 @@ typedef enum { TINA_COMPLEX = 0, TINA_REAL = 1 } tina_kind;       /* "real_or_co
 typedef enum {
     TINA_PREC_FP32 = 0,   /* fp32-accurate: error-compensated bf16x3 tensor-core contraction
                              (rel. L2 per frame <= 1e-5 against a float64 reference)           */
-    TINA_PREC_BF16 = 1    /* single-pass bf16 operands, fp32 accumulate (<= 2e-2)              */
+    TINA_PREC_BF16 = 1,   /* single-pass bf16 operands, fp32 accumulate (<= 2e-2)              */
+    TINA_PREC_FP16 = 2    /* single-pass fp16 operands, fp32 accumulate (the paper's "16 bit",
+                             PAPER.md:206): ~5e-4, but |subfiltered sample| must stay < 65504  */
 } tina_precision;
 
 /* ---------------------------------------------------------------------------------------

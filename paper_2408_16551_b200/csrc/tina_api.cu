@@ -99,7 +99,7 @@ tina_status tina_dft(const void* x, void* out, long long B, int N, int inverse,
     if (!x || !out) return fail(TINA_ERR_NULL_POINTER, "tina_dft: null pointer");
     if (B < 1 || N < 2) return fail(TINA_ERR_BAD_SHAPE, "tina_dft: need B >= 1, N >= 2");
     if (N > kMaxP) return fail(TINA_ERR_UNSUPPORTED, "tina_dft: N > %d", kMaxP);
-    if (prec != TINA_PREC_FP32 && prec != TINA_PREC_BF16) return fail(TINA_ERR_BAD_SHAPE, "tina_dft: bad precision");
+    if (prec != TINA_PREC_FP32 && prec != TINA_PREC_BF16 && prec != TINA_PREC_FP16) return fail(TINA_ERR_BAD_SHAPE, "tina_dft: bad precision");
     if (x == out) return fail(TINA_ERR_BAD_SHAPE, "tina_dft: in-place not supported");
     if (!aligned16(x) || !aligned16(out)) return fail(TINA_ERR_ALIGNMENT, "tina_dft: x, out must be 16-byte aligned");
     // A DFT batch is a PFB with M = 1 and unit taps over one stream of B*N samples.
@@ -115,7 +115,7 @@ tina_status tina_pfb_batched(const void* x, int S, long long n_samples, int P, i
     long long F;
     tina_status st = pfb_validate(x, S, n_samples, P, M, window, kind, out, "tina_pfb", &F);
     if (st != TINA_OK) return st;
-    if (prec != TINA_PREC_FP32 && prec != TINA_PREC_BF16) return fail(TINA_ERR_BAD_SHAPE, "tina_pfb: bad precision");
+    if (prec != TINA_PREC_FP32 && prec != TINA_PREC_BF16 && prec != TINA_PREC_FP16) return fail(TINA_ERR_BAD_SHAPE, "tina_pfb: bad precision");
     const bool real = kind == TINA_REAL;
     if (umma_supported(P, real))
         return umma_pfb(x, S, n_samples, P, M, window, real, false, prec, out, (cudaStream_t)stream);

@@ -242,9 +242,10 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr)
     return d;
 }
 // Instruction descriptor for kind::f16 with bf16 A/B (both K-major), fp32 D.
-__host__ __device__ constexpr uint32_t idesc_bf16(int M, int N)
+// (a_format / b_format: 1 = bf16, 0 = fp16)
+__host__ __device__ constexpr uint32_t idesc_bf16(int M, int N, bool fp16 = false)
 {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+    return (1u << 4) | ((fp16 ? 0u : 1u) << 7) | ((fp16 ? 0u : 1u) << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
 }}  // namespace tina::ptx

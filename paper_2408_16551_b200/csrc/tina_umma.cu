@@ -28,6 +28,7 @@
 
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include <atomic>
 #include <cstdlib>
@@ -88,7 +89,8 @@ struct UmmaParams {
     int P, M;
     int tiles_per_stream, n_passes, total_work;
     int nt_pass;               // accumulator columns per pass
-    int parts;                 // 2: bf16x3 (hi+lo), 1: single bf16 pass
+    int parts;                 // 2: bf16x3 (hi+lo), 1: single pass
+    int fp16;                  // 1: the single pass uses fp16 operands (TINA_PREC_FP16)
     unsigned long long* prof;  // optional [grid][16] cycle counters (TINA_PROF=1, diagnostics only)
     int out_tma;               // 1: epilogue leaves through TMA tensor stores (always for the complex kind)
     int debug;                 // TINA_DEBUG_SKIP bits (1: no FIR work, 2: no epilogue global traffic, 4: no MMAs, 8: no TMA)
@@ -99,7 +101,7 @@ struct UmmaParams {
 // Plan: twiddle matrix Tt[part][n][c] (bf16, "K-major" = row n holds the K contraction index)
 // built on the device from float64 sincospi, + its TMA tensor map.
 // =====================================================================================
-__global__ void twiddle_kernel(__nv_bfloat16* __restrict__ tt, int P, int real, int inverse, int parts)
+__global__ void twiddle_kernel(__nv_bfloat16* __restrict__ tt, int P, int real, int inverse, int parts, int fp16)
 {
     const int N = real ? P : 2 * P;
     const long long total = (long long)N * N;
@@ -130,6 +132,7 @@ __global__ void twiddle_kernel(__nv_bfloat16* __restrict__ tt, int P, int real, 
             v = (j == 0) ? (i == 0 ? cs : sn) : (i == 0 ? -sn : cs);
         }
         v *= scale;
+        if (fp16) { reinterpret_cast<__half*>(tt)[e] = __double2half(v); continue; }   // single part only
         const __nv_bfloat16 hi = __double2bfloat16(v);
         tt[e] = hi;
         if (parts > 1) tt[total + e] = __double2bfloat16(v - (double)__bfloat162float(hi));
@@ -140,7 +143,7 @@ struct Plan {
     __nv_bfloat16* tt = nullptr;
     CUtensorMap tmap;
 };
-using PlanKey = std::tuple<int, int, int, int, int>;   // device, P, real, inverse, parts
+using PlanKey = std::tuple<int, int, int, int, int, int>;   // device, P, real, inverse, parts, fp16
 static std::mutex g_plan_mu;
 static std::map<PlanKey, Plan> g_plans;
 
@@ -161,13 +164,13 @@ static EncodeTiledFn encode_fn()
     return fn;
 }
 
-static tina_status get_plan(int P, bool real, bool inverse, int parts, cudaStream_t st, const Plan** out)
+static tina_status get_plan(int P, bool real, bool inverse, int parts, bool fp16, cudaStream_t st, const Plan** out)
 {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return check_cuda(e, "cudaGetDevice");
     std::lock_guard<std::mutex> lk(g_plan_mu);
-    const PlanKey key{dev, P, real ? 1 : 0, inverse ? 1 : 0, parts};
+    const PlanKey key{dev, P, real ? 1 : 0, inverse ? 1 : 0, parts, fp16 ? 1 : 0};
     auto it = g_plans.find(key);
     if (it != g_plans.end()) { *out = &it->second; return TINA_OK; }
 
@@ -176,7 +179,7 @@ static tina_status get_plan(int P, bool real, bool inverse, int parts, cudaStrea
     const size_t bytes = (size_t)parts * N * N * sizeof(__nv_bfloat16);
     e = cudaMalloc(&pl.tt, bytes);
     if (e != cudaSuccess) return check_cuda(e, "cudaMalloc(twiddles)");
-    twiddle_kernel<<<592, 256, 0, st>>>(pl.tt, P, real ? 1 : 0, inverse ? 1 : 0, parts);
+    twiddle_kernel<<<592, 256, 0, st>>>(pl.tt, P, real ? 1 : 0, inverse ? 1 : 0, parts, fp16 ? 1 : 0);
     count_launch();
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -188,7 +191,7 @@ static tina_status get_plan(int P, bool real, bool inverse, int parts, cudaStrea
     const cuuint64_t strides[1] = {(cuuint64_t)N * sizeof(__nv_bfloat16)};
     const cuuint32_t box[2] = {(cuuint32_t)KC, (cuuint32_t)((N < NSUB ? N : NSUB) / UMMA_CG)};
     const cuuint32_t estr[2] = {1, 1};
-    CUresult r = enc(&pl.tmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, pl.tt, dims, strides, box, estr,
+    CUresult r = enc(&pl.tmap, fp16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, pl.tt, dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { cudaFree(pl.tt); return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r); }
@@ -301,7 +304,8 @@ __device__ __forceinline__ void fir_load(FirRegs<MT>& rg, const float* __restric
 // advanced together so that four independent FMA chains are in flight.
 template <int MT>
 __device__ __forceinline__ void fir_compute_store(const FirRegs<MT>& rg, uint32_t slot, const uint32_t (&swz)[8], bool split,
-                                                  uint32_t rslot = 0)   // rslot != 0: also write the sibling CTA's slot
+                                                  uint32_t rslot = 0,   // rslot != 0: also write the sibling CTA's slot
+                                                  bool fp16 = false)   // single-pass fp16 operands instead of bf16
 {
     constexpr int WA = FirRegs<MT>::WA;
     constexpr int FG = 8;                  // frames advanced together (independent FMA chains in flight)
@@ -322,8 +326,9 @@ __device__ __forceinline__ void fir_compute_store(const FirRegs<MT>& rg, uint32_
 #pragma unroll
         for (int g = 0; g < FG; ++g) {
             const int i = i0 + g;
-            const __nv_bfloat162 hi = __floats2bfloat162_rn(y[g].x, y[g].y);
-            const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
+            uint32_t hb;
+            if (fp16) { const __half2 hh = __floats2half2_rn(y[g].x, y[g].y); hb = *reinterpret_cast<const uint32_t*>(&hh); }
+            else { const __nv_bfloat162 hi = __floats2bfloat162_rn(y[g].x, y[g].y); hb = *reinterpret_cast<const uint32_t*>(&hi); }
             const uint32_t addr = slot + swz[i & 7] + (uint32_t)i * 128u;
             sts32(addr, hb);
             const uint32_t raddr = rslot + swz[i & 7] + (uint32_t)i * 128u;
@@ -481,7 +486,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             const int n_sub = (nt + NSUB - 1) / NSUB;
             const bool active = h < n_sub;                     // this warp's column half exists in this pass
             const int nw = active ? min(NSUB, nt - h * NSUB) : 0;
-            const uint32_t idesc = idesc_bf16(BM * CG, nw);
+            const uint32_t idesc = idesc_bf16(BM * CG, nw, prm.fp16 != 0);
             for (int ks = 0; ks < prm.k_splits; ++ks) {
             const uint32_t blk = (n_acc == 2 ? t.idx : 0) + h;   // this warp's 256-column TMEM block
             const uint32_t d = tmem_base + blk * 256;
@@ -852,7 +857,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             pq_x = PF_NOW(); mbar_wait(smem_u32(&ctl->a_empty[slot_i]), slot_ph ^ 1); pq_w += PF_NOW() - pq_x;
             pq_x = PF_NOW();
             if (!(prm.debug & 1))
-                fir_compute_store<MT>(rg, a_ring_s + slot_i * a_slot_bytes, swz, split);
+                fir_compute_store<MT>(rg, a_ring_s + slot_i * a_slot_bytes, swz, split, 0, prm.fp16 != 0);
             if (have2) {
                 if (w2 != w) set_tile(w2);
                 load(kc2);
@@ -946,7 +951,8 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     const int K = real ? P : 2 * P;
     const long long NBLK = n_samples / P;
     const long long F = NBLK - M + 1;
-    const int parts = prec == TINA_PREC_BF16 ? 1 : 2;
+    const int parts = prec == TINA_PREC_FP32 ? 2 : 1;
+    const bool fp16 = prec == TINA_PREC_FP16;
 
     if (window && M > 16) {
         // Rare shape: more taps than the register window is unrolled for.  Run the subfilter
@@ -962,7 +968,7 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     }
 
     const Plan* plan = nullptr;
-    tina_status ps = get_plan(P, real, inverse, parts, st, &plan);
+    tina_status ps = get_plan(P, real, inverse, parts, fp16, st, &plan);
     if (ps != TINA_OK) return ps;
 
     UmmaParams prm;
@@ -1010,6 +1016,7 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     if (total > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: too many tiles");
     prm.total_work = (int)total;
     prm.parts = parts;
+    prm.fp16 = fp16 ? 1 : 0;
     prm.prof = nullptr;
     { const char* dbg = getenv("TINA_DEBUG_SKIP"); prm.debug = dbg ? atoi(dbg) : 0; }
     { const char* ksm = getenv("TINA_KSPLIT"); const int kmax = ksm ? atoi(ksm) : KSPLIT_MAX; prm.k_splits = (K + kmax - 1) / kmax; }

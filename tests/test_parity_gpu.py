@@ -189,6 +189,20 @@ def test_pfb_bf16_small(tina, oracle, P, M, F, real):
     assert rel_l2_rows(got[0], ref) <= TOL_BF16
 
 
+@pytest.mark.parametrize("P,M,F,real", [(64, 4, 200, False), (256, 8, 150, True), (1024, 16, 130, False)])
+def test_pfb_fp16_single_pass(tina, oracle, P, M, F, real):
+    """TINA_PREC_FP16: the paper's "16 bit" variant (fp16 operands, fp32 accumulate)."""
+    case = ti.pfb_case(P, M, F, real=real, seed=520 + P)
+    got = _run_pfb(tina, case, prec=2)
+    ref = oracle.pfb(case.x[0], P, M, case.window)
+    err = rel_l2_rows(got[0], ref)
+    assert err <= 2e-3            # 11-bit significands: ~4x tighter than the bf16 pass
+    x = ti.noise_complex(np.random.default_rng(9), 300 * 256).reshape(300, 256)
+    import torch
+    Z = tina.dft(_cuda(x), prec=2); torch.cuda.synchronize()
+    assert rel_l2_rows(Z.cpu().numpy(), oracle.dft(x)) <= 2e-3
+
+
 def test_pfb_batched_streams_and_tail(tina, oracle):
     """S streams in one launch; n_samples not a multiple of P (tail ignored, reading R8)."""
     P, M, F, S = 64, 4, 140, 3
