@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libtina.so")
 _lib = None
 
-EXPORTS = ["tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
+EXPORTS = ["tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
            "tina_pfb_batched_host", "tina_pfb_num_frames", "tina_status_string", "tina_last_error",
            "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path"]
 
@@ -42,8 +42,9 @@ def lib() -> ctypes.CDLL:
     L.tina_pfb.argtypes = [vp, ll, ci, ci, vp, ci, ci, vp, vp]
     L.tina_pfb_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, ci, vp, vp]
     L.tina_pfb_fir_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, vp, vp]
+    L.tina_pfb_fft_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, vp, vp]
     L.tina_pfb_batched_host.argtypes = [vp, ci, ll, ci, ci, vp, ci, ci, vp, vp]
-    for f in ("tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched",
+    for f in ("tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
               "tina_pfb_batched_host", "tina_clear_plan_cache", "tina_version", "tina_last_path"):
         getattr(L, f).restype = ci
     L.tina_pfb_num_frames.argtypes = [ll, ci, ci]
@@ -177,6 +178,20 @@ def pfb(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=None)
     _dev(out, torch.complex64, "out")
     _check(lib().tina_pfb_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind, prec,
                                   out.data_ptr(), _stream_ptr(stream)))
+    return out[0] if squeeze else out
+
+
+def pfb_fft(x, P: int, M: int, window, out=None, stream=None):
+    """tina_pfb_fft_batched: PFB with the factorised (32 x 32) Fourier stage; same result as pfb()."""
+    import torch
+    squeeze = x.dim() == 1
+    x, kind, S, n, F = _pfb_args(x, P, M, window)
+    NK = P if kind == COMPLEX else P // 2 + 1
+    if out is None:
+        out = torch.empty((S, max(F, 0), NK), dtype=torch.complex64, device=x.device)
+    _dev(out, torch.complex64, "out")
+    _check(lib().tina_pfb_fft_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind,
+                                      out.data_ptr(), _stream_ptr(stream)))
     return out[0] if squeeze else out
 
 

@@ -128,6 +128,17 @@ tina_status tina_pfb(const void* x, long long n_samples, int P, int M, const flo
     return tina_pfb_batched(x, 1, n_samples, P, M, window, kind, prec, out, stream);
 }
 
+tina_status tina_pfb_fft_batched(const void* x, int S, long long n_samples, int P, int M, const float* window,
+                                 tina_kind kind, void* out, void* stream)
+{
+    long long F;
+    tina_status st = pfb_validate(x, S, n_samples, P, M, window, kind, out, "tina_pfb_fft", &F);
+    if (st != TINA_OK) return st;
+    if (kind != TINA_COMPLEX || P != 1024 || M > 16)
+        return fail(TINA_ERR_UNSUPPORTED, "tina_pfb_fft: this version covers the complex kind with P = 1024, M <= 16");
+    return ct_pfb(x, S, n_samples, M, window, out, (cudaStream_t)stream);
+}
+
 tina_status tina_pfb_fir_batched(const void* x, int S, long long n_samples, int P, int M,
                                  const float* window, tina_kind kind, void* y, void* stream)
 {

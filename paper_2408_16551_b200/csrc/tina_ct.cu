@@ -1,0 +1,237 @@
+// tina_ct.cu -- PFB with a FACTORISED Fourier stage on the tensor cores.
+//
+// The paper allows "either a Discrete or Fast Fourier Transform" after the subfilter stage
+// (PAPER.md:233).  tina_pfb keeps the dense P x P contraction the method prescribes (Eq. (12)); this
+// file is the two-stage Cooley-Tukey form of the same transform for P = 1024 = 32 x 32 (complex kind):
+// with p = a + 32 b and k = kb + 32 ka,
+//     G[f][a][kb]  = sum_b y[f][a + 32 b] W32^(b kb)                        (32-point DFTs, stage 1)
+//     G'[f][a][kb] = G[f][a][kb] * W1024^(a kb)                             (twiddle)
+//     X[f][kb + 32 ka] = sum_a G'[f][a][kb] W32^(a ka)                      (32-point DFTs, stage 2)
+// Both stages are 128 x 64 x 64 real-block GEMMs on tcgen05 (bf16x3, fp32 accumulate in TMEM) against
+// the SAME 64 x 64 matrix, with the subfilter stage (Eq. (20)) as producer of the first A tile and the
+// twiddle + transpose done by the first epilogue straight into the second A tile: nothing round-trips
+// through HBM, and the tensor work drops from 8 P^2 to 8 P (32 + 32) flops per frame, which makes the
+// kernel HBM / FMA bound instead of tensor bound.  One CTA = 4 frames per iteration (128 GEMM rows).
+#include "tina_common.cuh"
+#include "tina_ptx.cuh"
+
+#include <cuda_bf16.h>
+
+namespace tina {
+
+using namespace ptx;
+
+constexpr int CT_P = 1024, CT_A = 32, CT_B = 32;      // p = a + CT_A * b
+constexpr int CT_FR = 4;                              // frames per group (CT_FR * 32 = 128 GEMM rows)
+constexpr int CT_THREADS = 512;
+constexpr int CT_TILE = 128 * 64 * 2;                 // one bf16 128 x 64 tile: 16 KB
+
+struct CtSmem {
+    uint8_t a1[2 * CT_TILE];                          // stage-1 A operand hi | lo (also the output staging area)
+    uint8_t a2[2 * CT_TILE];                          // stage-2 A operand hi | lo
+    uint8_t bm[2 * 64 * 64 * 2];                      // W32 block matrix hi | lo, K-major SWIZZLE_128B (64 rows)
+    float2 tw[CT_A * CT_B];                           // W1024^(a kb)
+    uint64_t bar[2];
+    uint32_t tmem_base;
+};
+
+__device__ __forceinline__ uint32_t sw128_off(uint32_t row, uint32_t kbyte)   // byte offset in a K-major SW128 tile
+{
+    return row * 128u + ((((kbyte >> 4) ^ (row & 7u)) << 4) | (kbyte & 15u));
+}
+
+__device__ __forceinline__ void split_store(uint8_t* tile, uint32_t off, float vx, float vy)
+{
+    const __nv_bfloat162 hi = __floats2bfloat162_rn(vx, vy);
+    const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
+    const __nv_bfloat162 lo = __floats2bfloat162_rn(vx - __uint_as_float(hb << 16), vy - __uint_as_float(hb & 0xffff0000u));
+    *reinterpret_cast<uint32_t*>(tile + off) = hb;
+    *reinterpret_cast<uint32_t*>(tile + CT_TILE + off) = *reinterpret_cast<const uint32_t*>(&lo);
+}
+
+template <int MT>
+__global__ void __launch_bounds__(CT_THREADS, 1)
+pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float* __restrict__ window,
+              const __nv_bfloat16* __restrict__ w32, float2* __restrict__ out, long long F, long long NBLK, int M,
+              int groups_per_stream, int total_groups)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    CtSmem& sm = *reinterpret_cast<CtSmem*>(smem_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    // ---- one-time setup: W32 block matrix into the swizzled layout, twiddle table, barriers, TMEM
+    for (int e = tid; e < 2 * 64 * 64; e += CT_THREADS) {
+        const int part = e / 4096, n = (e % 4096) / 64, c = e % 64;
+        *reinterpret_cast<__nv_bfloat16*>(sm.bm + part * 8192 + sw128_off(n, c * 2)) = w32[part * 4096 + n * 64 + c];
+    }
+    for (int e = tid; e < CT_A * CT_B; e += CT_THREADS) {
+        const int a = e / CT_B, kb = e % CT_B;
+        double sn, cs;
+        sincospi(2.0 * (double)((a * kb) % CT_P) / (double)CT_P, &sn, &cs);
+        sm.tw[e] = make_float2((float)cs, (float)-sn);
+    }
+    if (tid == 0) { mbar_init(smem_u32(&sm.bar[0]), 1); mbar_init(smem_u32(&sm.bar[1]), 1); fence_mbar_init(); }
+    if (warp == 0) { tmem_alloc<1>(smem_u32(&sm.tmem_base), 128); tmem_relinquish<1>(); }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+    const uint32_t idesc = idesc_bf16(128, 64);
+    const uint64_t d_a1h = smem_desc_sw128(smem_u32(sm.a1)), d_a1l = smem_desc_sw128(smem_u32(sm.a1 + CT_TILE));
+    const uint64_t d_a2h = smem_desc_sw128(smem_u32(sm.a2)), d_a2l = smem_desc_sw128(smem_u32(sm.a2 + CT_TILE));
+    const uint64_t d_bh = smem_desc_sw128(smem_u32(sm.bm)), d_bl = smem_desc_sw128(smem_u32(sm.bm + 8192));
+
+    constexpr int WA = MT;
+    uint32_t it = 0;
+    for (int g = blockIdx.x; g < total_groups; g += gridDim.x, ++it) {
+        const int s = g / groups_per_stream;
+        const long long f0 = (long long)(g % groups_per_stream) * CT_FR;
+        const float2* xs = x + (long long)s * stream_stride;
+        // ---- subfilter stage, Eq. (20): thread (warp w, lane a) owns p = a + 32 b for b = 2w, 2w+1
+#pragma unroll 1
+        for (int cb = 0; cb < 2; ++cb) {
+            const int b = 2 * warp + cb, p = lane + CT_A * b;
+            float tap[WA];
+            float2 row[WA - 1 + CT_FR];
+#pragma unroll
+            for (int m = 0; m < WA; ++m) tap[m] = m < M ? __ldg(window + (long long)m * CT_P + p) : 0.f;
+            const long long r0 = f0 + M - WA;
+#pragma unroll
+            for (int j = 0; j < WA - 1 + CT_FR; ++j) {
+                const long long r = r0 + j;
+                row[j] = (r >= 0 && r < NBLK) ? __ldg(xs + r * CT_P + p) : make_float2(0.f, 0.f);
+            }
+#pragma unroll
+            for (int fl = 0; fl < CT_FR; ++fl) {
+                float yr = 0.f, yi = 0.f;
+#pragma unroll
+                for (int m = 0; m < WA; ++m) {
+                    yr = fmaf(tap[m], row[fl + WA - 1 - m].x, yr);
+                    yi = fmaf(tap[m], row[fl + WA - 1 - m].y, yi);
+                }
+                split_store(sm.a1, sw128_off(fl * 32 + lane, b * 4), yr, yi);       // row (fl, a), K cell b
+            }
+        }
+        fence_proxy_async();
+        __syncthreads();
+        // ---- stage 1: D1 = A1 * W32  (TMEM columns 0..63)
+        if (tid == 0) {
+            tc_fence_after();
+#pragma unroll
+            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem, d_a1l + 2 * k, d_bh + 2 * k, idesc, k > 0);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem, d_a1h + 2 * k, d_bh + 2 * k, idesc, 1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem, d_a1h + 2 * k, d_bl + 2 * k, idesc, 1);
+            umma_commit(smem_u32(&sm.bar[0]));
+        }
+        mbar_wait(smem_u32(&sm.bar[0]), it & 1u);
+        tc_fence_after();
+        // ---- epilogue 1: twiddle, split, transposed write into A2: row (fl, kb), K cell a
+        if (warp < 4) {
+            const int fl = warp, a = lane;
+            const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16);
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                uint32_t v[32];
+                tmem_ld32(taddr + half * 32, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const int kb = half * 16 + q;
+                    const float gr = __uint_as_float(v[2 * q]), gi = __uint_as_float(v[2 * q + 1]);
+                    const float2 w = sm.tw[a * CT_B + kb];
+                    split_store(sm.a2, sw128_off(fl * 32 + kb, a * 4), gr * w.x - gi * w.y, gr * w.y + gi * w.x);
+                }
+            }
+        }
+        fence_proxy_async();
+        tc_fence_before();
+        __syncthreads();
+        // ---- stage 2: D2 = A2 * W32  (TMEM columns 64..127)
+        if (tid == 0) {
+            tc_fence_after();
+#pragma unroll
+            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64, d_a2l + 2 * k, d_bh + 2 * k, idesc, k > 0);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64, d_a2h + 2 * k, d_bh + 2 * k, idesc, 1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64, d_a2h + 2 * k, d_bl + 2 * k, idesc, 1);
+            umma_commit(smem_u32(&sm.bar[1]));
+        }
+        mbar_wait(smem_u32(&sm.bar[1]), it & 1u);
+        tc_fence_after();
+        // ---- epilogue 2: row (fl, kb) holds X[f][kb + 32 ka] for all ka -> natural order through the A1 area
+        float2* stage = reinterpret_cast<float2*>(sm.a1);                // [fl][ka][kb], 4 x 8 KB
+        if (warp < 4) {
+            const int fl = warp, kb = lane;
+            const uint32_t taddr = tmem + 64 + ((uint32_t)(warp * 32) << 16);
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                uint32_t v[32];
+                tmem_ld32(taddr + half * 32, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 16; ++q)
+                    stage[fl * CT_P + (half * 16 + q) * 32 + kb] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+            }
+        }
+        tc_fence_before();
+        __syncthreads();
+        {
+            float4* o4 = reinterpret_cast<float4*>(out + ((long long)s * F + f0) * CT_P);
+            const float4* s4 = reinterpret_cast<const float4*>(stage);
+#pragma unroll
+            for (int i = 0; i < CT_FR * CT_P / 2 / CT_THREADS; ++i) {
+                const int e = tid + i * CT_THREADS;                      // float4 index; 512 float4 per frame
+                if (f0 + e / 512 < F) o4[e] = s4[e];
+            }
+        }
+        __syncthreads();                                                 // the A1 area is rewritten by the next group
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<1>(tmem, 128);
+}
+
+}  // namespace tina
+
+namespace tina {
+
+// defined in tina_umma.cu: the cached bf16 hi | lo block matrix of a P-point complex DFT ([2][2P][2P], row n = output)
+const __nv_bfloat16* umma_twiddle_plan(int P, bool real, bool inverse, cudaStream_t st, tina_status* status);
+
+tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st)
+{
+    const long long NBLK = n_samples / CT_P, F = NBLK - M + 1;
+    tina_status ps = TINA_OK;
+    const __nv_bfloat16* w32 = umma_twiddle_plan(32, false, false, st, &ps);
+    if (!w32) return ps;
+    const long long gps = (F + CT_FR - 1) / CT_FR;
+    if (gps * S > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb_fft: too many frames");
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaError_t e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ct_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CtSmem) + 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ct_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CtSmem) + 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ct_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CtSmem) + 1024);
+        if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "pfb_ct_kernel setup"); }
+    }
+    const int total = (int)(gps * S);
+    const int per_sm = 1;                                   // 512 threads x ~100 registers: one CTA per SM
+    const int grid = total < n_sm * per_sm ? total : n_sm * per_sm;
+    const size_t smem = sizeof(CtSmem) + 1024;
+    const float2* xf = static_cast<const float2*>(x);
+    float2* of = static_cast<float2*>(out);
+    if (M <= 4) pfb_ct_kernel<4><<<grid, CT_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
+    else if (M <= 8) pfb_ct_kernel<8><<<grid, CT_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
+    else pfb_ct_kernel<16><<<grid, CT_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
+    count_launch();
+    g_last_path = kPathUmma;
+    return check_cuda(cudaGetLastError(), "pfb_ct_kernel launch");
+}
+
+}  // namespace tina

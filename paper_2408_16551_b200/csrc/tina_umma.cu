@@ -200,6 +200,13 @@ static tina_status get_plan(int P, bool real, bool inverse, int parts, bool fp16
     return TINA_OK;
 }
 
+const __nv_bfloat16* umma_twiddle_plan(int P, bool real, bool inverse, cudaStream_t st, tina_status* status)
+{
+    const Plan* pl = nullptr;
+    *status = get_plan(P, real, inverse, 2, false, st, &pl);
+    return *status == TINA_OK ? pl->tt : nullptr;
+}
+
 void umma_clear_plans()
 {
     std::lock_guard<std::mutex> lk(g_plan_mu);

@@ -315,6 +315,23 @@ def test_config5_full_size_sampled(tina, oracle, prec, tol):
     assert np.all(got[:, 0].imag == 0) and np.all(got[:, 2048].imag == 0)
 
 
+@pytest.mark.parametrize("M,F,S", [(16, 130, 1), (4, 7, 2), (8, 257, 1), (1, 64, 1), (16, 1, 1)])
+def test_pfb_fft_factorised_stage(tina, oracle, M, F, S):
+    """tina_pfb_fft_batched (two-stage 32 x 32 Fourier stage on the tensor cores) gives the same result as
+    the oracle's direct O(P^2) DFT, within the fp32 contract; ragged groups of 4 frames, several streams."""
+    rng = np.random.default_rng(40 + M)
+    case = ti.pfb_case(1024, M, F, streams=S, seed=41 + M + F, window=ti.random_taps(rng, 1024 * M))
+    import torch
+    out = tina.pfb_fft(_cuda(case.x), 1024, M, _cuda(case.window)); torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert got.shape == (S, F, 1024)
+    for s in range(S):
+        assert rel_l2_rows(got[s], oracle.pfb(case.x[s], 1024, M, case.window)) <= TOL_FP32
+    with pytest.raises(tina.TinaError) as e:
+        tina.pfb_fft(_cuda(case.x[:, : (F + M - 1) * 512]), 512, M, _cuda(case.window[: 512 * M]))
+    assert e.value.status == 3
+
+
 def test_pfb_fir_only(tina, oracle):
     import torch
     for real in (False, True):
