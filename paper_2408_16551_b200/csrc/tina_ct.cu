@@ -23,7 +23,9 @@ using namespace ptx;
 
 constexpr int CT_P = 1024, CT_A = 32, CT_B = 32;      // p = a + CT_A * b
 constexpr int CT_FR = 4;                              // frames per group (CT_FR * 32 = 128 GEMM rows)
-constexpr int CT_THREADS = 512;
+constexpr int CT_THREADS = 256;                       // 8 warps; two CTAs per SM overlap each other's phases
+constexpr int CT_NW = CT_THREADS / 32;
+constexpr int CT_BPW = CT_B / CT_NW;                  // b values (input columns per lane) per warp
 constexpr int CT_TILE = 128 * 64 * 2;                 // one bf16 128 x 64 tile: 16 KB
 
 struct CtSmem {
@@ -50,7 +52,7 @@ __device__ __forceinline__ void split_store(uint8_t* tile, uint32_t off, float v
 }
 
 template <int MT>
-__global__ void __launch_bounds__(CT_THREADS, 1)
+__global__ void __launch_bounds__(CT_THREADS, 2)
 pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float* __restrict__ window,
               const __nv_bfloat16* __restrict__ w32, float2* __restrict__ out, long long F, long long NBLK, int M,
               int groups_per_stream, int total_groups)
@@ -88,30 +90,38 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         const int s = g / groups_per_stream;
         const long long f0 = (long long)(g % groups_per_stream) * CT_FR;
         const float2* xs = x + (long long)s * stream_stride;
-        // ---- subfilter stage, Eq. (20): thread (warp w, lane a) owns p = a + 32 b for b = 2w, 2w+1
+        // ---- subfilter stage, Eq. (20): thread (warp w, lane a) owns p = a + 32 b for b = CT_BPW w .. CT_BPW w + CT_BPW - 1,
+        //      two columns at a time (their loads are in flight together)
 #pragma unroll 1
-        for (int cb = 0; cb < 2; ++cb) {
-            const int b = 2 * warp + cb, p = lane + CT_A * b;
-            float tap[WA];
-            float2 row[WA - 1 + CT_FR];
+        for (int cb = 0; cb < CT_BPW; cb += 2) {
+            const int b = CT_BPW * warp + cb, p = lane + CT_A * b;
+            float tap[2][WA];
+            float2 row[2][WA - 1 + CT_FR];
 #pragma unroll
-            for (int m = 0; m < WA; ++m) tap[m] = m < M ? __ldg(window + (long long)m * CT_P + p) : 0.f;
+            for (int m = 0; m < WA; ++m) {
+                tap[0][m] = m < M ? __ldg(window + (long long)m * CT_P + p) : 0.f;
+                tap[1][m] = m < M ? __ldg(window + (long long)m * CT_P + p + CT_A) : 0.f;
+            }
             const long long r0 = f0 + M - WA;
 #pragma unroll
             for (int j = 0; j < WA - 1 + CT_FR; ++j) {
                 const long long r = r0 + j;
-                row[j] = (r >= 0 && r < NBLK) ? __ldg(xs + r * CT_P + p) : make_float2(0.f, 0.f);
+                const bool ok = r >= 0 && r < NBLK;
+                row[0][j] = ok ? __ldg(xs + r * CT_P + p) : make_float2(0.f, 0.f);
+                row[1][j] = ok ? __ldg(xs + r * CT_P + p + CT_A) : make_float2(0.f, 0.f);
             }
 #pragma unroll
-            for (int fl = 0; fl < CT_FR; ++fl) {
-                float yr = 0.f, yi = 0.f;
+            for (int c2 = 0; c2 < 2; ++c2)
 #pragma unroll
-                for (int m = 0; m < WA; ++m) {
-                    yr = fmaf(tap[m], row[fl + WA - 1 - m].x, yr);
-                    yi = fmaf(tap[m], row[fl + WA - 1 - m].y, yi);
+                for (int fl = 0; fl < CT_FR; ++fl) {
+                    float yr = 0.f, yi = 0.f;
+#pragma unroll
+                    for (int m = 0; m < WA; ++m) {
+                        yr = fmaf(tap[c2][m], row[c2][fl + WA - 1 - m].x, yr);
+                        yi = fmaf(tap[c2][m], row[c2][fl + WA - 1 - m].y, yi);
+                    }
+                    split_store(sm.a1, sw128_off(fl * 32 + lane, (b + c2) * 4), yr, yi);   // row (fl, a), K cell b
                 }
-                split_store(sm.a1, sw128_off(fl * 32 + lane, b * 4), yr, yi);       // row (fl, a), K cell b
-            }
         }
         fence_proxy_async();
         __syncthreads();
@@ -129,21 +139,19 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         mbar_wait(smem_u32(&sm.bar[0]), it & 1u);
         tc_fence_after();
         // ---- epilogue 1: twiddle, split, transposed write into A2: row (fl, kb), K cell a
-        if (warp < 4) {
-            const int fl = warp, a = lane;
-            const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16);
+        {
+            // warp w reads TMEM lanes 32 (w % 4) .. +31 (rows (fl, a)) and the column slice w / 4
+            constexpr int CPW = 64 / (CT_NW / 4);                 // accumulator columns per warp (32)
+            const int fl = warp & 3, a = lane, c0 = (warp >> 2) * CPW;
+            uint32_t v[32];
+            tmem_ld32(tmem + ((uint32_t)(fl * 32) << 16) + c0, v);
+            tmem_ld_wait();
 #pragma unroll
-            for (int half = 0; half < 2; ++half) {
-                uint32_t v[32];
-                tmem_ld32(taddr + half * 32, v);
-                tmem_ld_wait();
-#pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    const int kb = half * 16 + q;
-                    const float gr = __uint_as_float(v[2 * q]), gi = __uint_as_float(v[2 * q + 1]);
-                    const float2 w = sm.tw[a * CT_B + kb];
-                    split_store(sm.a2, sw128_off(fl * 32 + kb, a * 4), gr * w.x - gi * w.y, gr * w.y + gi * w.x);
-                }
+            for (int q = 0; q < CPW / 2; ++q) {
+                const int kb = c0 / 2 + q;
+                const float gr = __uint_as_float(v[2 * q]), gi = __uint_as_float(v[2 * q + 1]);
+                const float2 w = sm.tw[a * CT_B + kb];
+                split_store(sm.a2, sw128_off(fl * 32 + kb, a * 4), gr * w.x - gi * w.y, gr * w.y + gi * w.x);
             }
         }
         fence_proxy_async();
@@ -164,18 +172,15 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         tc_fence_after();
         // ---- epilogue 2: row (fl, kb) holds X[f][kb + 32 ka] for all ka -> natural order through the A1 area
         float2* stage = reinterpret_cast<float2*>(sm.a1);                // [fl][ka][kb], 4 x 8 KB
-        if (warp < 4) {
-            const int fl = warp, kb = lane;
-            const uint32_t taddr = tmem + 64 + ((uint32_t)(warp * 32) << 16);
+        {
+            constexpr int CPW = 64 / (CT_NW / 4);
+            const int fl = warp & 3, kb = lane, c0 = (warp >> 2) * CPW;
+            uint32_t v[32];
+            tmem_ld32(tmem + 64 + ((uint32_t)(fl * 32) << 16) + c0, v);
+            tmem_ld_wait();
 #pragma unroll
-            for (int half = 0; half < 2; ++half) {
-                uint32_t v[32];
-                tmem_ld32(taddr + half * 32, v);
-                tmem_ld_wait();
-#pragma unroll
-                for (int q = 0; q < 16; ++q)
-                    stage[fl * CT_P + (half * 16 + q) * 32 + kb] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-            }
+            for (int q = 0; q < CPW / 2; ++q)
+                stage[fl * CT_P + (c0 / 2 + q) * 32 + kb] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
         }
         tc_fence_before();
         __syncthreads();
@@ -221,7 +226,7 @@ tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float
         if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "pfb_ct_kernel setup"); }
     }
     const int total = (int)(gps * S);
-    const int per_sm = 1;                                   // 512 threads x ~100 registers: one CTA per SM
+    const int per_sm = 2;                                   // 256 threads, 89 KB shared memory, 128 TMEM columns per CTA
     const int grid = total < n_sm * per_sm ? total : n_sm * per_sm;
     const size_t smem = sizeof(CtSmem) + 1024;
     const float2* xf = static_cast<const float2*>(x);
