@@ -11,26 +11,31 @@
 // the SAME 64 x 64 matrix, with the subfilter stage (Eq. (20)) as producer of the first A tile and the
 // twiddle + transpose done by the first epilogue straight into the second A tile: nothing round-trips
 // through HBM, and the tensor work drops from 8 P^2 to 8 P (32 + 32) flops per frame, which makes the
-// kernel HBM / FMA bound instead of tensor bound.  One CTA = 4 frames per iteration (128 GEMM rows).
+// kernel HBM / FMA bound instead of tensor bound.  One CTA = 8 frames per iteration (two 128-row GEMM tiles); one shared-memory area serves as first A operand, second A operand and output staging in turn.
 #include "tina_common.cuh"
 #include "tina_ptx.cuh"
 
 #include <cuda_bf16.h>
+#include <cstdlib>
 
 namespace tina {
 
 using namespace ptx;
 
 constexpr int CT_P = 1024, CT_A = 32, CT_B = 32;      // p = a + CT_A * b
-constexpr int CT_FR = 4;                              // frames per group (CT_FR * 32 = 128 GEMM rows)
+constexpr int CT_FR = 8;                              // frames per group: CT_NT GEMM tiles of 4 frames x 32 rows
+constexpr int CT_NT = CT_FR / 4;
 constexpr int CT_THREADS = 256;                       // 8 warps; two CTAs per SM overlap each other's phases
 constexpr int CT_NW = CT_THREADS / 32;
 constexpr int CT_BPW = CT_B / CT_NW;                  // b values (input columns per lane) per warp
 constexpr int CT_TILE = 128 * 64 * 2;                 // one bf16 128 x 64 tile: 16 KB
+static_assert(CT_NW == 4 * CT_NT, "one warp per (tile, TMEM lane quarter) in the epilogues");
 
 struct CtSmem {
-    uint8_t a1[2 * CT_TILE];                          // stage-1 A operand hi | lo (also the output staging area)
-    uint8_t a2[2 * CT_TILE];                          // stage-2 A operand hi | lo
+    // per tile hi | lo.  The same area is, in turn, the stage-1 A operand (written by the subfilter stage), the
+    // stage-2 A operand (written by epilogue 1 once the stage-1 MMAs have retired) and the fp32 output staging area
+    // (written by epilogue 2 once the stage-2 MMAs have retired): CT_FR frames x 8 KB.
+    uint8_t a[CT_NT * 2 * CT_TILE];
     uint8_t bm[2 * 64 * 64 * 2];                      // W32 block matrix hi | lo, K-major SWIZZLE_128B (64 rows)
     float2 tw[CT_A * CT_B];                           // W1024^(a kb)
     uint64_t bar[2];
@@ -49,6 +54,16 @@ __device__ __forceinline__ void split_store(uint8_t* tile, uint32_t off, float v
     const __nv_bfloat162 lo = __floats2bfloat162_rn(vx - __uint_as_float(hb << 16), vy - __uint_as_float(hb & 0xffff0000u));
     *reinterpret_cast<uint32_t*>(tile + off) = hb;
     *reinterpret_cast<uint32_t*>(tile + CT_TILE + off) = *reinterpret_cast<const uint32_t*>(&lo);
+}
+
+// d = (a, a) * b + c on a packed fp32 pair (fma.rn.f32x2, SASS FFMA2 with a broadcast scalar operand)
+__device__ __forceinline__ float2 ffma2_bc(float a, float2 b, float2 c)
+{
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %2};\n\tmov.b64 rb, {%3, %4};\n\tmov.b64 rc, {%5, %6};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return d;
 }
 
 template <int MT>
@@ -80,107 +95,104 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
     const uint32_t idesc = idesc_bf16(128, 64);
-    const uint64_t d_a1h = smem_desc_sw128(smem_u32(sm.a1)), d_a1l = smem_desc_sw128(smem_u32(sm.a1 + CT_TILE));
-    const uint64_t d_a2h = smem_desc_sw128(smem_u32(sm.a2)), d_a2l = smem_desc_sw128(smem_u32(sm.a2 + CT_TILE));
+    const uint64_t d_ah = smem_desc_sw128(smem_u32(sm.a)), d_al = smem_desc_sw128(smem_u32(sm.a + CT_TILE));
     const uint64_t d_bh = smem_desc_sw128(smem_u32(sm.bm)), d_bl = smem_desc_sw128(smem_u32(sm.bm + 8192));
+    constexpr uint64_t TILE_DESC = (uint64_t)(2 * CT_TILE) >> 4;          // descriptor step from one tile to the next
 
     constexpr int WA = MT;
+    const int et = warp >> 2, eq = warp & 3;                              // epilogue role: tile, TMEM lane quarter
+    uint8_t* const etile = sm.a + et * 2 * CT_TILE;
     uint32_t it = 0;
     for (int g = blockIdx.x; g < total_groups; g += gridDim.x, ++it) {
         const int s = g / groups_per_stream;
         const long long f0 = (long long)(g % groups_per_stream) * CT_FR;
         const float2* xs = x + (long long)s * stream_stride;
         // ---- subfilter stage, Eq. (20): thread (warp w, lane a) owns p = a + 32 b for b = CT_BPW w .. CT_BPW w + CT_BPW - 1,
-        //      two columns at a time (their loads are in flight together)
+        //      one column at a time: WA - 1 + CT_FR rows and WA taps in registers, CT_FR outputs
 #pragma unroll 1
-        for (int cb = 0; cb < CT_BPW; cb += 2) {
+        for (int cb = 0; cb < CT_BPW; ++cb) {
             const int b = CT_BPW * warp + cb, p = lane + CT_A * b;
-            float tap[2][WA];
-            float2 row[2][WA - 1 + CT_FR];
+            float tap[WA];
+            float2 row[WA - 1 + CT_FR];
 #pragma unroll
-            for (int m = 0; m < WA; ++m) {
-                tap[0][m] = m < M ? __ldg(window + (long long)m * CT_P + p) : 0.f;
-                tap[1][m] = m < M ? __ldg(window + (long long)m * CT_P + p + CT_A) : 0.f;
-            }
+            for (int m = 0; m < WA; ++m) tap[m] = m < M ? __ldg(window + (long long)m * CT_P + p) : 0.f;
             const long long r0 = f0 + M - WA;
 #pragma unroll
             for (int j = 0; j < WA - 1 + CT_FR; ++j) {
                 const long long r = r0 + j;
-                const bool ok = r >= 0 && r < NBLK;
-                row[0][j] = ok ? __ldg(xs + r * CT_P + p) : make_float2(0.f, 0.f);
-                row[1][j] = ok ? __ldg(xs + r * CT_P + p + CT_A) : make_float2(0.f, 0.f);
+                row[j] = (r >= 0 && r < NBLK) ? __ldg(xs + r * CT_P + p) : make_float2(0.f, 0.f);
             }
 #pragma unroll
-            for (int c2 = 0; c2 < 2; ++c2)
+            for (int fl = 0; fl < CT_FR; ++fl) {
+                float2 y = make_float2(0.f, 0.f);
 #pragma unroll
-                for (int fl = 0; fl < CT_FR; ++fl) {
-                    float yr = 0.f, yi = 0.f;
-#pragma unroll
-                    for (int m = 0; m < WA; ++m) {
-                        yr = fmaf(tap[c2][m], row[c2][fl + WA - 1 - m].x, yr);
-                        yi = fmaf(tap[c2][m], row[c2][fl + WA - 1 - m].y, yi);
-                    }
-                    split_store(sm.a1, sw128_off(fl * 32 + lane, (b + c2) * 4), yr, yi);   // row (fl, a), K cell b
-                }
+                for (int m = 0; m < WA; ++m) y = ffma2_bc(tap[m], row[fl + WA - 1 - m], y);
+                split_store(sm.a + (fl >> 2) * 2 * CT_TILE, sw128_off((fl & 3) * 32 + lane, b * 4), y.x, y.y);   // row (fl, a), K cell b
+            }
         }
         fence_proxy_async();
         __syncthreads();
-        // ---- stage 1: D1 = A1 * W32  (TMEM columns 0..63)
+        // ---- stage 1: D1 = A1 * W32  (tile t -> TMEM columns 64 t .. 64 t + 63)
         if (tid == 0) {
             tc_fence_after();
 #pragma unroll
-            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem, d_a1l + 2 * k, d_bh + 2 * k, idesc, k > 0);
+            for (int t = 0; t < CT_NT; ++t) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem, d_a1h + 2 * k, d_bh + 2 * k, idesc, 1);
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, k > 0);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem, d_a1h + 2 * k, d_bl + 2 * k, idesc, 1);
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_ah + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, 1);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_ah + t * TILE_DESC + 2 * k, d_bl + 2 * k, idesc, 1);
+            }
             umma_commit(smem_u32(&sm.bar[0]));
         }
         mbar_wait(smem_u32(&sm.bar[0]), it & 1u);
         tc_fence_after();
-        // ---- epilogue 1: twiddle, split, transposed write into A2: row (fl, kb), K cell a
-        {
-            // warp w reads TMEM lanes 32 (w % 4) .. +31 (rows (fl, a)) and the column slice w / 4
-            constexpr int CPW = 64 / (CT_NW / 4);                 // accumulator columns per warp (32)
-            const int fl = warp & 3, a = lane, c0 = (warp >> 2) * CPW;
+        // ---- epilogue 1: twiddle, split, transposed write into A2 (over A1: its MMAs have retired): row (fl, kb), K cell a.
+        //      Warp (et, eq) reads TMEM lanes 32 eq .. +31 (rows (fl = eq, a = lane)) of tile et.
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
             uint32_t v[32];
-            tmem_ld32(tmem + ((uint32_t)(fl * 32) << 16) + c0, v);
+            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 64 * et + 32 * h, v);
             tmem_ld_wait();
 #pragma unroll
-            for (int q = 0; q < CPW / 2; ++q) {
-                const int kb = c0 / 2 + q;
+            for (int q = 0; q < 16; ++q) {
+                const int kb = 16 * h + q;
                 const float gr = __uint_as_float(v[2 * q]), gi = __uint_as_float(v[2 * q + 1]);
-                const float2 w = sm.tw[a * CT_B + kb];
-                split_store(sm.a2, sw128_off(fl * 32 + kb, a * 4), gr * w.x - gi * w.y, gr * w.y + gi * w.x);
+                const float2 w = sm.tw[lane * CT_B + kb];
+                split_store(etile, sw128_off(eq * 32 + kb, lane * 4), gr * w.x - gi * w.y, gr * w.y + gi * w.x);
             }
         }
         fence_proxy_async();
         tc_fence_before();
         __syncthreads();
-        // ---- stage 2: D2 = A2 * W32  (TMEM columns 64..127)
+        // ---- stage 2: D2 = A2 * W32  (over D1: every warp has read its part)
         if (tid == 0) {
             tc_fence_after();
 #pragma unroll
-            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64, d_a2l + 2 * k, d_bh + 2 * k, idesc, k > 0);
+            for (int t = 0; t < CT_NT; ++t) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64, d_a2h + 2 * k, d_bh + 2 * k, idesc, 1);
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, k > 0);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64, d_a2h + 2 * k, d_bl + 2 * k, idesc, 1);
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_ah + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, 1);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_ah + t * TILE_DESC + 2 * k, d_bl + 2 * k, idesc, 1);
+            }
             umma_commit(smem_u32(&sm.bar[1]));
         }
         mbar_wait(smem_u32(&sm.bar[1]), it & 1u);
         tc_fence_after();
-        // ---- epilogue 2: row (fl, kb) holds X[f][kb + 32 ka] for all ka -> natural order through the A1 area
-        float2* stage = reinterpret_cast<float2*>(sm.a1);                // [fl][ka][kb], 4 x 8 KB
-        {
-            constexpr int CPW = 64 / (CT_NW / 4);
-            const int fl = warp & 3, kb = lane, c0 = (warp >> 2) * CPW;
+        // ---- epilogue 2: row (fl, kb) holds X[f][kb + 32 ka] for all ka -> natural order [fl][ka][kb] over the A area.
+        //      All stage-2 MMAs have retired, and each warp only reads TMEM, so the overwrite is safe.
+        float2* stage = reinterpret_cast<float2*>(sm.a);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
             uint32_t v[32];
-            tmem_ld32(tmem + 64 + ((uint32_t)(fl * 32) << 16) + c0, v);
+            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 64 * et + 32 * h, v);
             tmem_ld_wait();
 #pragma unroll
-            for (int q = 0; q < CPW / 2; ++q)
-                stage[fl * CT_P + (c0 / 2 + q) * 32 + kb] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+            for (int q = 0; q < 16; ++q)
+                stage[(et * 4 + eq) * CT_P + (16 * h + q) * 32 + lane] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
         }
         tc_fence_before();
         __syncthreads();
@@ -193,7 +205,7 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
                 if (f0 + e / 512 < F) o4[e] = s4[e];
             }
         }
-        __syncthreads();                                                 // the A1 area is rewritten by the next group
+        __syncthreads();                                                 // the A area is rewritten by the next group
     }
     tc_fence_before();
     __syncthreads();
