@@ -37,7 +37,7 @@ struct CtSmem {
     // (written by epilogue 2 once the stage-2 MMAs have retired): CT_FR frames x 8 KB.
     uint8_t a[CT_NT * 2 * CT_TILE];
     uint8_t bm[2 * 64 * 64 * 2];                      // W32 block matrix hi | lo, K-major SWIZZLE_128B (64 rows)
-    float2 tw[CT_A * CT_B];                           // W1024^(a kb)
+    float2 tw[CT_A * CT_B];                           // W1024^(a kb), [kb][a]
     uint64_t bar[2];
     uint32_t tmem_base;
 };
@@ -66,6 +66,14 @@ __device__ __forceinline__ float2 ffma2_bc(float a, float2 b, float2 c)
     return d;
 }
 
+// streaming load of an input sample: no reuse in L1, which is left to the window taps
+__device__ __forceinline__ float2 ldg_stream(const float2* p)
+{
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 template <int MT>
 __global__ void __launch_bounds__(CT_THREADS, 2)
 pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float* __restrict__ window,
@@ -82,7 +90,7 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         *reinterpret_cast<__nv_bfloat16*>(sm.bm + part * 8192 + sw128_off(n, c * 2)) = w32[part * 4096 + n * 64 + c];
     }
     for (int e = tid; e < CT_A * CT_B; e += CT_THREADS) {
-        const int a = e / CT_B, kb = e % CT_B;
+        const int kb = e / CT_A, a = e % CT_A;                          // [kb][a]: a lane reads consecutive a
         double sn, cs;
         sincospi(2.0 * (double)((a * kb) % CT_P) / (double)CT_P, &sn, &cs);
         sm.tw[e] = make_float2((float)cs, (float)-sn);
@@ -102,6 +110,8 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
     constexpr int WA = MT;
     const int et = warp >> 2, eq = warp & 3;                              // epilogue role: tile, TMEM lane quarter
     uint8_t* const etile = sm.a + et * 2 * CT_TILE;
+    const uint32_t fir_off = lane * 128 + ((warp ^ (lane & 7)) << 4);
+    static_assert(CT_BPW == 4, "one 16-byte swizzle chunk per warp");
     uint32_t it = 0;
     for (int g = blockIdx.x; g < total_groups; g += gridDim.x, ++it) {
         const int s = g / groups_per_stream;
@@ -109,25 +119,37 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         const float2* xs = x + (long long)s * stream_stride;
         // ---- subfilter stage, Eq. (20): thread (warp w, lane a) owns p = a + 32 b for b = CT_BPW w .. CT_BPW w + CT_BPW - 1,
         //      one column at a time: WA - 1 + CT_FR rows and WA taps in registers, CT_FR outputs
+        //      The shared-memory offset of (row (fl, a), K cell b) is fir_off + constants: b = 4 warp + cb puts the column in
+        //      16-byte chunk `warp` of its row, and the 128-byte swizzle XORs the chunk with a & 7.
+        const long long r0 = f0 + M - WA;
+        const bool interior = M == WA && r0 >= 0 && r0 + WA - 1 + CT_FR <= NBLK;   // every row and tap exists (uniform)
+        const float2* xg = xs + r0 * CT_P + lane + CT_A * CT_BPW * warp;
+        const float* wg = window + lane + CT_A * CT_BPW * warp;
 #pragma unroll 1
-        for (int cb = 0; cb < CT_BPW; ++cb) {
-            const int b = CT_BPW * warp + cb, p = lane + CT_A * b;
+        for (int cb = 0; cb < CT_BPW; ++cb, xg += CT_A, wg += CT_A) {
             float tap[WA];
             float2 row[WA - 1 + CT_FR];
+            if (interior) {
 #pragma unroll
-            for (int m = 0; m < WA; ++m) tap[m] = m < M ? __ldg(window + (long long)m * CT_P + p) : 0.f;
-            const long long r0 = f0 + M - WA;
+                for (int m = 0; m < WA; ++m) tap[m] = __ldg(wg + m * CT_P);
 #pragma unroll
-            for (int j = 0; j < WA - 1 + CT_FR; ++j) {
-                const long long r = r0 + j;
-                row[j] = (r >= 0 && r < NBLK) ? __ldg(xs + r * CT_P + p) : make_float2(0.f, 0.f);
+                for (int j = 0; j < WA - 1 + CT_FR; ++j) row[j] = ldg_stream(xg + j * CT_P);
+            } else {
+#pragma unroll
+                for (int m = 0; m < WA; ++m) tap[m] = m < M ? __ldg(wg + m * CT_P) : 0.f;
+#pragma unroll
+                for (int j = 0; j < WA - 1 + CT_FR; ++j) {
+                    const long long r = r0 + j;
+                    row[j] = (r >= 0 && r < NBLK) ? ldg_stream(xg + j * CT_P) : make_float2(0.f, 0.f);
+                }
             }
+            uint8_t* const dst = sm.a + fir_off + cb * 4;
 #pragma unroll
             for (int fl = 0; fl < CT_FR; ++fl) {
-                float2 y = make_float2(0.f, 0.f);
+                float2 y = make_float2(tap[0] * row[fl + WA - 1].x, tap[0] * row[fl + WA - 1].y);
 #pragma unroll
-                for (int m = 0; m < WA; ++m) y = ffma2_bc(tap[m], row[fl + WA - 1 - m], y);
-                split_store(sm.a + (fl >> 2) * 2 * CT_TILE, sw128_off((fl & 3) * 32 + lane, b * 4), y.x, y.y);   // row (fl, a), K cell b
+                for (int m = 1; m < WA; ++m) y = ffma2_bc(tap[m], row[fl + WA - 1 - m], y);
+                split_store(dst + (fl >> 2) * 2 * CT_TILE, (fl & 3) * 32 * 128, y.x, y.y);
             }
         }
         fence_proxy_async();
@@ -159,7 +181,7 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
             for (int q = 0; q < 16; ++q) {
                 const int kb = 16 * h + q;
                 const float gr = __uint_as_float(v[2 * q]), gi = __uint_as_float(v[2 * q + 1]);
-                const float2 w = sm.tw[lane * CT_B + kb];
+                const float2 w = sm.tw[kb * CT_A + lane];
                 split_store(etile, sw128_off(eq * 32 + kb, lane * 4), gr * w.x - gi * w.y, gr * w.y + gi * w.x);
             }
         }
