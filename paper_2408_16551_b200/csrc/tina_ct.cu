@@ -56,6 +56,15 @@ __device__ __forceinline__ void split_store(uint8_t* tile, uint32_t off, float v
     *reinterpret_cast<uint32_t*>(tile + CT_TILE + off) = *reinterpret_cast<const uint32_t*>(&lo);
 }
 
+// (vx, vy) -> packed bf16 pairs: hi = round(v), lo = round(v - hi)
+__device__ __forceinline__ void split_pack(float vx, float vy, uint32_t& hb, uint32_t& lb)
+{
+    const __nv_bfloat162 hi = __floats2bfloat162_rn(vx, vy);
+    hb = *reinterpret_cast<const uint32_t*>(&hi);
+    const __nv_bfloat162 lo = __floats2bfloat162_rn(vx - __uint_as_float(hb << 16), vy - __uint_as_float(hb & 0xffff0000u));
+    lb = *reinterpret_cast<const uint32_t*>(&lo);
+}
+
 // d = (a, a) * b + c on a packed fp32 pair (fma.rn.f32x2, SASS FFMA2 with a broadcast scalar operand)
 __device__ __forceinline__ float2 ffma2_bc(float a, float2 b, float2 c)
 {
@@ -96,7 +105,7 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         sm.tw[e] = make_float2((float)cs, (float)-sn);
     }
     if (tid == 0) { mbar_init(smem_u32(&sm.bar[0]), 1); mbar_init(smem_u32(&sm.bar[1]), 1); fence_mbar_init(); }
-    if (warp == 0) { tmem_alloc<1>(smem_u32(&sm.tmem_base), 128); tmem_relinquish<1>(); }
+    if (warp == 0) { tmem_alloc<1>(smem_u32(&sm.tmem_base), 256); tmem_relinquish<1>(); }
     fence_proxy_async();
     tc_fence_before();
     __syncthreads();
@@ -111,6 +120,19 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
     const int et = warp >> 2, eq = warp & 3;                              // epilogue role: tile, TMEM lane quarter
     uint8_t* const etile = sm.a + et * 2 * CT_TILE;
     const uint32_t fir_off = lane * 128 + ((warp ^ (lane & 7)) << 4);
+    // ---- the window taps of this thread's CT_BPW columns live in TMEM columns 128..255 (its own lane of its warp's lane
+    //      quarter; 16 columns per input column, zero beyond M): tensor memory the accumulators leave unused serves as a
+    //      per-thread constant store, so the subfilter stage re-reads no taps through L1 / L2.
+    const uint32_t tap_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + 128 + (warp >> 2) * 64;
+#pragma unroll 1
+    for (int cb = 0; cb < CT_BPW; ++cb) {
+        uint32_t tv[16];
+#pragma unroll
+        for (int m = 0; m < 16; ++m)
+            tv[m] = m < M ? __float_as_uint(__ldg(window + (long long)m * CT_P + lane + CT_A * (CT_BPW * warp + cb))) : 0u;
+        tmem_st16(tap_addr + cb * 16, tv);
+    }
+    tmem_st_wait();
     static_assert(CT_BPW == 4, "one 16-byte swizzle chunk per warp");
     uint32_t it = 0;
     for (int g = blockIdx.x; g < total_groups; g += gridDim.x, ++it) {
@@ -122,34 +144,41 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         //      The shared-memory offset of (row (fl, a), K cell b) is fir_off + constants: b = 4 warp + cb puts the column in
         //      16-byte chunk `warp` of its row, and the 128-byte swizzle XORs the chunk with a & 7.
         const long long r0 = f0 + M - WA;
-        const bool interior = M == WA && r0 >= 0 && r0 + WA - 1 + CT_FR <= NBLK;   // every row and tap exists (uniform)
+        const bool interior = r0 >= 0 && r0 + WA - 1 + CT_FR <= NBLK;      // every row of the group exists (uniform)
         const float2* xg = xs + r0 * CT_P + lane + CT_A * CT_BPW * warp;
-        const float* wg = window + lane + CT_A * CT_BPW * warp;
-#pragma unroll 1
-        for (int cb = 0; cb < CT_BPW; ++cb, xg += CT_A, wg += CT_A) {
-            float tap[WA];
+        uint32_t hprev[CT_FR], lprev[CT_FR];                               // the even column's results wait for the odd one
+#pragma unroll
+        for (int cb = 0; cb < CT_BPW; ++cb) {
+            uint32_t tv[16];
             float2 row[WA - 1 + CT_FR];
+            tmem_ld16(tap_addr + cb * 16, tv);
             if (interior) {
 #pragma unroll
-                for (int m = 0; m < WA; ++m) tap[m] = __ldg(wg + m * CT_P);
-#pragma unroll
-                for (int j = 0; j < WA - 1 + CT_FR; ++j) row[j] = ldg_stream(xg + j * CT_P);
+                for (int j = 0; j < WA - 1 + CT_FR; ++j) row[j] = ldg_stream(xg + cb * CT_A + j * CT_P);
             } else {
-#pragma unroll
-                for (int m = 0; m < WA; ++m) tap[m] = m < M ? __ldg(wg + m * CT_P) : 0.f;
 #pragma unroll
                 for (int j = 0; j < WA - 1 + CT_FR; ++j) {
                     const long long r = r0 + j;
-                    row[j] = (r >= 0 && r < NBLK) ? ldg_stream(xg + j * CT_P) : make_float2(0.f, 0.f);
+                    row[j] = (r >= 0 && r < NBLK) ? ldg_stream(xg + cb * CT_A + j * CT_P) : make_float2(0.f, 0.f);
                 }
             }
-            uint8_t* const dst = sm.a + fir_off + cb * 4;
+            tmem_ld_wait();
 #pragma unroll
             for (int fl = 0; fl < CT_FR; ++fl) {
-                float2 y = make_float2(tap[0] * row[fl + WA - 1].x, tap[0] * row[fl + WA - 1].y);
+                const float t0 = __uint_as_float(tv[0]);
+                float2 y = make_float2(t0 * row[fl + WA - 1].x, t0 * row[fl + WA - 1].y);
 #pragma unroll
-                for (int m = 1; m < WA; ++m) y = ffma2_bc(tap[m], row[fl + WA - 1 - m], y);
-                split_store(dst + (fl >> 2) * 2 * CT_TILE, (fl & 3) * 32 * 128, y.x, y.y);
+                for (int m = 1; m < WA; ++m) y = ffma2_bc(__uint_as_float(tv[m]), row[fl + WA - 1 - m], y);
+                uint32_t hb, lb;
+                split_pack(y.x, y.y, hb, lb);
+                if (cb & 1) {                                              // K cells b - 1, b: one 8-byte store per part
+                    uint8_t* const dst = sm.a + fir_off + (cb - 1) * 4 + (fl >> 2) * 2 * CT_TILE + (fl & 3) * 32 * 128;
+                    *reinterpret_cast<uint2*>(dst) = make_uint2(hprev[fl], hb);
+                    *reinterpret_cast<uint2*>(dst + CT_TILE) = make_uint2(lprev[fl], lb);
+                } else {
+                    hprev[fl] = hb;
+                    lprev[fl] = lb;
+                }
             }
         }
         fence_proxy_async();
@@ -231,7 +260,7 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) tmem_dealloc<1>(tmem, 128);
+    if (warp == 0) tmem_dealloc<1>(tmem, 256);
 }
 
 }  // namespace tina
