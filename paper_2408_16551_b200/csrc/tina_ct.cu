@@ -32,9 +32,8 @@ constexpr int CT_TILE = 128 * 64 * 2;                 // one bf16 128 x 64 tile:
 static_assert(CT_NW == 4 * CT_NT, "one warp per (tile, TMEM lane quarter) in the epilogues");
 
 struct CtSmem {
-    // per tile hi | lo.  The same area is, in turn, the stage-1 A operand (written by the subfilter stage), the
-    // stage-2 A operand (written by epilogue 1 once the stage-1 MMAs have retired) and the fp32 output staging area
-    // (written by epilogue 2 once the stage-2 MMAs have retired): CT_FR frames x 8 KB.
+    // per tile hi | lo.  The same area is, in turn, the stage-1 A operand (written by the subfilter stage) and the
+    // stage-2 A operand (written by epilogue 1 once the stage-1 MMAs have retired).
     uint8_t a[CT_NT * 2 * CT_TILE];
     uint8_t bm[2 * 64 * 64 * 2];                      // W32 block matrix hi | lo, K-major SWIZZLE_128B (64 rows)
     float2 tw[CT_A * CT_B];                           // W1024^(a kb), [kb][a]
@@ -233,30 +232,25 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         }
         mbar_wait(smem_u32(&sm.bar[1]), it & 1u);
         tc_fence_after();
-        // ---- epilogue 2: row (fl, kb) holds X[f][kb + 32 ka] for all ka -> natural order [fl][ka][kb] over the A area.
-        //      All stage-2 MMAs have retired, and each warp only reads TMEM, so the overwrite is safe.
-        float2* stage = reinterpret_cast<float2*>(sm.a);
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            uint32_t v[32];
-            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 64 * et + 32 * h, v);
-            tmem_ld_wait();
-#pragma unroll
-            for (int q = 0; q < 16; ++q)
-                stage[(et * 4 + eq) * CT_P + (16 * h + q) * 32 + lane] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-        }
-        tc_fence_before();
-        __syncthreads();
+        // ---- epilogue 2: row (fl, kb) holds X[f][kb + 32 ka] for all ka: for a fixed ka the 32 lanes of a warp hold 32
+        //      consecutive channels, so the accumulators go straight to global memory, 256 contiguous bytes per store.
         {
-            float4* o4 = reinterpret_cast<float4*>(out + ((long long)s * F + f0) * CT_P);
-            const float4* s4 = reinterpret_cast<const float4*>(stage);
+            const long long f = f0 + et * 4 + eq;
+            float2* const orow = out + ((long long)s * F + f) * CT_P + lane;
 #pragma unroll
-            for (int i = 0; i < CT_FR * CT_P / 2 / CT_THREADS; ++i) {
-                const int e = tid + i * CT_THREADS;                      // float4 index; 512 float4 per frame
-                if (f0 + e / 512 < F) o4[e] = s4[e];
+            for (int h = 0; h < 2; ++h) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 64 * et + 32 * h, v);
+                tmem_ld_wait();
+                if (f < F) {
+#pragma unroll
+                    for (int q = 0; q < 16; ++q)
+                        orow[(16 * h + q) * 32] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+                }
             }
         }
-        __syncthreads();                                                 // the A area is rewritten by the next group
+        tc_fence_before();
+        __syncthreads();                                                 // TMEM and the A area are rewritten by the next group
     }
     tc_fence_before();
     __syncthreads();
