@@ -11,7 +11,7 @@
 // the SAME 64 x 64 matrix, with the subfilter stage (Eq. (20)) as producer of the first A tile and the
 // twiddle + transpose done by the first epilogue straight into the second A tile: nothing round-trips
 // through HBM, and the tensor work drops from 8 P^2 to 8 P (32 + 32) flops per frame, which makes the
-// kernel HBM / FMA bound instead of tensor bound.  One CTA = 8 frames per iteration (two 128-row GEMM tiles); one shared-memory area serves as first A operand, second A operand and output staging in turn.
+// kernel HBM / FMA bound instead of tensor bound.  One CTA = 8 frames per iteration (two 128-row GEMM tiles); one shared-memory area serves as first and second A operand in turn.
 #include "tina_common.cuh"
 #include "tina_ptx.cuh"
 
@@ -250,7 +250,8 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
             }
         }
         tc_fence_before();
-        __syncthreads();                                                 // TMEM and the A area are rewritten by the next group
+        // no barrier here: the next group's subfilter stage only writes the A area (its MMAs have retired), and the next
+        // MMA into these TMEM columns is issued behind the barrier that ends that stage
     }
     tc_fence_before();
     __syncthreads();
