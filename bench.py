@@ -57,6 +57,9 @@ def workload_spec(name: str):
         return dict(call="pfb", P=16, M=4, S=1, F=4096, real=False, prec=0)
     if name == "c4fir":   # subfilter stage only (Fig. 3 left column), config-4 shape
         return dict(call="pfb_fir", P=1024, M=16, S=8, F=8192, real=False, prec=0)
+    if name == "c4fft":   # config-4 shape through the factorised (32 x 32 Cooley-Tukey) Fourier stage: same result,
+        # HBM / FMA bound instead of tensor bound; reported separately from the dense-contraction headline
+        return dict(call="pfb_fft", P=1024, M=16, S=8, F=8192, real=False, prec=0)
     if name == "c2":
         return dict(call="dft", B=65536, N=256)
     if name == "c3":
@@ -71,6 +74,9 @@ def useful_flops_and_bytes(w):
         P, M, S, F = w["P"], w["M"], w["S"], w["F"]
         esz = 4 if w["real"] else 8
         return S * F * P * (esz // 4) * 2.0 * M, float(S * (F + M - 1) * P * esz + S * F * P * esz + P * M * 4), S * (F + M - 1) * P, S * F
+    if w["call"] == "pfb_fft":
+        P, M, S, F = w["P"], w["M"], w["S"], w["F"]
+        return S * F * 8.0 * P * 64, float(S * (F + M - 1) * P * 8 + S * F * P * 8 + P * M * 4), S * (F + M - 1) * P, S * F
     if w["call"] == "pfb":
         P, M, S, F = w["P"], w["M"], w["S"], w["F"]
         frames = S * F
@@ -136,7 +142,7 @@ class ClockSampler:
 
 def make_inputs(w, seed_offset: int = 0):
     """Seeded synthetic host arrays for the workload (tina_inputs recipes)."""
-    if w["call"] in ("pfb", "pfb_fir"):
+    if w["call"] in ("pfb", "pfb_fir", "pfb_fft"):
         if (w["P"], w["M"], w["real"]) == (1024, 16, False):
             case = ti.pfb_case(1024, 16, w["F"], streams=w["S"], seed=ti.SEED_BASE + 4 + 100 * seed_offset,
                                tones=3, name="c4")
@@ -156,7 +162,7 @@ def cpu_oracle_rate(w, budget_s: float = 15.0):
     import oracle
     oracle.build()
     cores = oracle.num_threads()
-    if w["call"] in ("pfb", "pfb_fir"):
+    if w["call"] in ("pfb", "pfb_fir", "pfb_fft"):
         P, M = w["P"], w["M"]
         probe = max(cores, 8)
         case = ti.pfb_case(P, M, probe, real=w["real"], seed=1)
@@ -233,6 +239,10 @@ def run_ours(args, w):
         NK = w["P"] // 2 + 1 if w["real"] else w["P"]
         out = torch.empty((w["S"], w["F"], NK), dtype=torch.complex64, device="cuda")
         step = lambda: tina.pfb(xd, w["P"], w["M"], wd, prec=w["prec"], out=out)
+    elif w["call"] == "pfb_fft":
+        xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()
+        out = torch.empty((w["S"], w["F"], w["P"]), dtype=torch.complex64, device="cuda")
+        step = lambda: tina.pfb_fft(xd, w["P"], w["M"], wd, out=out)
     elif w["call"] == "pfb_fir":
         xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()
         out = torch.empty((w["S"], w["F"], w["P"]), dtype=xd.dtype, device="cuda")
@@ -332,7 +342,7 @@ def run_ours(args, w):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": ("bf16x3->f32" if w.get("prec", 0) == 0 else ("bf16" if w.get("prec", 0) == 1 else "f16")) if tensor_bound else "f32",
+        "dtype": ("bf16x3->f32" if w.get("prec", 0) == 0 else ("bf16" if w.get("prec", 0) == 1 else "f16")) if (tensor_bound or w["call"] == "pfb_fft") else "f32",
         "data": "synthetic", "spectra_per_s": world * frames / (ms_per_step * 1e-3),
         "config": {"workload": args.workload, **{k: v for k, v in w.items() if k != "call"},
                    "l2": "inputs and outputs each exceed the 126 MB L2; no explicit flush",
