@@ -60,6 +60,8 @@ def workload_spec(name: str):
     if name == "c4fft":   # config-4 shape through the factorised (32 x 32 Cooley-Tukey) Fourier stage: same result,
         # HBM / FMA bound instead of tensor bound; reported separately from the dense-contraction headline
         return dict(call="pfb_fft", P=1024, M=16, S=8, F=8192, real=False, prec=0)
+    if name == "c5fft":   # config 5 (real, P = 4096 = 64 x 64) through the factorised Fourier stage
+        return dict(call="pfb_fft", P=4096, M=8, S=1, F=32761, real=True, prec=0)
     if name == "c2":
         return dict(call="dft", B=65536, N=256)
     if name == "c3":
@@ -76,6 +78,8 @@ def useful_flops_and_bytes(w):
         return S * F * P * (esz // 4) * 2.0 * M, float(S * (F + M - 1) * P * esz + S * F * P * esz + P * M * 4), S * (F + M - 1) * P, S * F
     if w["call"] == "pfb_fft":
         P, M, S, F = w["P"], w["M"], w["S"], w["F"]
+        if w["real"]:    # stage 1: 2 P sqrt(P) real MACs, stage 2: 2 x 2 x (P / 2) sqrt(P)
+            return S * F * 8.0 * P * 64, float(S * (F + M - 1) * P * 4 + S * F * (P // 2 + 1) * 8 + P * M * 4), S * (F + M - 1) * P, S * F
         return S * F * 8.0 * P * 64, float(S * (F + M - 1) * P * 8 + S * F * P * 8 + P * M * 4), S * (F + M - 1) * P, S * F
     if w["call"] == "pfb":
         P, M, S, F = w["P"], w["M"], w["S"], w["F"]
@@ -241,7 +245,7 @@ def run_ours(args, w):
         step = lambda: tina.pfb(xd, w["P"], w["M"], wd, prec=w["prec"], out=out)
     elif w["call"] == "pfb_fft":
         xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()
-        out = torch.empty((w["S"], w["F"], w["P"]), dtype=torch.complex64, device="cuda")
+        out = torch.empty((w["S"], w["F"], w["P"] // 2 + 1 if w["real"] else w["P"]), dtype=torch.complex64, device="cuda")
         step = lambda: tina.pfb_fft(xd, w["P"], w["M"], wd, out=out)
     elif w["call"] == "pfb_fir":
         xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()

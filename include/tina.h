@@ -100,11 +100,11 @@ tina_status tina_pfb_batched(const void* x, int S, long long n_samples, int P, i
 
 /* PFB with a FACTORISED Fourier stage ("either a Discrete or Fast Fourier Transform"):
  * same arguments and the same result as tina_pfb_batched (fp32-accurate, rel. L2 per frame <= 1e-5),
- * but the P-point DFT is computed as two stages of 32-point DFTs (P = 32 x 32, both stages tensor-core
- * contractions against the 32-point Fourier matrix, twiddle multiply in between, all on chip): 8 P (32+32)
- * instead of 8 P^2 flops per frame, i.e. HBM / FMA bound instead of tensor bound.  Reported separately
- * from the dense contraction that tina_pfb implements.  Supported in this version: kind = COMPLEX,
- * P = 1024, M <= 16; anything else -> UNSUPPORTED.                                                    */
+ * but the P-point DFT is computed as two stages of sqrt(P)-point DFTs (both stages tensor-core contractions
+ * against one small Fourier matrix, twiddle multiply in between, all on chip): 16 P sqrt(P) instead of 8 P^2
+ * flops per complex frame, i.e. HBM / FMA bound instead of tensor bound.  Reported separately from the dense
+ * contraction that tina_pfb implements.  Supported in this version: kind = COMPLEX with P = 1024 (32 x 32),
+ * M <= 16, and kind = REAL with P = 4096 (64 x 64; BASELINE config 5), M <= 8; anything else -> UNSUPPORTED. */
 tina_status tina_pfb_fft_batched(const void* x, int S, long long n_samples, int P, int M,
                                  const float* window, tina_kind kind, void* out, void* stream);
 

@@ -134,9 +134,9 @@ tina_status tina_pfb_fft_batched(const void* x, int S, long long n_samples, int 
     long long F;
     tina_status st = pfb_validate(x, S, n_samples, P, M, window, kind, out, "tina_pfb_fft", &F);
     if (st != TINA_OK) return st;
-    if (kind != TINA_COMPLEX || P != 1024 || M > 16)
-        return fail(TINA_ERR_UNSUPPORTED, "tina_pfb_fft: this version covers the complex kind with P = 1024, M <= 16");
-    return ct_pfb(x, S, n_samples, M, window, out, (cudaStream_t)stream);
+    if (kind == TINA_COMPLEX && P == 1024 && M <= 16) return ct_pfb(x, S, n_samples, M, window, out, (cudaStream_t)stream);
+    if (kind == TINA_REAL && P == 4096 && M <= 8) return ctr_pfb(x, S, n_samples, M, window, out, (cudaStream_t)stream);
+    return fail(TINA_ERR_UNSUPPORTED, "tina_pfb_fft: this version covers COMPLEX P = 1024 M <= 16 and REAL P = 4096 M <= 8");
 }
 
 tina_status tina_pfb_fir_batched(const void* x, int S, long long n_samples, int P, int M,

@@ -1,0 +1,323 @@
+// tina_ctr.cu -- PFB with a FACTORISED Fourier stage for the REAL kind at P = 4096 = 64 x 64 (BASELINE config 5;
+// SURVEY.md section 8(f) rank 2, "either a Discrete or Fast Fourier Transform").
+//
+// With p = a + 64 b and k = kb + 64 ka, for real y:
+//     G[f][a][kb]  = sum_b y[f][a + 64 b] W64^(b kb)                        (64-point DFTs of real data, stage 1)
+//     G'[f][a][kb] = G[f][a][kb] * W4096^(a kb)                             (twiddle)
+//     X[f][kb + 64 ka] = sum_a G'[f][a][kb] W64^(a ka),  k = 0 .. 2048      (stage 2; ka = 0 .. 31, plus k = 2048)
+// Both stages contract against ONE 128 x 64 matrix B1[(kb, c)][b] = (cos, -sin)(2 pi b kb / 64) held in shared memory
+// (bf16 hi | lo, bf16x3 products, fp32 accumulation in TMEM):
+//   stage 1 is computed TRANSPOSED, D1^T[(kb, c)][(frame, a)] = B1 * A1^T, so that an epilogue thread (one TMEM lane =
+//     one (kb, re | im)) sees consecutive a in consecutive columns: after one shuffle with its partner lane it owns the
+//     real OR the imaginary part of G' for 64 consecutive a, which it packs eight to a 16-byte store into the stage-2
+//     operand (rows (frame, kb), K = a), real parts and imaginary parts in two separate tiles;
+//   stage 2 runs the two tiles against the first 64 rows of B1 (ka = 0 .. 31):  D_R = Re(G') B1^T = (C_r, -S_r),
+//     D_I = Im(G') B1^T = (C_i, -S_i), and X = (D_R.re - D_I.im, D_R.im + D_I.re);
+//   X[2048] = sum_a (-1)^a G[a][0] is a thread-local alternating sum in the first epilogue.
+// One CTA per SM (193 KB of shared memory), 512 threads, 4 frames (two 128-row tiles) per iteration; the window taps
+// live in the upper 256 TMEM columns (tcgen05.st once, tcgen05.ld per column), so they cost no L1 / L2 traffic.
+#include "tina_common.cuh"
+#include "tina_ptx.cuh"
+
+#include <cuda_bf16.h>
+#include <cstdlib>
+
+namespace tina {
+
+using namespace ptx;
+
+constexpr int CR_P = 4096, CR_NK = CR_P / 2 + 1;
+constexpr int CR_FR = 4;                              // frames per group: 2 tiles x 2 frames x 64 rows
+constexpr int CR_THREADS = 512;
+constexpr int CR_BPW = 4;                             // b values per warp in the subfilter stage (16 warps x 4 = 64)
+constexpr int CR_TILE = 128 * 64 * 2;                 // one bf16 128 x 64 tile: 16 KB
+constexpr int CR_TWP = 66;                            // twiddle table row pitch in float2 (64 + 2: conflict-free 16-byte reads)
+
+struct CrSmem {
+    // [tile][block: real | imaginary parts of G'][hi | lo].  The stage-1 operand of tile t (rows (frame, a), K = b)
+    // occupies a[t][0] until its MMAs have retired; epilogue 1 then overwrites it.
+    uint8_t a[2][2][2][CR_TILE];
+    uint8_t bm[2][CR_TILE];                           // B1 hi | lo: row n = 2 kb + c, K = b, K-major SWIZZLE_128B
+    float2 tw[64 * CR_TWP];                           // W4096^(a kb), [kb][a]
+    uint64_t bar[2];
+    uint32_t tmem_base;
+};
+static_assert(sizeof(CrSmem) + 1024 <= 227 * 1024, "shared memory budget");
+
+__device__ __forceinline__ uint32_t cr_sw128(uint32_t row, uint32_t kbyte)    // byte offset in a K-major SW128 tile
+{
+    return row * 128u + ((((kbyte >> 4) ^ (row & 7u)) << 4) | (kbyte & 15u));
+}
+
+// packed fp32 pair d = a * b + c (fma.rn.f32x2)
+__device__ __forceinline__ float2 cr_ffma2(float2 a, float2 b, float2 c)
+{
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return d;
+}
+
+// (vx, vy) -> packed bf16 pairs: hi = round(v), lo = round(v - hi); vx in the low half
+__device__ __forceinline__ void cr_split(float vx, float vy, uint32_t& hb, uint32_t& lb)
+{
+    const __nv_bfloat162 hi = __floats2bfloat162_rn(vx, vy);
+    hb = *reinterpret_cast<const uint32_t*>(&hi);
+    const __nv_bfloat162 lo = __floats2bfloat162_rn(vx - __uint_as_float(hb << 16), vy - __uint_as_float(hb & 0xffff0000u));
+    lb = *reinterpret_cast<const uint32_t*>(&lo);
+}
+
+__device__ __forceinline__ float cr_ldg(const float* p)
+{
+    float v;
+    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+
+template <int MT>
+__global__ void __launch_bounds__(CR_THREADS, 1)
+pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float* __restrict__ window,
+               float2* __restrict__ out, long long F, long long NBLK, int M, int groups_per_stream, int total_groups)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    CrSmem& sm = *reinterpret_cast<CrSmem*>(smem_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    // ---- one-time setup: B1, twiddle table, barriers, TMEM, taps
+    for (int e = tid; e < 128 * 64; e += CR_THREADS) {
+        const int n = e >> 6, b = e & 63, kb = n >> 1;
+        float sn, cs;
+        sincospif((float)((b * kb) & 63) * (1.0f / 32.0f), &sn, &cs);
+        const float v = (n & 1) ? -sn : cs;
+        const __nv_bfloat16 hi = __float2bfloat16_rn(v);
+        *reinterpret_cast<__nv_bfloat16*>(sm.bm[0] + cr_sw128(n, b * 2)) = hi;
+        *reinterpret_cast<__nv_bfloat16*>(sm.bm[1] + cr_sw128(n, b * 2)) = __float2bfloat16_rn(v - __bfloat162float(hi));
+    }
+    for (int e = tid; e < 64 * 64; e += CR_THREADS) {
+        const int kb = e >> 6, a = e & 63;
+        double sn, cs;
+        sincospi((double)(a * kb) / 2048.0, &sn, &cs);
+        sm.tw[kb * CR_TWP + a] = make_float2((float)cs, (float)-sn);
+    }
+    if (tid == 0) { mbar_init(smem_u32(&sm.bar[0]), 1); mbar_init(smem_u32(&sm.bar[1]), 1); fence_mbar_init(); }
+    if (warp == 0) { tmem_alloc<1>(smem_u32(&sm.tmem_base), 512); tmem_relinquish<1>(); }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+    // taps of this thread's columns p = lane (+ 32) + 64 (4 warp + bi): TMEM columns 256 .. 511, its own lane of its
+    // warp's lane quarter, 16 columns per bi holding (tap m of a, tap m of a + 32) pairs, zero beyond M
+    const uint32_t tap_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + 256 + (warp >> 2) * 64;
+#pragma unroll 1
+    for (int bi = 0; bi < CR_BPW; ++bi) {
+        uint32_t tv[16];
+        const float* wp = window + lane + 64 * (CR_BPW * warp + bi);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            tv[2 * m] = m < M ? __float_as_uint(__ldg(wp + (long long)m * CR_P)) : 0u;
+            tv[2 * m + 1] = m < M ? __float_as_uint(__ldg(wp + (long long)m * CR_P + 32)) : 0u;
+        }
+        tmem_st16(tap_addr + bi * 16, tv);
+    }
+    tmem_st_wait();
+
+    const uint32_t idesc1 = idesc_bf16(128, 128), idesc2 = idesc_bf16(128, 64);
+    const uint64_t d_bh = smem_desc_sw128(smem_u32(sm.bm[0])), d_bl = smem_desc_sw128(smem_u32(sm.bm[1]));
+    const uint64_t d_a = smem_desc_sw128(smem_u32(&sm.a[0][0][0][0]));
+    constexpr uint64_t PART = (uint64_t)CR_TILE >> 4, BLOCK = 2 * PART, TILE = 2 * BLOCK;   // descriptor steps
+
+    constexpr int WA = MT, NR = WA - 1 + CR_FR;
+    // subfilter-stage store offset: row a = lane (second row + 32), K bytes 8 warp .. 8 warp + 7 (b = 4 warp .. + 3)
+    const uint32_t fir_off = lane * 128 + ((((uint32_t)warp >> 1) ^ (lane & 7)) << 4) + 8 * (warp & 1);
+    // epilogue roles: TMEM lane quarter, tile, column half
+    const int eq = warp & 3, et = (warp >> 2) & 1, eh = warp >> 3;
+    uint32_t it = 0;
+    for (int g = blockIdx.x; g < total_groups; g += gridDim.x, ++it) {
+        const int s = g / groups_per_stream;
+        const long long f0 = (long long)(g % groups_per_stream) * CR_FR;
+        // ---- subfilter stage, Eq. (20): thread (warp w, lane l) owns rows a = l, l + 32 of columns b = 4 w .. 4 w + 3
+        {
+            const long long r0 = f0 + M - WA;
+            const bool interior = r0 >= 0 && r0 + NR <= NBLK;              // uniform
+            const float* xg = x + (long long)s * stream_stride + r0 * CR_P + lane + 64 * (CR_BPW * warp);
+            uint32_t hA[CR_FR][2], lA[CR_FR][2], hB[CR_FR][2], lB[CR_FR][2];   // packed K cells of rows a, a + 32
+            uint32_t hprev[CR_FR], lprev[CR_FR];
+#pragma unroll
+            for (int bi = 0; bi < CR_BPW; ++bi) {
+                uint32_t tv[16];
+                float2 row[NR];
+                tmem_ld16(tap_addr + bi * 16, tv);
+                if (interior) {
+#pragma unroll
+                    for (int j = 0; j < NR; ++j)
+                        row[j] = make_float2(cr_ldg(xg + bi * 64 + j * CR_P), cr_ldg(xg + bi * 64 + j * CR_P + 32));
+                } else {
+#pragma unroll
+                    for (int j = 0; j < NR; ++j) {
+                        const long long r = r0 + j;
+                        row[j] = (r >= 0 && r < NBLK) ? make_float2(cr_ldg(xg + bi * 64 + j * CR_P), cr_ldg(xg + bi * 64 + j * CR_P + 32))
+                                                      : make_float2(0.f, 0.f);
+                    }
+                }
+                tmem_ld_wait();
+#pragma unroll
+                for (int fl = 0; fl < CR_FR; ++fl) {
+                    float2 y = make_float2(__uint_as_float(tv[0]) * row[fl + WA - 1].x, __uint_as_float(tv[1]) * row[fl + WA - 1].y);
+#pragma unroll
+                    for (int m = 1; m < WA; ++m)
+                        y = cr_ffma2(make_float2(__uint_as_float(tv[2 * m]), __uint_as_float(tv[2 * m + 1])), row[fl + WA - 1 - m], y);
+                    uint32_t hb, lb;                                       // low half: row a, high half: row a + 32
+                    cr_split(y.x, y.y, hb, lb);
+                    if (bi & 1) {
+                        hA[fl][bi >> 1] = __byte_perm(hprev[fl], hb, 0x5410);
+                        hB[fl][bi >> 1] = __byte_perm(hprev[fl], hb, 0x7632);
+                        lA[fl][bi >> 1] = __byte_perm(lprev[fl], lb, 0x5410);
+                        lB[fl][bi >> 1] = __byte_perm(lprev[fl], lb, 0x7632);
+                    } else {
+                        hprev[fl] = hb;
+                        lprev[fl] = lb;
+                    }
+                }
+            }
+#pragma unroll
+            for (int fl = 0; fl < CR_FR; ++fl) {
+                uint8_t* const dst = &sm.a[fl >> 1][0][0][0] + (fl & 1) * 64 * 128 + fir_off;
+                *reinterpret_cast<uint2*>(dst) = make_uint2(hA[fl][0], hA[fl][1]);
+                *reinterpret_cast<uint2*>(dst + CR_TILE) = make_uint2(lA[fl][0], lA[fl][1]);
+                *reinterpret_cast<uint2*>(dst + 32 * 128) = make_uint2(hB[fl][0], hB[fl][1]);
+                *reinterpret_cast<uint2*>(dst + 32 * 128 + CR_TILE) = make_uint2(lB[fl][0], lB[fl][1]);
+            }
+        }
+        fence_proxy_async();
+        __syncthreads();
+        // ---- stage 1 (transposed): D1^T[t] = B1 * A1[t]^T -> TMEM columns 128 t .. 128 t + 127 = (frame, a)
+        if (tid == 0) {
+            tc_fence_after();
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 128 * t, d_bh + 2 * k, d_a + t * TILE + PART + 2 * k, idesc1, k > 0);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 128 * t, d_bl + 2 * k, d_a + t * TILE + 2 * k, idesc1, 1);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 128 * t, d_bh + 2 * k, d_a + t * TILE + 2 * k, idesc1, 1);
+            }
+            umma_commit(smem_u32(&sm.bar[0]));
+        }
+        mbar_wait(smem_u32(&sm.bar[0]), it & 1u);
+        tc_fence_after();
+        // ---- epilogue 1: warp (eq, et, eh) reads TMEM lanes 32 eq .. + 31 = (kb = 16 eq + lane / 2, c = lane & 1) and the
+        //      64 columns a = 0 .. 63 of frame 2 et + eh; the partner lane (lane ^ 1) holds the other part of G[a][kb].
+        //      G' = G * w:  Re = Gr wr - Gi wi,  Im = Gi wr + Gr wi  ->  own * wr + partner * (c ? wi : -wi).
+        {
+            const int kb = 16 * eq + (lane >> 1), c = lane & 1;
+            const float sgn = c ? 1.f : -1.f;
+            const long long f = f0 + 2 * et + eh;
+            const uint32_t row = eh * 64 + kb;
+            uint8_t* const blk = &sm.a[et][c][0][0];
+            const float4* twr = reinterpret_cast<const float4*>(sm.tw + kb * CR_TWP);
+            float nyq = 0.f;
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 * eh + 32 * hh, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int j8 = 0; j8 < 4; ++j8) {
+                    uint32_t hw[4], lw[4];
+#pragma unroll
+                    for (int i2 = 0; i2 < 4; ++i2) {
+                        const int i = 8 * j8 + 2 * i2;                     // a = 32 hh + i, i + 1
+                        const float4 w = twr[(32 * hh + i) >> 1];
+                        const float v0 = __uint_as_float(v[i]), v1 = __uint_as_float(v[i + 1]);
+                        const float p0 = __shfl_xor_sync(0xffffffffu, v0, 1), p1 = __shfl_xor_sync(0xffffffffu, v1, 1);
+                        nyq += v0 - v1;
+                        const float o0 = fmaf(p0, sgn * w.y, v0 * w.x), o1 = fmaf(p1, sgn * w.w, v1 * w.z);
+                        cr_split(o0, o1, hw[i2], lw[i2]);
+                    }
+                    const uint32_t off = cr_sw128(row, 64 * hh + 16 * j8);
+                    *reinterpret_cast<uint4*>(blk + off) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+                    *reinterpret_cast<uint4*>(blk + CR_TILE + off) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+                }
+            }
+            // k = 2048: X = sum_a (-1)^a G[a][0] (real; the lane holding (kb = 0, re) has all 64 terms)
+            if (eq == 0 && lane == 0 && f < F) out[((long long)s * F + f) * CR_NK + CR_P / 2] = make_float2(nyq, 0.f);
+        }
+        fence_proxy_async();
+        tc_fence_before();
+        __syncthreads();
+        // ---- stage 2: D_R[t] = Re(G')[t] * B1[0..63]^T -> columns 128 t .. + 63,  D_I[t] = Im(G')[t] * B1[0..63]^T -> + 64 .. + 127
+        if (tid == 0) {
+            tc_fence_after();
+#pragma unroll
+            for (int t = 0; t < 2; ++t)
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const uint64_t da = d_a + t * TILE + c * BLOCK;
+                    const uint32_t dcol = tmem + 128 * t + 64 * c;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + PART + 2 * k, d_bh + 2 * k, idesc2, k > 0);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bh + 2 * k, idesc2, 1);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bl + 2 * k, idesc2, 1);
+                }
+            umma_commit(smem_u32(&sm.bar[1]));
+        }
+        mbar_wait(smem_u32(&sm.bar[1]), it & 1u);
+        tc_fence_after();
+        // ---- epilogue 2: warp (eq, et, eh) reads rows 32 eq .. + 31 = (frame 2 et + eq / 2, kb = 32 (eq & 1) + lane) and
+        //      ka = 16 eh .. 16 eh + 15.  D_R = (C_r, -S_r), D_I = (C_i, -S_i):  X = (C_r + S_i, C_i - S_r).
+        //      For a fixed ka the 32 lanes hold 32 consecutive channels: 256 contiguous bytes per warp store.
+        {
+            const long long f = f0 + 2 * et + (eq >> 1);
+            float2* const orow = out + ((long long)s * F + f) * CR_NK + 32 * (eq & 1) + lane + 64 * 16 * eh;
+            uint32_t vr[32], vi[32];
+            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 32 * eh, vr);
+            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 + 32 * eh, vi);
+            tmem_ld_wait();
+            if (f < F) {
+#pragma unroll
+                for (int i = 0; i < 16; ++i)
+                    orow[64 * i] = make_float2(__uint_as_float(vr[2 * i]) - __uint_as_float(vi[2 * i + 1]),
+                                               __uint_as_float(vr[2 * i + 1]) + __uint_as_float(vi[2 * i]));
+            }
+        }
+        tc_fence_before();
+        // no barrier here: the next subfilter stage only writes shared memory whose MMAs have retired, and the next MMA
+        // into these TMEM columns is issued behind the barrier that ends that stage
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<1>(tmem, 512);
+}
+
+tina_status ctr_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st)
+{
+    const long long NBLK = n_samples / CR_P, F = NBLK - M + 1;
+    const long long gps = (F + CR_FR - 1) / CR_FR;
+    if (gps * S > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb_fft: too many frames");
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaError_t e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctr_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CrSmem) + 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctr_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CrSmem) + 1024);
+        if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "pfb_ctr_kernel setup"); }
+    }
+    const int total = (int)(gps * S);
+    const int grid = total < n_sm ? total : n_sm;           // 512 threads, 193 KB shared memory, all 512 TMEM columns
+    const size_t smem = sizeof(CrSmem) + 1024;
+    const float* xf = static_cast<const float*>(x);
+    float2* of = static_cast<float2*>(out);
+    if (M <= 4) pfb_ctr_kernel<4><<<grid, CR_THREADS, smem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
+    else pfb_ctr_kernel<8><<<grid, CR_THREADS, smem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
+    count_launch();
+    g_last_path = kPathUmma;
+    return check_cuda(cudaGetLastError(), "pfb_ctr_kernel launch");
+}
+
+}  // namespace tina

@@ -332,6 +332,52 @@ def test_pfb_fft_factorised_stage(tina, oracle, M, F, S):
     assert e.value.status == 3
 
 
+@pytest.mark.parametrize("M,F,S", [(8, 130, 1), (4, 7, 2), (6, 33, 1), (1, 16, 1), (8, 1, 1), (8, 4, 3)])
+def test_pfb_fft_factorised_stage_real(tina, oracle, M, F, S):
+    """Real kind, P = 4096 = 64 x 64 (the config-5 shape): factorised Fourier stage against the oracle's direct DFT;
+    ragged groups of 4 frames, M below the unrolled tap count, several streams; Im X[0] = Im X[P/2] = 0."""
+    rng = np.random.default_rng(60 + M)
+    case = ti.pfb_case(4096, M, F, real=True, streams=S, seed=61 + M + F, window=ti.random_taps(rng, 4096 * M))
+    import torch
+    out = tina.pfb_fft(_cuda(case.x), 4096, M, _cuda(case.window)); torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert got.shape == (S, F, 2049)
+    for s in range(S):
+        ref = oracle.pfb(case.x[s], 4096, M, case.window)
+        assert rel_l2_rows(got[s], ref) <= TOL_FP32
+        assert np.abs(got[s][:, 2048] - ref[:, 2048]).max() <= 1e-5 * np.linalg.norm(ref, axis=1).max()
+    assert np.all(got[..., 2048].imag == 0)
+    with pytest.raises(tina.TinaError) as e:                 # M > 8 is not covered by the real-kind factorised kernel
+        tina.pfb_fft(_cuda(np.zeros((1, 4096 * 12), np.float32)), 4096, 9, _cuda(np.ones(4096 * 9, np.float32)))
+    assert e.value.status == 3
+
+
+def test_config5_full_size_factorised_sampled(tina, oracle):
+    """c5 at full size through tina_pfb_fft_batched: first / last / seeded frames against the oracle."""
+    import torch
+    case = ti.config5()
+    out = tina.pfb_fft(_cuda(case.x), 4096, 8, _cuda(case.window)); torch.cuda.synchronize()
+    got = out.cpu().numpy()[0]
+    assert got.shape == (32761, 2049)
+    fr = ti.sample_frames(32761, 64, ti.SEED_BASE + 51)
+    ref = oracle.pfb(case.x[0], 4096, 8, case.window, frames=fr)
+    assert rel_l2_rows(got[fr], ref) <= TOL_FP32
+    assert np.all(got[:, 2048].imag == 0)
+
+
+def test_config4_full_size_factorised_sampled(tina, oracle):
+    """c4 at full size through tina_pfb_fft_batched: seeded frames of every stream against the oracle."""
+    import torch
+    case = ti.config4()
+    out = tina.pfb_fft(_cuda(case.x), 1024, 16, _cuda(case.window)); torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert got.shape == (8, 8192, 1024)
+    for s in (0, 3, 7):
+        fr = ti.sample_frames(8192, 24, ti.SEED_BASE + 60 + s)
+        ref = oracle.pfb(case.x[s], 1024, 16, case.window, frames=fr)
+        assert rel_l2_rows(got[s][fr], ref) <= TOL_FP32
+
+
 def test_pfb_fir_only(tina, oracle):
     import torch
     for real in (False, True):
