@@ -182,7 +182,7 @@ def pfb(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=None)
 
 
 def pfb_fft(x, P: int, M: int, window, out=None, stream=None):
-    """tina_pfb_fft_batched: PFB with the factorised (32 x 32) Fourier stage; same result as pfb()."""
+    """tina_pfb_fft_batched: PFB with the factorised Fourier stage (complex P=1024 or real P=4096); same result as pfb()."""
     import torch
     squeeze = x.dim() == 1
     x, kind, S, n, F = _pfb_args(x, P, M, window)

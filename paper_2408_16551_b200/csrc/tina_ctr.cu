@@ -68,10 +68,10 @@ __device__ __forceinline__ void cr_split(float vx, float vy, uint32_t& hb, uint3
     lb = *reinterpret_cast<const uint32_t*>(&lo);
 }
 
-__device__ __forceinline__ float cr_ldg(const float* p)
+__device__ __forceinline__ float2 cr_ldg2(const float* p)
 {
-    float v;
-    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
     return v;
 }
 
@@ -107,17 +107,17 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
-    // taps of this thread's columns p = lane (+ 32) + 64 (4 warp + bi): TMEM columns 256 .. 511, its own lane of its
-    // warp's lane quarter, 16 columns per bi holding (tap m of a, tap m of a + 32) pairs, zero beyond M
+    // taps of this thread's columns p = 2 lane (+ 1) + 64 (4 warp + bi): TMEM columns 256 .. 511, its own lane of its
+    // warp's lane quarter, 16 columns per bi holding (tap m of a, tap m of a + 1) pairs, zero beyond M
     const uint32_t tap_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + 256 + (warp >> 2) * 64;
 #pragma unroll 1
     for (int bi = 0; bi < CR_BPW; ++bi) {
         uint32_t tv[16];
-        const float* wp = window + lane + 64 * (CR_BPW * warp + bi);
+        const float* wp = window + 2 * lane + 64 * (CR_BPW * warp + bi);
 #pragma unroll
         for (int m = 0; m < 8; ++m) {
             tv[2 * m] = m < M ? __float_as_uint(__ldg(wp + (long long)m * CR_P)) : 0u;
-            tv[2 * m + 1] = m < M ? __float_as_uint(__ldg(wp + (long long)m * CR_P + 32)) : 0u;
+            tv[2 * m + 1] = m < M ? __float_as_uint(__ldg(wp + (long long)m * CR_P + 1)) : 0u;
         }
         tmem_st16(tap_addr + bi * 16, tv);
     }
@@ -129,38 +129,47 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
     constexpr uint64_t PART = (uint64_t)CR_TILE >> 4, BLOCK = 2 * PART, TILE = 2 * BLOCK;   // descriptor steps
 
     constexpr int WA = MT, NR = WA - 1 + CR_FR;
-    // subfilter-stage store offset: row a = lane (second row + 32), K bytes 8 warp .. 8 warp + 7 (b = 4 warp .. + 3)
+    // subfilter-stage store offset.  A thread owns a = 2 lane and 2 lane + 1 (one 8-byte load); within a frame's 64 tile
+    // rows a sits at row rho(a) = a / 2 + 32 (a & 1), so the two rows are lane and lane + 32 (2-way instead of 4-way
+    // bank conflicts); epilogue 1 undoes the permutation for free when it picks TMEM columns.  K bytes 8 warp .. + 7.
     const uint32_t fir_off = lane * 128 + ((((uint32_t)warp >> 1) ^ (lane & 7)) << 4) + 8 * (warp & 1);
     // epilogue roles: TMEM lane quarter, tile, column half
     const int eq = warp & 3, et = (warp >> 2) & 1, eh = warp >> 3;
+    // the NR = WA - 1 + CR_FR samples of input columns (2 lane, 2 lane + 1) + 64 (4 warp + bi) that group gg needs; rows
+    // outside the stream read as zero (the first groups when M < WA and the last group of a stream take that path)
+    auto load_col = [&](int gg, int bi, float2 (&row)[NR]) {
+        const long long r0 = (long long)(gg % groups_per_stream) * CR_FR + M - WA;
+        const float* xg = x + (long long)(gg / groups_per_stream) * stream_stride + r0 * CR_P + 2 * lane + 64 * (CR_BPW * warp + bi);
+        if (r0 >= 0 && r0 + NR <= NBLK) {                                  // uniform
+#pragma unroll
+            for (int j = 0; j < NR; ++j) row[j] = cr_ldg2(xg + j * CR_P);
+        } else {
+#pragma unroll
+            for (int j = 0; j < NR; ++j)
+                row[j] = (r0 + j >= 0 && r0 + j < NBLK) ? cr_ldg2(xg + j * CR_P) : make_float2(0.f, 0.f);
+        }
+    };
+    // Loads run one column ahead of the FMAs: column bi + 1 is requested before column bi is computed, and column 0 of
+    // the NEXT group right after this group's subfilter stage, so it is in flight during the MMA waits and epilogues.
+    float2 pre[NR];
+    if ((int)blockIdx.x < total_groups) load_col(blockIdx.x, 0, pre);
     uint32_t it = 0;
     for (int g = blockIdx.x; g < total_groups; g += gridDim.x, ++it) {
         const int s = g / groups_per_stream;
         const long long f0 = (long long)(g % groups_per_stream) * CR_FR;
-        // ---- subfilter stage, Eq. (20): thread (warp w, lane l) owns rows a = l, l + 32 of columns b = 4 w .. 4 w + 3
+        // ---- subfilter stage, Eq. (20): thread (warp w, lane l) owns a = 2 l, 2 l + 1 of columns b = 4 w .. 4 w + 3
         {
-            const long long r0 = f0 + M - WA;
-            const bool interior = r0 >= 0 && r0 + NR <= NBLK;              // uniform
-            const float* xg = x + (long long)s * stream_stride + r0 * CR_P + lane + 64 * (CR_BPW * warp);
-            uint32_t hA[CR_FR][2], lA[CR_FR][2], hB[CR_FR][2], lB[CR_FR][2];   // packed K cells of rows a, a + 32
+            uint32_t hA[CR_FR][2], lA[CR_FR][2], hB[CR_FR][2], lB[CR_FR][2];   // packed K cells of tile rows lane, lane + 32
             uint32_t hprev[CR_FR], lprev[CR_FR];
+            float2 rows[2][NR];
+#pragma unroll
+            for (int j = 0; j < NR; ++j) rows[0][j] = pre[j];
 #pragma unroll
             for (int bi = 0; bi < CR_BPW; ++bi) {
                 uint32_t tv[16];
-                float2 row[NR];
                 tmem_ld16(tap_addr + bi * 16, tv);
-                if (interior) {
-#pragma unroll
-                    for (int j = 0; j < NR; ++j)
-                        row[j] = make_float2(cr_ldg(xg + bi * 64 + j * CR_P), cr_ldg(xg + bi * 64 + j * CR_P + 32));
-                } else {
-#pragma unroll
-                    for (int j = 0; j < NR; ++j) {
-                        const long long r = r0 + j;
-                        row[j] = (r >= 0 && r < NBLK) ? make_float2(cr_ldg(xg + bi * 64 + j * CR_P), cr_ldg(xg + bi * 64 + j * CR_P + 32))
-                                                      : make_float2(0.f, 0.f);
-                    }
-                }
+                if (bi + 1 < CR_BPW) load_col(g, bi + 1, rows[(bi + 1) & 1]);
+                float2 (&row)[NR] = rows[bi & 1];
                 tmem_ld_wait();
 #pragma unroll
                 for (int fl = 0; fl < CR_FR; ++fl) {
@@ -168,7 +177,7 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
 #pragma unroll
                     for (int m = 1; m < WA; ++m)
                         y = cr_ffma2(make_float2(__uint_as_float(tv[2 * m]), __uint_as_float(tv[2 * m + 1])), row[fl + WA - 1 - m], y);
-                    uint32_t hb, lb;                                       // low half: row a, high half: row a + 32
+                    uint32_t hb, lb;                                       // low half: a = 2 l, high half: a = 2 l + 1
                     cr_split(y.x, y.y, hb, lb);
                     if (bi & 1) {
                         hA[fl][bi >> 1] = __byte_perm(hprev[fl], hb, 0x5410);
@@ -181,6 +190,7 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
                     }
                 }
             }
+            if (g + (int)gridDim.x < total_groups) load_col(g + (int)gridDim.x, 0, pre);
 #pragma unroll
             for (int fl = 0; fl < CR_FR; ++fl) {
                 uint8_t* const dst = &sm.a[fl >> 1][0][0][0] + (fl & 1) * 64 * 128 + fir_off;
@@ -218,29 +228,29 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
             const uint32_t row = eh * 64 + kb;
             uint8_t* const blk = &sm.a[et][c][0][0];
             const float4* twr = reinterpret_cast<const float4*>(sm.tw + kb * CR_TWP);
+            // TMEM column rho of this frame holds a = 2 rho (rho < 32) or 2 (rho - 32) + 1: even a in ve, odd a in vo
+            // TMEM column rho of this frame holds a = 2 rho (rho < 32) or 2 (rho - 32) + 1: even a in ve, odd a in vo
+            uint32_t ve[32], vo[32];
+            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 * eh, ve);
+            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 * eh + 32, vo);
+            tmem_ld_wait();
             float nyq = 0.f;
 #pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-                uint32_t v[32];
-                tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 * eh + 32 * hh, v);
-                tmem_ld_wait();
+            for (int j8 = 0; j8 < 8; ++j8) {                               // a = 8 j8 .. 8 j8 + 7
+                uint32_t hw[4], lw[4];
 #pragma unroll
-                for (int j8 = 0; j8 < 4; ++j8) {
-                    uint32_t hw[4], lw[4];
-#pragma unroll
-                    for (int i2 = 0; i2 < 4; ++i2) {
-                        const int i = 8 * j8 + 2 * i2;                     // a = 32 hh + i, i + 1
-                        const float4 w = twr[(32 * hh + i) >> 1];
-                        const float v0 = __uint_as_float(v[i]), v1 = __uint_as_float(v[i + 1]);
-                        const float p0 = __shfl_xor_sync(0xffffffffu, v0, 1), p1 = __shfl_xor_sync(0xffffffffu, v1, 1);
-                        nyq += v0 - v1;
-                        const float o0 = fmaf(p0, sgn * w.y, v0 * w.x), o1 = fmaf(p1, sgn * w.w, v1 * w.z);
-                        cr_split(o0, o1, hw[i2], lw[i2]);
-                    }
-                    const uint32_t off = cr_sw128(row, 64 * hh + 16 * j8);
-                    *reinterpret_cast<uint4*>(blk + off) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
-                    *reinterpret_cast<uint4*>(blk + CR_TILE + off) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+                for (int i2 = 0; i2 < 4; ++i2) {
+                    const int i = 4 * j8 + i2;                             // a = 2 i, 2 i + 1
+                    const float4 w = twr[i];
+                    const float v0 = __uint_as_float(ve[i]), v1 = __uint_as_float(vo[i]);
+                    const float p0 = __shfl_xor_sync(0xffffffffu, v0, 1), p1 = __shfl_xor_sync(0xffffffffu, v1, 1);
+                    nyq += v0 - v1;
+                    const float o0 = fmaf(p0, sgn * w.y, v0 * w.x), o1 = fmaf(p1, sgn * w.w, v1 * w.z);
+                    cr_split(o0, o1, hw[i2], lw[i2]);
                 }
+                const uint32_t off = cr_sw128(row, 16 * j8);
+                *reinterpret_cast<uint4*>(blk + off) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+                *reinterpret_cast<uint4*>(blk + CR_TILE + off) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
             }
             // k = 2048: X = sum_a (-1)^a G[a][0] (real; the lane holding (kb = 0, re) has all 64 terms)
             if (eq == 0 && lane == 0 && f < F) out[((long long)s * F + f) * CR_NK + CR_P / 2] = make_float2(nyq, 0.f);
