@@ -58,6 +58,13 @@ def _load():
     lib.oracle_pfb.argtypes = [vp, ll, ll, ll, vp, ci, vp, ll, vp, vp]
     lib.oracle_pfb.restype = ci
     lib.oracle_num_threads.restype = ci
+    for name in ("oracle_mul", "oracle_add"):
+        getattr(lib, name).argtypes = [vp, vp, vp, ll]
+        getattr(lib, name).restype = ci
+    lib.oracle_sum.argtypes = [vp, vp, ll, ll]
+    lib.oracle_sum.restype = ci
+    lib.oracle_matmul.argtypes = [vp, vp, vp, ll, ll, ll]
+    lib.oracle_matmul.restype = ci
     lib.oracle_set_num_threads.argtypes = [ci]
     _lib = lib
     return lib
@@ -100,6 +107,57 @@ def unfold(x, J: int) -> np.ndarray:
     if rc:
         raise ValueError(f"oracle_unfold rc={rc}")
     return y
+
+
+def _binary(name, a, b):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    b = np.ascontiguousarray(b, dtype=np.float32)
+    if a.shape != b.shape:
+        raise ValueError("shape mismatch")
+    o = np.empty(a.shape, dtype=np.float64)
+    rc = getattr(_load(), name)(_ptr(a), _ptr(b), _ptr(o), a.size)
+    if rc:
+        raise ValueError(f"{name} rc={rc}")
+    return o
+
+
+def mul(a, b) -> np.ndarray:
+    """Eq. (6): elementwise product of two float32 arrays -> float64."""
+    return _binary("oracle_mul", a, b)
+
+
+def add(a, b) -> np.ndarray:
+    """Eq. (10): elementwise sum of two float32 arrays -> float64."""
+    return _binary("oracle_add", a, b)
+
+
+def summation(x) -> np.ndarray:
+    """Eq. (11): sum over the last axis.  x: [rows, n] (or [n]) float32 -> float64 [rows] (or scalar array)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    one_d = x.ndim == 1
+    if one_d:
+        x = x[None, :]
+    rows, n = x.shape
+    o = np.empty(rows, dtype=np.float64)
+    rc = _load().oracle_sum(_ptr(x), _ptr(o), rows, n)
+    if rc:
+        raise ValueError(f"oracle_sum rc={rc}")
+    return o[0] if one_d else o
+
+
+def matmul(x, y) -> np.ndarray:
+    """Eq. (7): Z = X Y.  x: [M, L], y: [L, N] float32 -> float64 [M, N]."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    y = np.ascontiguousarray(y, dtype=np.float32)
+    M, L = x.shape
+    L2, N = y.shape
+    if L != L2:
+        raise ValueError("inner dimensions differ")
+    z = np.empty((M, N), dtype=np.float64)
+    rc = _load().oracle_matmul(_ptr(x), _ptr(y), _ptr(z), M, L, N)
+    if rc:
+        raise ValueError(f"oracle_matmul rc={rc}")
+    return z
 
 
 def dft(x, inverse: bool = False) -> np.ndarray:

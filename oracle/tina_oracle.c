@@ -14,6 +14,8 @@
  *   oracle_pfb   Eq. (20), followed by the DFT of sec. 4.1
  *
  *   oracle_unfold Eq. (17), PAPER.md:187     Y(i,j) = X(i+j)
+ *   oracle_mul / oracle_add / oracle_sum / oracle_matmul   Eq. (6), (10), (11), (7): PAPER.md:96, :127,
+ *                :136, :104 -- the arithmetic building blocks of section 3
  *
  * Readings of the paper where it is silent (SURVEY.md
  * section 8(c) R1..R16): 0-based sums, valid mode, x_p(n') = x[n'P+p],
@@ -82,6 +84,54 @@ int oracle_unfold(const float *x, double *y, long long I, long long J)
     for (long long i = 0; i < I - J + 1; ++i)
         for (long long j = 0; j < J; ++j)
             y[i * J + j] = (double)x[i + j];
+    return 0;
+}
+
+/* Eq. (6): O(c) = I(c) K(c).                                     */
+int oracle_mul(const float *a, const float *b, double *o, long long n)
+{
+    if (!a || !b || !o || n < 0) return 1;
+    for (long long c = 0; c < n; ++c) o[c] = (double)a[c] * (double)b[c];
+    return 0;
+}
+
+/* Eq. (10): O(c) = b(c) + I(c).                                 */
+int oracle_add(const float *a, const float *b, double *o, long long n)
+{
+    if (!a || !b || !o || n < 0) return 1;
+    for (long long c = 0; c < n; ++c) o[c] = (double)b[c] + (double)a[c];
+    return 0;
+}
+
+/* Eq. (11): O = sum_c I(c), one sum per row of x[rows][n], in
+ * index order (double accumulation; compensated, so the order does not show). */
+int oracle_sum(const float *x, double *o, long long rows, long long n)
+{
+    if (!x || !o || rows < 0 || n < 0) return 1;
+    for (long long r = 0; r < rows; ++r) {
+        double acc = 0.0, comp = 0.0;                    /* Neumaier: exact to ~1 ulp of double */
+        for (long long c = 0; c < n; ++c) {
+            const double v = (double)x[r * n + c], t = acc + v;
+            comp += fabs(acc) >= fabs(v) ? (acc - t) + v : (v - t) + acc;
+            acc = t;
+        }
+        o[r] = acc + comp;
+    }
+    return 0;
+}
+
+/* Eq. (7): Z(m,n) = sum_l X(m,l) Y(l,n); X [M][L], Y [L][N],
+ * Z [M][N], row-major.                                                        */
+int oracle_matmul(const float *x, const float *y, double *z, long long M, long long L, long long N)
+{
+    if (!x || !y || !z || M < 0 || L < 0 || N < 0) return 1;
+#pragma omp parallel for schedule(static)
+    for (long long m = 0; m < M; ++m)
+        for (long long n = 0; n < N; ++n) {
+            double acc = 0.0;
+            for (long long l = 0; l < L; ++l) acc += (double)x[m * L + l] * (double)y[l * N + n];
+            z[m * N + n] = acc;
+        }
     return 0;
 }
 

@@ -253,3 +253,57 @@ def test_config4_tone_bins_dominate(oracle):
     sw = float(c.window.astype(np.float64).sum())
     for k in c.tone_bins[0]:
         assert abs(abs(X[2, k]) - 10 * sw) < 0.15 * 10 * sw
+
+
+# ---------------------------------------------------------------- section 3 arithmetic blocks
+def test_arith_mul_add_closed_forms(oracle):
+    """Eq. (6) / (10) on values whose products and sums are exact in binary: powers of two and small integers."""
+    a = np.array([1, 2, -3, 0.5, 1024, -0.25, 7, 0], np.float32)
+    b = np.array([4, -0.5, 3, 8, 2 ** -10, -16, 0, 5], np.float32)
+    assert oracle.mul(a, b).tolist() == [4.0, -1.0, -9.0, 4.0, 1.0, 4.0, 0.0, 0.0]
+    assert oracle.add(a, b).tolist() == [5.0, 1.5, 0.0, 8.5, 1024 + 2 ** -10, -16.25, 7.0, 5.0]
+    rng = np.random.default_rng(5)
+    x, y = rng.standard_normal(1000).astype(np.float32), rng.standard_normal(1000).astype(np.float32)
+    assert np.array_equal(oracle.add(x, y), oracle.add(y, x))                 # commutative
+    assert np.array_equal(oracle.mul(x, np.ones_like(x)), x.astype(np.float64))   # K = 1 is the identity (Eq. (10) step)
+    assert oracle.mul(x, y).dtype == np.float64 and oracle.mul(x.reshape(10, 100), y.reshape(10, 100)).shape == (10, 100)
+
+
+def test_arith_sum_gauss_and_cancellation(oracle):
+    """Eq. (11): 1 + 2 + ... + n = n (n + 1) / 2; a sum whose naive float32 accumulation fails; math.fsum."""
+    import math
+    n = 4096
+    assert oracle.summation(np.arange(1, n + 1, dtype=np.float32)) == n * (n + 1) / 2
+    x = np.array([1e8, 1.0, -1e8, 1.0] * 100, np.float32)
+    assert oracle.summation(x) == 200.0
+    rng = np.random.default_rng(6)
+    r = rng.standard_normal((3, 5000)).astype(np.float32)
+    got = oracle.summation(r)
+    for i in range(3):
+        assert abs(got[i] - math.fsum(float(v) for v in r[i])) <= 1e-12 * np.abs(r[i]).sum()
+    assert oracle.summation(np.zeros((2, 0), np.float32)).tolist() == [0.0, 0.0]
+
+
+def test_arith_matmul_textbook_and_dft(oracle):
+    """Eq. (7): a 2x3 by 3x2 product worked by hand; identity / permutation; (XY)^T = Y^T X^T; and the cross-pin the
+    paper itself draws (section 4.1): the DFT is a matrix product with the Fourier matrix, so the real and imaginary
+    parts of oracle.dft must equal oracle.matmul against cos / -sin matrices built here with numpy."""
+    X = np.array([[1, 2, 3], [4, 5, 6]], np.float32)
+    Y = np.array([[7, 8], [9, 10], [11, 12]], np.float32)
+    assert oracle.matmul(X, Y).tolist() == [[58.0, 64.0], [139.0, 154.0]]
+    rng = np.random.default_rng(7)
+    A = rng.standard_normal((5, 7)).astype(np.float32)
+    B = rng.standard_normal((7, 4)).astype(np.float32)
+    assert np.array_equal(oracle.matmul(A, np.eye(7, dtype=np.float32)), A.astype(np.float64))
+    perm = np.eye(7, dtype=np.float32)[:, ::-1]
+    assert np.array_equal(oracle.matmul(A, perm), A[:, ::-1].astype(np.float64))
+    np.testing.assert_allclose(oracle.matmul(A, B).T, oracle.matmul(B.T.copy(), A.T.copy()), rtol=0, atol=1e-14)
+    brute = [[sum(float(A[m, l]) * float(B[l, n]) for l in range(7)) for n in range(4)] for m in range(5)]
+    np.testing.assert_allclose(oracle.matmul(A, B), brute, rtol=0, atol=1e-14)
+    N = 16
+    x = rng.standard_normal((3, N)).astype(np.float32)
+    ang = 2 * np.pi * np.outer(np.arange(N), np.arange(N)) / N
+    C, S = np.cos(ang).astype(np.float32), (-np.sin(ang)).astype(np.float32)
+    Z = oracle.dft(x.astype(np.complex64))
+    np.testing.assert_allclose(oracle.matmul(x, C), Z.real, atol=2e-6)      # float32 twiddles: ~N * 6e-8 * |x|
+    np.testing.assert_allclose(oracle.matmul(x, S), Z.imag, atol=2e-6)
