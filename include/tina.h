@@ -132,6 +132,20 @@ tina_status tina_pfb_batched_host(const void* x_host, int S, long long n_samples
  * re-reads of x are served by L1 / L2).  Errors: NULL_POINTER, BAD_SHAPE, CUDA.                  */
 tina_status tina_unfold(const float* x, float* y, long long I, int J, void* stream);
 
+/* Arithmetic building blocks of the paper's section 3 (device pointers, float32, row-major):
+ *   tina_mul    Eq. (6):   out[c] = a[c] * b[c],        c in [0, n)
+ *   tina_add    Eq. (10):  out[c] = b[c] + a[c]
+ *   tina_sum    Eq. (11):  out[r] = sum_c x[r][c],      x [rows][n], out [rows]; accumulated in
+ *               short float32 chains combined in double precision; rows <= 65535; n = 0 gives 0
+ *   tina_matmul Eq. (7):  z[m][n] = sum_l x[m][l] y[l][n],  x [M][L], y [L][N], z [M][N];
+ *               float32 FMAs on the CUDA cores (a plain GEMM); z must not alias x or y; L = 0 gives zeros
+ * out may alias a or b in tina_mul / tina_add.  n, rows, M, L, N >= 0 else BAD_SHAPE; NULL_POINTER for a null
+ * pointer with non-empty data; CUDA on a launch failure.  All calls are asynchronous on `stream`.         */
+tina_status tina_mul(const float* a, const float* b, float* out, long long n, void* stream);
+tina_status tina_add(const float* a, const float* b, float* out, long long n, void* stream);
+tina_status tina_sum(const float* x, long long rows, long long n, float* out, void* stream);
+tina_status tina_matmul(const float* x, const float* y, float* z, long long M, long long L, long long N, void* stream);
+
 /* F = floor(n_samples / P) - M + 1; <= 0 means the input is too short.                     */
 long long   tina_pfb_num_frames(long long n_samples, int P, int M);
 

@@ -18,7 +18,8 @@ _lib = None
 
 EXPORTS = ["tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
            "tina_pfb_batched_host", "tina_pfb_num_frames", "tina_status_string", "tina_last_error",
-           "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path"]
+           "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path",
+           "tina_mul", "tina_add", "tina_sum", "tina_matmul"]
 
 
 class TinaError(RuntimeError):
@@ -44,6 +45,12 @@ def lib() -> ctypes.CDLL:
     L.tina_pfb_fir_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, vp, vp]
     L.tina_pfb_fft_batched.argtypes = [vp, ci, ll, ci, ci, vp, ci, vp, vp]
     L.tina_pfb_batched_host.argtypes = [vp, ci, ll, ci, ci, vp, ci, ci, vp, vp]
+    L.tina_mul.argtypes = [vp, vp, vp, ll, vp]
+    L.tina_add.argtypes = [vp, vp, vp, ll, vp]
+    L.tina_sum.argtypes = [vp, ll, ll, vp, vp]
+    L.tina_matmul.argtypes = [vp, vp, vp, ll, ll, ll, vp]
+    for f in ("tina_mul", "tina_add", "tina_sum", "tina_matmul"):
+        getattr(L, f).restype = ci
     for f in ("tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
               "tina_pfb_batched_host", "tina_clear_plan_cache", "tina_version", "tina_last_path"):
         getattr(L, f).restype = ci
@@ -128,6 +135,60 @@ def unfold(x, J: int, out=None, stream=None):
         out = torch.empty((max(I - J + 1, 0), J), dtype=torch.float32, device=x.device)
     _dev(out, torch.float32, "out")
     _check(lib().tina_unfold(x.data_ptr(), out.data_ptr(), I, J, _stream_ptr(stream)))
+    return out
+
+
+def _ew(fn, a, b, out, stream):
+    import torch
+    a, b = _dev(a, torch.float32, "a"), _dev(b, torch.float32, "b")
+    if a.shape != b.shape:
+        raise ValueError("a and b must have the same shape")
+    if out is None:
+        out = torch.empty_like(a)
+    _dev(out, torch.float32, "out")
+    _check(fn(a.data_ptr(), b.data_ptr(), out.data_ptr(), a.numel(), _stream_ptr(stream)))
+    return out
+
+
+def mul(a, b, out=None, stream=None):
+    """tina_mul, Eq. (6): elementwise product of two float32 CUDA tensors."""
+    return _ew(lib().tina_mul, a, b, out, stream)
+
+
+def add(a, b, out=None, stream=None):
+    """tina_add, Eq. (10): elementwise sum of two float32 CUDA tensors."""
+    return _ew(lib().tina_add, a, b, out, stream)
+
+
+def summation(x, out=None, stream=None):
+    """tina_sum, Eq. (11): sum over the last axis.  x [rows, n] (or [n]) float32 CUDA -> [rows] (or 0-d)."""
+    import torch
+    x = _dev(x, torch.float32, "x")
+    one_d = x.dim() == 1
+    if one_d:
+        x = x[None, :]
+    if x.dim() != 2:
+        raise ValueError("x must be 1-D or 2-D")
+    rows, n = x.shape
+    if out is None:
+        out = torch.empty((rows,), dtype=torch.float32, device=x.device)
+    _dev(out, torch.float32, "out")
+    _check(lib().tina_sum(x.data_ptr(), rows, n, out.data_ptr(), _stream_ptr(stream)))
+    return out[0] if one_d else out
+
+
+def matmul(x, y, out=None, stream=None):
+    """tina_matmul, Eq. (7): x [M, L] @ y [L, N] -> [M, N], float32 CUDA, row-major."""
+    import torch
+    x, y = _dev(x, torch.float32, "x"), _dev(y, torch.float32, "y")
+    if x.dim() != 2 or y.dim() != 2 or x.shape[1] != y.shape[0]:
+        raise ValueError("need x [M, L] and y [L, N]")
+    M, L = x.shape
+    N = y.shape[1]
+    if out is None:
+        out = torch.empty((M, N), dtype=torch.float32, device=x.device)
+    _dev(out, torch.float32, "out")
+    _check(lib().tina_matmul(x.data_ptr(), y.data_ptr(), out.data_ptr(), M, L, N, _stream_ptr(stream)))
     return out
 
 

@@ -240,6 +240,36 @@ tina_status tina_unfold(const float* x, float* y, long long I, int J, void* stre
     return simt_unfold(x, y, I, J, (cudaStream_t)stream);
 }
 
+tina_status tina_mul(const float* a, const float* b, float* out, long long n, void* stream)
+{
+    if (n < 0) return fail(TINA_ERR_BAD_SHAPE, "tina_mul: n < 0");
+    if (n > 0 && (!a || !b || !out)) return fail(TINA_ERR_NULL_POINTER, "tina_mul: null pointer");
+    return arith_ew(a, b, out, n, true, (cudaStream_t)stream);
+}
+
+tina_status tina_add(const float* a, const float* b, float* out, long long n, void* stream)
+{
+    if (n < 0) return fail(TINA_ERR_BAD_SHAPE, "tina_add: n < 0");
+    if (n > 0 && (!a || !b || !out)) return fail(TINA_ERR_NULL_POINTER, "tina_add: null pointer");
+    return arith_ew(a, b, out, n, false, (cudaStream_t)stream);
+}
+
+tina_status tina_sum(const float* x, long long rows, long long n, float* out, void* stream)
+{
+    if (rows < 0 || n < 0) return fail(TINA_ERR_BAD_SHAPE, "tina_sum: negative size");
+    if (rows > 0 && (!out || (n > 0 && !x))) return fail(TINA_ERR_NULL_POINTER, "tina_sum: null pointer");
+    return arith_sum(x, rows, n, out, (cudaStream_t)stream);
+}
+
+tina_status tina_matmul(const float* x, const float* y, float* z, long long M, long long L, long long N, void* stream)
+{
+    if (M < 0 || L < 0 || N < 0) return fail(TINA_ERR_BAD_SHAPE, "tina_matmul: negative size");
+    if (M > 0 && N > 0 && (!z || (L > 0 && (!x || !y)))) return fail(TINA_ERR_NULL_POINTER, "tina_matmul: null pointer");
+    if ((const void*)z == (const void*)x || (const void*)z == (const void*)y)
+        return fail(TINA_ERR_BAD_SHAPE, "tina_matmul: in-place not supported");
+    return arith_matmul(x, y, z, M, L, N, (cudaStream_t)stream);
+}
+
 long long tina_pfb_num_frames(long long n_samples, int P, int M)
 {
     if (P < 1 || M < 1 || n_samples < 0) return 0;

@@ -43,6 +43,9 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
 void umma_clear_plans();
 // PFB with the factorised (two-stage, 32 x 32) Fourier stage: complex kind, P = 1024, M <= 16 (tina_ct.cu)
 tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st);
+tina_status arith_ew(const float* a, const float* b, float* o, long long n, bool mul, cudaStream_t st);
+tina_status arith_sum(const float* x, long long rows, long long n, float* out, cudaStream_t st);
+tina_status arith_matmul(const float* x, const float* y, float* z, long long M, long long L, long long N, cudaStream_t st);
 tina_status ctr_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st);
 // standalone FIR as a Toeplitz contraction on the tensor cores; false = shape not covered (use simt_fir)
 bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, int M, cudaStream_t st,

@@ -435,3 +435,69 @@ def test_error_paths(tina):
     with pytest.raises(tina.TinaError) as e:
         tina.dft(torch.zeros((1, 16384), dtype=torch.complex64, device="cuda"))
     assert e.value.status == 3
+
+
+# ---------------------------------------------------------------- section 3 arithmetic blocks
+@pytest.mark.parametrize("n", [0, 1, 5, 1023, 4096, (1 << 20) + 3])
+def test_arith_mul_add(tina, oracle, n):
+    """Eq. (6) / (10): one float32 rounding per element (the oracle's float64 value rounded to float32 is the exact
+    expected result, so the comparison is bit-exact); unaligned views take the scalar path; in-place is allowed."""
+    import torch
+    rng = np.random.default_rng(900 + n % 97)
+    a = rng.standard_normal(n + 1).astype(np.float32)
+    b = rng.standard_normal(n + 1).astype(np.float32)
+    for off in (0, 1):                                       # off = 1: 4-byte-aligned views
+        ad, bd = _cuda(a)[off:off + n], _cuda(b)[off:off + n]
+        ah, bh = a[off:off + n], b[off:off + n]
+        got_m = tina.mul(ad, bd); got_a = tina.add(ad, bd); torch.cuda.synchronize()
+        assert np.array_equal(got_m.cpu().numpy(), oracle.mul(ah, bh).astype(np.float32))
+        assert np.array_equal(got_a.cpu().numpy(), oracle.add(ah, bh).astype(np.float32))
+    if n:
+        ad = _cuda(a[:n].copy())
+        tina.mul(ad, _cuda(b[:n].copy()), out=ad); torch.cuda.synchronize()
+        assert np.array_equal(ad.cpu().numpy(), oracle.mul(a[:n], b[:n]).astype(np.float32))
+
+
+@pytest.mark.parametrize("rows,n", [(1, 0), (1, 1), (3, 1000), (1, 4096 * 37 + 11), (257, 513), (2, 1 << 22), (4096, 64)])
+def test_arith_sum(tina, oracle, rows, n):
+    """Eq. (11): |got - ref| <= 1e-6 sum|x| + one float32 rounding of the result."""
+    import torch
+    rng = np.random.default_rng(910 + rows)
+    x = (rng.standard_normal((rows, n)) + 0.25).astype(np.float32)
+    got = tina.summation(_cuda(x)); torch.cuda.synchronize()
+    ref = oracle.summation(x)
+    tol = 1e-6 * np.abs(x).sum(axis=1, dtype=np.float64) + 6e-8 * np.abs(ref) + 1e-30
+    assert np.all(np.abs(got.cpu().numpy().astype(np.float64) - ref) <= tol)
+    if n:
+        one = tina.summation(_cuda(x[0])); torch.cuda.synchronize()
+        assert abs(float(one) - ref[0]) <= tol[0]
+
+
+@pytest.mark.parametrize("M,L,N", [(1, 1, 1), (2, 3, 2), (128, 16, 128), (129, 17, 131), (300, 1000, 70), (64, 4096, 256),
+                                   (5, 0, 7), (1000, 64, 1000)])
+def test_arith_matmul(tina, oracle, M, L, N):
+    """Eq. (7) against the float64 triple loop: |Z - Zref|(m, n) <= 1e-5 |X(m, :)| |Y(:, n)| (fp32 FMA chains of length L:
+    the bound is L eps / 2 in the worst case, sqrt(L) eps typically); ragged tiles; L = 0 gives zeros."""
+    import torch
+    rng = np.random.default_rng(920 + M + N)
+    X = rng.standard_normal((M, L)).astype(np.float32)
+    Y = rng.standard_normal((L, N)).astype(np.float32)
+    got = tina.matmul(_cuda(X), _cuda(Y)); torch.cuda.synchronize()
+    ref = oracle.matmul(X, Y)
+    bound = 1e-5 * np.outer(np.linalg.norm(X.astype(np.float64), axis=1), np.linalg.norm(Y.astype(np.float64), axis=0)) + 1e-30
+    assert got.shape == (M, N)
+    assert np.all(np.abs(got.cpu().numpy().astype(np.float64) - ref) <= bound)
+    if (M, L, N) == (2, 3, 2):                               # the hand-worked example of the oracle pin
+        Z = tina.matmul(_cuda(np.array([[1, 2, 3], [4, 5, 6]], np.float32)), _cuda(np.array([[7, 8], [9, 10], [11, 12]], np.float32)))
+        assert Z.cpu().numpy().tolist() == [[58.0, 64.0], [139.0, 154.0]]
+
+
+def test_arith_error_paths(tina):
+    import torch
+    L = tina.lib()
+    x = torch.zeros(16, device="cuda")
+    assert L.tina_mul(x.data_ptr(), x.data_ptr(), x.data_ptr(), -1, None) == 2
+    assert L.tina_add(None, x.data_ptr(), x.data_ptr(), 4, None) == 1
+    assert L.tina_sum(x.data_ptr(), -1, 4, x.data_ptr(), None) == 2
+    assert L.tina_matmul(x.data_ptr(), x.data_ptr(), x.data_ptr(), 2, 2, 2, None) == 2      # aliasing
+    assert L.tina_matmul(None, x.data_ptr(), x.data_ptr(), 2, 2, 2, None) == 1
