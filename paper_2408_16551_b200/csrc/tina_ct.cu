@@ -258,6 +258,225 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
     if (warp == 0) tmem_dealloc<1>(tmem, 256);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Warp-specialised variant: one CTA per SM, 20 warps.  Warps 0-7 (two warpgroups, 144 registers) only run the subfilter
+// stage and keep TWO columns of loads in flight; warps 8-15 (80 registers) only run the two epilogues; warp 16 (32
+// registers) issues the MMAs.  setmaxnreg moves registers inside the CTA's launch allocation (96 x 640 = 61440), so
+// 256 x 144 + 256 x 80 + 128 x 32 must not exceed it.  Two operand slots (2 x 64 KB) and two accumulator slots (2 x 128 TMEM columns) form a ring, so the loads and
+// FMAs of group i + 1 overlap the MMAs and epilogues of group i inside the CTA.  Same arithmetic as pfb_ct_kernel.
+constexpr int WS_THREADS = 640, WS_PROD = 256, WS_EPI = 256;
+constexpr int WS_SLOTS = 2;
+constexpr int WS_SLOT_BYTES = CT_NT * 2 * CT_TILE;        // 64 KB
+
+struct WsSmem {
+    uint8_t a[WS_SLOTS][WS_SLOT_BYTES];
+    uint8_t bm[2 * 64 * 64 * 2];
+    float2 tw[CT_A * CT_B];
+    uint64_t a1_full[WS_SLOTS], d1_full[WS_SLOTS], a2_full[WS_SLOTS], d2_full[WS_SLOTS], d_free[WS_SLOTS];
+    uint32_t tmem_base;
+};
+
+template <int R> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(R)); }
+template <int R> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(R)); }
+
+template <int MT>
+__global__ void __maxnreg__(96)
+pfb_ctws_kernel(const float2* __restrict__ x, long long stream_stride, const float* __restrict__ window,
+                const __nv_bfloat16* __restrict__ w32, float2* __restrict__ out, long long F, long long NBLK, int M,
+                int groups_per_stream, int total_groups)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    WsSmem& sm = *reinterpret_cast<WsSmem*>(smem_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    for (int e = tid; e < 2 * 64 * 64; e += WS_THREADS) {
+        const int part = e / 4096, n = (e % 4096) / 64, c = e % 64;
+        *reinterpret_cast<__nv_bfloat16*>(sm.bm + part * 8192 + sw128_off(n, c * 2)) = w32[part * 4096 + n * 64 + c];
+    }
+    for (int e = tid; e < CT_A * CT_B; e += WS_THREADS) {
+        const int kb = e / CT_A, a = e % CT_A;
+        double sn, cs;
+        sincospi(2.0 * (double)((a * kb) % CT_P) / (double)CT_P, &sn, &cs);
+        sm.tw[e] = make_float2((float)cs, (float)-sn);
+    }
+    if (tid == 0) {
+        for (int s = 0; s < WS_SLOTS; ++s) {
+            mbar_init(smem_u32(&sm.a1_full[s]), WS_PROD);
+            mbar_init(smem_u32(&sm.d1_full[s]), 1);
+            mbar_init(smem_u32(&sm.a2_full[s]), WS_EPI);
+            mbar_init(smem_u32(&sm.d2_full[s]), 1);
+            mbar_init(smem_u32(&sm.d_free[s]), WS_EPI);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 0) { tmem_alloc<1>(smem_u32(&sm.tmem_base), 512); tmem_relinquish<1>(); }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+    const int n_groups = ((int)blockIdx.x < total_groups) ? (total_groups - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    constexpr int WA = MT, NR = WA - 1 + CT_FR;
+
+    if (warp < 8) {
+        // ================================================================== producers: subfilter stage
+        setmaxnreg_inc<144>();
+        const uint32_t fir_off = lane * 128 + ((warp ^ (lane & 7)) << 4);
+        const uint32_t tap_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + 256 + (warp >> 2) * 64;
+#pragma unroll 1
+        for (int cb = 0; cb < CT_BPW; ++cb) {
+            uint32_t tv[16];
+#pragma unroll
+            for (int m = 0; m < 16; ++m)
+                tv[m] = m < M ? __float_as_uint(__ldg(window + (long long)m * CT_P + lane + CT_A * (CT_BPW * warp + cb))) : 0u;
+            tmem_st16(tap_addr + cb * 16, tv);
+        }
+        tmem_st_wait();
+        auto load_col = [&](int gg, int cb, float2 (&row)[NR]) {
+            const long long r0 = (long long)(gg % groups_per_stream) * CT_FR + M - WA;
+            const float2* xg = x + (long long)(gg / groups_per_stream) * stream_stride + r0 * CT_P + lane + CT_A * (CT_BPW * warp + cb);
+            if (r0 >= 0 && r0 + NR <= NBLK) {
+#pragma unroll
+                for (int j = 0; j < NR; ++j) row[j] = ldg_stream(xg + j * CT_P);
+            } else {
+#pragma unroll
+                for (int j = 0; j < NR; ++j) row[j] = (r0 + j >= 0 && r0 + j < NBLK) ? ldg_stream(xg + j * CT_P) : make_float2(0.f, 0.f);
+            }
+        };
+        float2 rows[2][NR];
+        if (n_groups > 0) load_col(blockIdx.x, 0, rows[0]);
+#pragma unroll 1
+        for (int i = 0; i < n_groups; ++i) {
+            const int g = (int)blockIdx.x + i * (int)gridDim.x, slot = i & 1;
+            uint8_t* const abase = sm.a[slot];
+            uint32_t hprev[CT_FR], lprev[CT_FR];
+#pragma unroll
+            for (int cb = 0; cb < CT_BPW; ++cb) {
+                uint32_t tv[16];
+                tmem_ld16(tap_addr + cb * 16, tv);
+                // the next column (or column 0 of the next group) is requested before this one is computed
+                if (cb + 1 < CT_BPW) load_col(g, cb + 1, rows[(cb + 1) & 1]);
+                else if (i + 1 < n_groups) load_col(g + (int)gridDim.x, 0, rows[0]);
+                float2 (&row)[NR] = rows[cb & 1];
+                tmem_ld_wait();
+                // the slot's previous contents (stage-2 operand of group i - 2) must have been consumed
+                if (cb == 1 && i >= WS_SLOTS) mbar_wait(smem_u32(&sm.d2_full[slot]), ((i >> 1) - 1) & 1u);
+#pragma unroll
+                for (int fl = 0; fl < CT_FR; ++fl) {
+                    const float t0 = __uint_as_float(tv[0]);
+                    float2 y = make_float2(t0 * row[fl + WA - 1].x, t0 * row[fl + WA - 1].y);
+#pragma unroll
+                    for (int m = 1; m < WA; ++m) y = ffma2_bc(__uint_as_float(tv[m]), row[fl + WA - 1 - m], y);
+                    uint32_t hb, lb;
+                    split_pack(y.x, y.y, hb, lb);
+                    if (cb & 1) {
+                        uint8_t* const dst = abase + fir_off + (cb - 1) * 4 + (fl >> 2) * 2 * CT_TILE + (fl & 3) * 32 * 128;
+                        *reinterpret_cast<uint2*>(dst) = make_uint2(hprev[fl], hb);
+                        *reinterpret_cast<uint2*>(dst + CT_TILE) = make_uint2(lprev[fl], lb);
+                    } else {
+                        hprev[fl] = hb;
+                        lprev[fl] = lb;
+                    }
+                }
+            }
+            fence_proxy_async();
+            mbar_arrive(smem_u32(&sm.a1_full[slot]));
+        }
+    } else if (warp < 16) {
+        // ================================================================== epilogue warps
+        setmaxnreg_dec<80>();
+        const int e = warp - 8, et = e >> 2, eq = e & 3;
+        auto epi2 = [&](int i) {
+            const int g = (int)blockIdx.x + i * (int)gridDim.x, slot = i & 1;
+            const int s = g / groups_per_stream;
+            const long long f = (long long)(g % groups_per_stream) * CT_FR + et * 4 + eq;
+            mbar_wait(smem_u32(&sm.d2_full[slot]), (i >> 1) & 1u);
+            tc_fence_after();
+            float2* const orow = out + ((long long)s * F + f) * CT_P + lane;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * slot + 64 * et + 32 * h, v);
+                tmem_ld_wait();
+                if (f < F) {
+#pragma unroll
+                    for (int q = 0; q < 16; ++q)
+                        orow[(16 * h + q) * 32] = make_float2(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(smem_u32(&sm.d_free[slot]));
+        };
+#pragma unroll 1
+        for (int i = 0; i < n_groups; ++i) {
+            const int slot = i & 1;
+            uint8_t* const etile = sm.a[slot] + et * 2 * CT_TILE;
+            mbar_wait(smem_u32(&sm.d1_full[slot]), (i >> 1) & 1u);
+            tc_fence_after();
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * slot + 64 * et + 32 * h, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const int kb = 16 * h + q;
+                    const float gr = __uint_as_float(v[2 * q]), gi = __uint_as_float(v[2 * q + 1]);
+                    const float2 w = sm.tw[kb * CT_A + lane];
+                    split_store(etile, sw128_off(eq * 32 + kb, lane * 4), gr * w.x - gi * w.y, gr * w.y + gi * w.x);
+                }
+            }
+            fence_proxy_async();
+            tc_fence_before();
+            mbar_arrive(smem_u32(&sm.a2_full[slot]));
+            if (i >= 1) epi2(i - 1);                    // while the stage-2 MMAs of group i run
+        }
+        if (n_groups > 0) epi2(n_groups - 1);
+    } else {
+        // ================================================================== MMA issuer (warp 16; warps 17-19 idle)
+        setmaxnreg_dec<32>();
+        if (warp == 16 && lane == 0) {
+            const uint32_t idesc = idesc_bf16(128, 64);
+            const uint64_t d_bh = smem_desc_sw128(smem_u32(sm.bm)), d_bl = smem_desc_sw128(smem_u32(sm.bm + 8192));
+            constexpr uint64_t TILE_DESC = (uint64_t)(2 * CT_TILE) >> 4, PART_DESC = (uint64_t)CT_TILE >> 4;
+            auto stage = [&](int slot, uint64_t bar) {
+                const uint64_t d_ah = smem_desc_sw128(smem_u32(sm.a[slot]));
+#pragma unroll
+                for (int t = 0; t < CT_NT; ++t) {
+                    const uint32_t dcol = tmem + 128 * slot + 64 * t;
+                    const uint64_t da = d_ah + t * TILE_DESC;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + PART_DESC + 2 * k, d_bh + 2 * k, idesc, k > 0);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bh + 2 * k, idesc, 1);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bl + 2 * k, idesc, 1);
+                }
+                umma_commit((uint32_t)bar);
+            };
+#pragma unroll 1
+            for (int i = 0; i <= n_groups; ++i) {
+                if (i < n_groups) {
+                    const int slot = i & 1;
+                    mbar_wait(smem_u32(&sm.a1_full[slot]), (i >> 1) & 1u);
+                    if (i >= WS_SLOTS) mbar_wait(smem_u32(&sm.d_free[slot]), ((i >> 1) - 1) & 1u);   // accumulators drained
+                    tc_fence_after();
+                    stage(slot, smem_u32(&sm.d1_full[slot]));
+                }
+                if (i >= 1) {
+                    const int slot = (i - 1) & 1;
+                    mbar_wait(smem_u32(&sm.a2_full[slot]), ((i - 1) >> 1) & 1u);
+                    tc_fence_after();
+                    stage(slot, smem_u32(&sm.d2_full[slot]));
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<1>(tmem, 512);
+}
+
 }  // namespace tina
 
 namespace tina {
@@ -284,6 +503,26 @@ tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float
         if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "pfb_ct_kernel setup"); }
     }
     const int total = (int)(gps * S);
+    if (!getenv("TINA_CT_NO_WS")) {                         // warp-specialised variant: one 640-thread CTA per SM
+        static bool ws_ready = false;
+        if (!ws_ready) {
+            cudaError_t e = cudaFuncSetAttribute(pfb_ctws_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WsSmem) + 1024);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctws_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WsSmem) + 1024);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctws_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WsSmem) + 1024);
+            if (e != cudaSuccess) return check_cuda(e, "pfb_ctws_kernel setup");
+            ws_ready = true;
+        }
+        const int grid = total < n_sm ? total : n_sm;
+        const size_t smem = sizeof(WsSmem) + 1024;
+        const float2* xf = static_cast<const float2*>(x);
+        float2* of = static_cast<float2*>(out);
+        if (M <= 4) pfb_ctws_kernel<4><<<grid, WS_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
+        else if (M <= 8) pfb_ctws_kernel<8><<<grid, WS_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
+        else pfb_ctws_kernel<16><<<grid, WS_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
+        count_launch();
+        g_last_path = kPathUmma;
+        return check_cuda(cudaGetLastError(), "pfb_ctws_kernel launch");
+    }
     const int per_sm = 2;                                   // 256 threads, 89 KB shared memory, 128 TMEM columns per CTA
     const int grid = total < n_sm * per_sm ? total : n_sm * per_sm;
     const size_t smem = sizeof(CtSmem) + 1024;
