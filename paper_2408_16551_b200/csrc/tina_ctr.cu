@@ -304,6 +304,306 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
     if (warp == 0) tmem_dealloc<1>(tmem, 512);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Warp-specialised variant (the default; TINA_CTR_NO_WS=1 selects the kernel above).  One CTA per SM, 20 warps:
+//   warps 0-7   producers: subfilter stage only.  A thread owns a = 2 lane, 2 lane + 1 of columns b = 8 warp .. + 7 and a
+//               GROUP of 4 frames (two 128-row tiles), loads one column ahead, writes the stage-1 operands of both tiles;
+//   warps 8-15  epilogues, per TILE: epilogue 1 of tile T, then epilogue 2 of tile T - 1 (while the stage-2 MMAs of T run);
+//   warp 16     issues the MMAs: stage 1 of tile T, then stage 2 of tile T - 1.
+// Shared memory: four stage-1 operand tiles (a ring of two groups, 128 KB), ONE stage-2 operand tile (64 KB), B1 (32 KB).
+// The twiddle W4096^(a kb) no longer comes from a 34 KB table: an epilogue thread has a fixed kb, so it keeps
+// W^(8 ah kb), ah = 0..7, and W^(al kb), al = 0..7, in registers and multiplies the two.
+// TMEM: two 128-column accumulator slots (tile parity; stage 2 of a tile overwrites its own stage-1 columns once
+// epilogue 1 has read them) + 256 columns of window taps.  Registers move with setmaxnreg inside 96 x 640.
+constexpr int CW_THREADS = 640, CW_PROD = 256, CW_EPI = 256;
+constexpr int CW_BPW = 8;                             // b values per producer warp (8 warps x 8 = 64)
+
+struct CwSmem {
+    uint8_t a1[4][2][CR_TILE];                        // [tile slot][hi | lo]: rows (frame, rho(a)), K = b
+    uint8_t a2[2][2][CR_TILE];                        // [real | imaginary parts of G'][hi | lo]: rows (frame, kb), K = a
+    uint8_t bm[2][CR_TILE];
+    uint64_t a1_full[2], a1_free[2], d1_full[2], a2_full, d2_full[2], d_free[2];
+    uint32_t tmem_base;
+};
+static_assert(sizeof(CwSmem) + 1024 <= 227 * 1024, "shared memory budget");
+
+template <int R> __device__ __forceinline__ void cw_reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(R)); }
+template <int R> __device__ __forceinline__ void cw_reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(R)); }
+
+template <int MT>
+__global__ void __maxnreg__(96)
+pfb_ctrws_kernel(const float* __restrict__ x, long long stream_stride, const float* __restrict__ window,
+                 float2* __restrict__ out, long long F, long long NBLK, int M, int groups_per_stream, int total_groups)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    CwSmem& sm = *reinterpret_cast<CwSmem*>(smem_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    for (int e = tid; e < 128 * 64; e += CW_THREADS) {
+        const int n = e >> 6, b = e & 63, kb = n >> 1;
+        float sn, cs;
+        sincospif((float)((b * kb) & 63) * (1.0f / 32.0f), &sn, &cs);
+        const float v = (n & 1) ? -sn : cs;
+        const __nv_bfloat16 hi = __float2bfloat16_rn(v);
+        *reinterpret_cast<__nv_bfloat16*>(sm.bm[0] + cr_sw128(n, b * 2)) = hi;
+        *reinterpret_cast<__nv_bfloat16*>(sm.bm[1] + cr_sw128(n, b * 2)) = __float2bfloat16_rn(v - __bfloat162float(hi));
+    }
+    if (tid == 0) {
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(smem_u32(&sm.a1_full[s]), CW_PROD);
+            mbar_init(smem_u32(&sm.a1_free[s]), 1);
+            mbar_init(smem_u32(&sm.d1_full[s]), 1);
+            mbar_init(smem_u32(&sm.d2_full[s]), 1);
+            mbar_init(smem_u32(&sm.d_free[s]), CW_EPI);
+        }
+        mbar_init(smem_u32(&sm.a2_full), CW_EPI);
+        fence_mbar_init();
+    }
+    if (warp == 0) { tmem_alloc<1>(smem_u32(&sm.tmem_base), 512); tmem_relinquish<1>(); }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+    const int n_groups = ((int)blockIdx.x < total_groups) ? (total_groups - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    const int n_tiles = 2 * n_groups;
+    constexpr int WA = MT, NR = WA - 1 + CR_FR;
+
+    if (warp < 8) {
+        // ================================================================== producers: subfilter stage, Eq. (20)
+        cw_reg_inc<112>();
+        // taps of columns p = 2 lane (+ 1) + 64 (8 warp + bi): TMEM columns 256 + 128 (warp / 4) + 16 bi, (tap m of a,
+        // tap m of a + 1) pairs, zero beyond M
+        const uint32_t tap_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + 256 + (warp >> 2) * 128;
+#pragma unroll 1
+        for (int bi = 0; bi < CW_BPW; ++bi) {
+            uint32_t tv[16];
+            const float* wp = window + 2 * lane + 64 * (CW_BPW * warp + bi);
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                tv[2 * m] = m < M ? __float_as_uint(__ldg(wp + (long long)m * CR_P)) : 0u;
+                tv[2 * m + 1] = m < M ? __float_as_uint(__ldg(wp + (long long)m * CR_P + 1)) : 0u;
+            }
+            tmem_st16(tap_addr + bi * 16, tv);
+        }
+        tmem_st_wait();
+        // tile rows lane (a even) and lane + 32 (a odd) of each frame, K bytes 16 warp + 8 half .. + 7
+        const uint32_t fir_off = lane * 128 + ((((uint32_t)warp) ^ (lane & 7)) << 4);
+        auto load_col = [&](int gg, int bi, float2 (&row)[NR]) {
+            const long long r0 = (long long)(gg % groups_per_stream) * CR_FR + M - WA;
+            const float* xg = x + (long long)(gg / groups_per_stream) * stream_stride + r0 * CR_P + 2 * lane + 64 * (CW_BPW * warp + bi);
+            if (r0 >= 0 && r0 + NR <= NBLK) {                                  // uniform
+#pragma unroll
+                for (int j = 0; j < NR; ++j) row[j] = cr_ldg2(xg + j * CR_P);
+            } else {
+#pragma unroll
+                for (int j = 0; j < NR; ++j)
+                    row[j] = (r0 + j >= 0 && r0 + j < NBLK) ? cr_ldg2(xg + j * CR_P) : make_float2(0.f, 0.f);
+            }
+        };
+        float2 rows[2][NR];
+        if (n_groups > 0) load_col(blockIdx.x, 0, rows[0]);
+#pragma unroll 1
+        for (int i = 0; i < n_groups; ++i) {
+            const int g = (int)blockIdx.x + i * (int)gridDim.x;
+            uint8_t* const abase = &sm.a1[2 * (i & 1)][0][0] + fir_off;
+#pragma unroll 1
+            for (int half = 0; half < 2; ++half) {
+                uint32_t hA[CR_FR][2], lA[CR_FR][2], hB[CR_FR][2], lB[CR_FR][2];
+                uint32_t hprev[CR_FR], lprev[CR_FR];
+#pragma unroll
+                for (int b4 = 0; b4 < 4; ++b4) {
+                    const int bi = 4 * half + b4;
+                    uint32_t tv[16];
+                    tmem_ld16(tap_addr + bi * 16, tv);
+                    // the next column (or column 0 of the next group) is requested before this one is computed
+                    if (bi + 1 < CW_BPW) load_col(g, bi + 1, rows[(b4 + 1) & 1]);
+                    else if (i + 1 < n_groups) load_col(g + (int)gridDim.x, 0, rows[0]);
+                    float2 (&row)[NR] = rows[b4 & 1];
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int fl = 0; fl < CR_FR; ++fl) {
+                        float2 y = make_float2(__uint_as_float(tv[0]) * row[fl + WA - 1].x, __uint_as_float(tv[1]) * row[fl + WA - 1].y);
+#pragma unroll
+                        for (int m = 1; m < WA; ++m)
+                            y = cr_ffma2(make_float2(__uint_as_float(tv[2 * m]), __uint_as_float(tv[2 * m + 1])), row[fl + WA - 1 - m], y);
+                        uint32_t hb, lb;                                       // low half: a = 2 l, high half: a = 2 l + 1
+                        cr_split(y.x, y.y, hb, lb);
+                        if (b4 & 1) {
+                            hA[fl][b4 >> 1] = __byte_perm(hprev[fl], hb, 0x5410);
+                            hB[fl][b4 >> 1] = __byte_perm(hprev[fl], hb, 0x7632);
+                            lA[fl][b4 >> 1] = __byte_perm(lprev[fl], lb, 0x5410);
+                            lB[fl][b4 >> 1] = __byte_perm(lprev[fl], lb, 0x7632);
+                        } else {
+                            hprev[fl] = hb;
+                            lprev[fl] = lb;
+                        }
+                    }
+                }
+                // the slot's previous contents (stage-1 operands of group i - 2) must have been consumed
+                if (half == 0 && i >= 2) mbar_wait(smem_u32(&sm.a1_free[i & 1]), ((i >> 1) - 1) & 1u);
+#pragma unroll
+                for (int fl = 0; fl < CR_FR; ++fl) {
+                    uint8_t* const dst = abase + (fl >> 1) * 2 * CR_TILE + (fl & 1) * 64 * 128 + 8 * half;
+                    *reinterpret_cast<uint2*>(dst) = make_uint2(hA[fl][0], hA[fl][1]);
+                    *reinterpret_cast<uint2*>(dst + CR_TILE) = make_uint2(lA[fl][0], lA[fl][1]);
+                    *reinterpret_cast<uint2*>(dst + 32 * 128) = make_uint2(hB[fl][0], hB[fl][1]);
+                    *reinterpret_cast<uint2*>(dst + 32 * 128 + CR_TILE) = make_uint2(lB[fl][0], lB[fl][1]);
+                }
+            }
+            fence_proxy_async();
+            mbar_arrive(smem_u32(&sm.a1_full[i & 1]));
+        }
+    } else if (warp < 16) {
+        // ================================================================== epilogue warps
+        cw_reg_inc<104>();
+        const int e = warp - 8, eq = e & 3, eh = e >> 2;
+        const uint32_t tq = tmem + ((uint32_t)(eq * 32) << 16);
+        // epilogue 1: TMEM lane = (kb = 16 eq + lane / 2, c = lane & 1).  G' = G w with w = W4096^(a kb) = (wr, wi):
+        // Re = Gr wr - Gi wi, Im = Gi wr + Gr wi  ->  own * wr + partner * sgn wi, sgn = c ? 1 : -1.
+        // w(a) = base[a / 8] * step[a % 8]; the sign is folded into the imaginary parts (sgn^2 = 1).
+        const int kb = 16 * eq + (lane >> 1), c = lane & 1;
+        float br[8], bj[8], sr[8], sj[8];
+        {
+            // arguments j kb / 2048 are exact in fp32, so sincospif is good to about an ulp
+            const float sgn = c ? 1.f : -1.f;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                float sn, cs;
+                sincospif((float)((8 * j * kb) & 4095) * (1.0f / 2048.0f), &sn, &cs);
+                br[j] = cs;
+                bj[j] = -sn * sgn;
+                sincospif((float)(j * kb) * (1.0f / 2048.0f), &sn, &cs);
+                sr[j] = cs;
+                sj[j] = -sn * sgn;
+            }
+        }
+        auto epi2 = [&](int T) {
+            // rows 32 eq .. + 31 = (frame eq / 2 of the tile, kb = 32 (eq & 1) + lane), ka = 16 eh .. + 15.
+            // D_R = (C_r, -S_r), D_I = (C_i, -S_i):  X = (C_r + S_i, C_i - S_r); 256 contiguous bytes per warp store.
+            const int g = (int)blockIdx.x + (T >> 1) * (int)gridDim.x;
+            const int s = g / groups_per_stream;
+            const long long f = (long long)(g % groups_per_stream) * CR_FR + 2 * (T & 1) + (eq >> 1);
+            float2* const orow = out + ((long long)s * F + f) * CR_NK + 32 * (eq & 1) + lane + 64 * 16 * eh;
+            mbar_wait(smem_u32(&sm.d2_full[T & 1]), (T >> 1) & 1u);
+            tc_fence_after();
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                uint32_t vr[16], vi[16];
+                tmem_ld16(tq + 128 * (T & 1) + 32 * eh + 16 * h, vr);
+                tmem_ld16(tq + 128 * (T & 1) + 64 + 32 * eh + 16 * h, vi);
+                tmem_ld_wait();
+                if (f < F) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q)
+                        orow[64 * (8 * h + q)] = make_float2(__uint_as_float(vr[2 * q]) - __uint_as_float(vi[2 * q + 1]),
+                                                             __uint_as_float(vr[2 * q + 1]) + __uint_as_float(vi[2 * q]));
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(smem_u32(&sm.d_free[T & 1]));
+        };
+#pragma unroll 1
+        for (int T = 0; T < n_tiles; ++T) {
+            const int g = (int)blockIdx.x + (T >> 1) * (int)gridDim.x;
+            const long long f = (long long)(g % groups_per_stream) * CR_FR + 2 * (T & 1) + eh;
+            const uint32_t row = eh * 64 + kb;
+            uint8_t* const blk = &sm.a2[c][0][0];
+            mbar_wait(smem_u32(&sm.d1_full[T & 1]), (T >> 1) & 1u);
+            tc_fence_after();
+            float nyq = 0.f;
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                // TMEM column rho of this frame holds a = 2 rho (rho < 32) or 2 (rho - 32) + 1: even a in ve, odd a in vo
+                uint32_t ve[8], vo[8];
+                tmem_ld8(tq + 128 * (T & 1) + 64 * eh + 8 * h, ve);
+                tmem_ld8(tq + 128 * (T & 1) + 64 * eh + 32 + 8 * h, vo);
+                tmem_ld_wait();
+                // the stage-2 operand tile is free once the stage-2 MMAs of tile T - 1 have retired
+                if (h == 0 && T >= 1) mbar_wait(smem_u32(&sm.d2_full[(T - 1) & 1]), ((T - 1) >> 1) & 1u);
+#pragma unroll
+                for (int j2 = 0; j2 < 2; ++j2) {                           // a = 8 j8 .. 8 j8 + 7
+                    const int j8 = 2 * h + j2;
+                    uint32_t hw[4], lw[4];
+                    // opaque to the optimiser: otherwise all 64 products are hoisted out of the tile loop and spilled
+                    asm volatile("" : "+f"(br[j8]), "+f"(bj[j8]));
+#pragma unroll
+                    for (int i2 = 0; i2 < 4; ++i2) {
+                        const int i = 4 * j2 + i2;                         // a = 8 j8 + 2 i2, + 1
+                        const float w0r = br[j8] * sr[2 * i2] - bj[j8] * sj[2 * i2], w0j = br[j8] * sj[2 * i2] + bj[j8] * sr[2 * i2];
+                        const float w1r = br[j8] * sr[2 * i2 + 1] - bj[j8] * sj[2 * i2 + 1], w1j = br[j8] * sj[2 * i2 + 1] + bj[j8] * sr[2 * i2 + 1];
+                        const float v0 = __uint_as_float(ve[i]), v1 = __uint_as_float(vo[i]);
+                        const float p0 = __shfl_xor_sync(0xffffffffu, v0, 1), p1 = __shfl_xor_sync(0xffffffffu, v1, 1);
+                        nyq += v0 - v1;
+                        const float o0 = fmaf(p0, w0j, v0 * w0r), o1 = fmaf(p1, w1j, v1 * w1r);
+                        cr_split(o0, o1, hw[i2], lw[i2]);
+                    }
+                    const uint32_t off = cr_sw128(row, 16 * j8);
+                    *reinterpret_cast<uint4*>(blk + off) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+                    *reinterpret_cast<uint4*>(blk + CR_TILE + off) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+                }
+            }
+            // k = 2048: X = sum_a (-1)^a G[a][0] (real; the lane holding (kb = 0, re) has all 64 terms)
+            if (eq == 0 && lane == 0 && f < F) out[((long long)(g / groups_per_stream) * F + f) * CR_NK + CR_P / 2] = make_float2(nyq, 0.f);
+            fence_proxy_async();
+            tc_fence_before();
+            mbar_arrive(smem_u32(&sm.a2_full));
+            if (T >= 1) epi2(T - 1);                    // while the stage-2 MMAs of tile T run
+        }
+        if (n_tiles > 0) epi2(n_tiles - 1);
+    } else {
+        // ================================================================== MMA issuer (warp 16; warps 17-19 idle)
+        cw_reg_dec<40>();
+        if (warp == 16 && lane == 0) {
+            const uint32_t idesc1 = idesc_bf16(128, 128), idesc2 = idesc_bf16(128, 64);
+            const uint64_t d_bh = smem_desc_sw128(smem_u32(sm.bm[0])), d_bl = smem_desc_sw128(smem_u32(sm.bm[1]));
+            const uint64_t d_a1 = smem_desc_sw128(smem_u32(&sm.a1[0][0][0])), d_a2 = smem_desc_sw128(smem_u32(&sm.a2[0][0][0]));
+            constexpr uint64_t PART = (uint64_t)CR_TILE >> 4, BLOCK = 2 * PART;   // descriptor steps
+#pragma unroll 1
+            for (int T = 0; T <= n_tiles; ++T) {
+                if (T < n_tiles) {
+                    // ---- stage 1 (transposed): D1^T = B1 * A1^T -> accumulator slot T & 1, columns = (frame, rho(a))
+                    const int i = T >> 1;
+                    if ((T & 1) == 0) mbar_wait(smem_u32(&sm.a1_full[i & 1]), (i >> 1) & 1u);
+                    if (T >= 2) mbar_wait(smem_u32(&sm.d_free[T & 1]), ((T >> 1) - 1) & 1u);      // accumulators drained
+                    tc_fence_after();
+                    const uint32_t dcol = tmem + 128 * (T & 1);
+                    const uint64_t da = d_a1 + (uint64_t)(T & 3) * BLOCK;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, d_bh + 2 * k, da + PART + 2 * k, idesc1, k > 0);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, d_bl + 2 * k, da + 2 * k, idesc1, 1);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, d_bh + 2 * k, da + 2 * k, idesc1, 1);
+                    umma_commit(smem_u32(&sm.d1_full[T & 1]));
+                    if (T & 1) umma_commit(smem_u32(&sm.a1_free[i & 1]));
+                }
+                if (T >= 1) {
+                    // ---- stage 2 of tile U: D_R = Re(G') B1[0..63]^T -> columns + 0 .. 63, D_I = Im(G') B1[0..63]^T -> + 64 .. 127
+                    const int U = T - 1;
+                    mbar_wait(smem_u32(&sm.a2_full), U & 1u);
+                    tc_fence_after();
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        const uint64_t da = d_a2 + c * BLOCK;
+                        const uint32_t dcol = tmem + 128 * (U & 1) + 64 * c;
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + PART + 2 * k, d_bh + 2 * k, idesc2, k > 0);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bh + 2 * k, idesc2, 1);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bl + 2 * k, idesc2, 1);
+                    }
+                    umma_commit(smem_u32(&sm.d2_full[U & 1]));
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<1>(tmem, 512);
+}
+
 tina_status ctr_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st)
 {
     const long long NBLK = n_samples / CR_P, F = NBLK - M + 1;
@@ -319,10 +619,25 @@ tina_status ctr_pfb(const void* x, int S, long long n_samples, int M, const floa
         if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "pfb_ctr_kernel setup"); }
     }
     const int total = (int)(gps * S);
-    const int grid = total < n_sm ? total : n_sm;           // 512 threads, 193 KB shared memory, all 512 TMEM columns
-    const size_t smem = sizeof(CrSmem) + 1024;
+    const int grid = total < n_sm ? total : n_sm;           // one CTA per SM (all 512 TMEM columns)
     const float* xf = static_cast<const float*>(x);
     float2* of = static_cast<float2*>(out);
+    if (getenv("TINA_CTR_WS")) {                            // warp-specialised variant: one 640-thread CTA per SM
+        static bool ws_ready = false;
+        const size_t wsmem = sizeof(CwSmem) + 1024;
+        if (!ws_ready) {
+            cudaError_t e = cudaFuncSetAttribute(pfb_ctrws_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctrws_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem);
+            if (e != cudaSuccess) return check_cuda(e, "pfb_ctrws_kernel setup");
+            ws_ready = true;
+        }
+        if (M <= 4) pfb_ctrws_kernel<4><<<grid, CW_THREADS, wsmem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
+        else pfb_ctrws_kernel<8><<<grid, CW_THREADS, wsmem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
+        count_launch();
+        g_last_path = kPathUmma;
+        return check_cuda(cudaGetLastError(), "pfb_ctrws_kernel launch");
+    }
+    const size_t smem = sizeof(CrSmem) + 1024;
     if (M <= 4) pfb_ctr_kernel<4><<<grid, CR_THREADS, smem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
     else pfb_ctr_kernel<8><<<grid, CR_THREADS, smem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
     count_launch();
