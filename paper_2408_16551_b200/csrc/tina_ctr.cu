@@ -305,16 +305,21 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Warp-specialised variant (the default; TINA_CTR_NO_WS=1 selects the kernel above).  One CTA per SM, 20 warps:
+// Warp-specialised variant, OPT-IN (TINA_CTR_WS=1): correct (same parity tests) but measured SLOWER than the kernel
+// above at config 5 (0.65 ms vs 0.60 ms), so it is not the default; kept as the measured experiment DESIGN.md describes.
+// One CTA per SM, 20 warps:
 //   warps 0-7   producers: subfilter stage only.  A thread owns a = 2 lane, 2 lane + 1 of columns b = 8 warp .. + 7 and a
 //               GROUP of 4 frames (two 128-row tiles), loads one column ahead, writes the stage-1 operands of both tiles;
-//   warps 8-15  epilogues, per TILE: epilogue 1 of tile T, then epilogue 2 of tile T - 1 (while the stage-2 MMAs of T run);
-//   warp 16     issues the MMAs: stage 1 of tile T, then stage 2 of tile T - 1.
+//   warps 8-15  epilogues, per TILE: epilogue 2 of tile T - 1, then epilogue 1 of tile T;
+//   warp 16     issues the MMAs: stage 1 of tile T + 1, then stage 2 of tile T.
 // Shared memory: four stage-1 operand tiles (a ring of two groups, 128 KB), ONE stage-2 operand tile (64 KB), B1 (32 KB).
-// The twiddle W4096^(a kb) no longer comes from a 34 KB table: an epilogue thread has a fixed kb, so it keeps
+// The twiddle W4096^(a kb) does not come from a 34 KB table here: an epilogue thread has a fixed kb, so it keeps
 // W^(8 ah kb), ah = 0..7, and W^(al kb), al = 0..7, in registers and multiplies the two.
 // TMEM: two 128-column accumulator slots (tile parity; stage 2 of a tile overwrites its own stage-1 columns once
 // epilogue 1 has read them) + 256 columns of window taps.  Registers move with setmaxnreg inside 96 x 640.
+// Why it loses: with 64 K registers per SM only 8 producer warps with one column of loads in flight fit next to the
+// epilogue warps (22 KB in flight per SM); the subfilter stage alone then takes 0.43 ms (role-skipping runs), against
+// 0.21 ms when all 16 warps of the kernel above load.
 constexpr int CW_THREADS = 640, CW_PROD = 256, CW_EPI = 256;
 constexpr int CW_BPW = 8;                             // b values per producer warp (8 warps x 8 = 64)
 
@@ -509,6 +514,7 @@ pfb_ctrws_kernel(const float* __restrict__ x, long long stream_stride, const flo
             const long long f = (long long)(g % groups_per_stream) * CR_FR + 2 * (T & 1) + eh;
             const uint32_t row = eh * 64 + kb;
             uint8_t* const blk = &sm.a2[c][0][0];
+            if (T >= 1) epi2(T - 1);                    // frees tile T - 1's accumulators (stage 1 of T + 1) and implies A2 is free
             mbar_wait(smem_u32(&sm.d1_full[T & 1]), (T >> 1) & 1u);
             tc_fence_after();
             float nyq = 0.f;
@@ -519,8 +525,6 @@ pfb_ctrws_kernel(const float* __restrict__ x, long long stream_stride, const flo
                 tmem_ld8(tq + 128 * (T & 1) + 64 * eh + 8 * h, ve);
                 tmem_ld8(tq + 128 * (T & 1) + 64 * eh + 32 + 8 * h, vo);
                 tmem_ld_wait();
-                // the stage-2 operand tile is free once the stage-2 MMAs of tile T - 1 have retired
-                if (h == 0 && T >= 1) mbar_wait(smem_u32(&sm.d2_full[(T - 1) & 1]), ((T - 1) >> 1) & 1u);
 #pragma unroll
                 for (int j2 = 0; j2 < 2; ++j2) {                           // a = 8 j8 .. 8 j8 + 7
                     const int j8 = 2 * h + j2;
@@ -548,7 +552,6 @@ pfb_ctrws_kernel(const float* __restrict__ x, long long stream_stride, const flo
             fence_proxy_async();
             tc_fence_before();
             mbar_arrive(smem_u32(&sm.a2_full));
-            if (T >= 1) epi2(T - 1);                    // while the stage-2 MMAs of tile T run
         }
         if (n_tiles > 0) epi2(n_tiles - 1);
     } else {

@@ -352,6 +352,24 @@ def test_pfb_fft_factorised_stage_real(tina, oracle, M, F, S):
     assert e.value.status == 3
 
 
+def test_pfb_fft_real_warp_specialised_variant(tina, oracle, monkeypatch):
+    """Opt-in warp-specialised real-kind kernel (TINA_CTR_WS=1; slower than the default, kept as a measured experiment):
+    same contract, enough frames for the two-group operand ring and both accumulator slots to wrap several times."""
+    import torch
+    monkeypatch.setenv("TINA_CTR_WS", "1")
+    for (M, F, S) in [(8, 4 * 148 * 5 + 3, 1), (4, 7, 2), (8, 1, 1), (5, 1300, 2)]:
+        rng = np.random.default_rng(160 + M)
+        case = ti.pfb_case(4096, M, F, real=True, streams=S, seed=161 + M + F, window=ti.random_taps(rng, 4096 * M))
+        out = tina.pfb_fft(_cuda(case.x), 4096, M, _cuda(case.window)); torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        assert got.shape == (S, F, 2049)
+        fr = ti.sample_frames(F, min(F, 48), 77 + F)
+        for s in range(S):
+            ref = oracle.pfb(case.x[s], 4096, M, case.window, frames=fr)
+            assert rel_l2_rows(got[s][fr], ref) <= TOL_FP32
+        assert np.all(got[..., 2048].imag == 0)
+
+
 def test_config5_full_size_factorised_sampled(tina, oracle):
     """c5 at full size through tina_pfb_fft_batched: first / last / seeded frames against the oracle."""
     import torch
