@@ -39,7 +39,8 @@ struct CrSmem {
     uint8_t a[2][2][2][CR_TILE];
     uint8_t bm[2][CR_TILE];                           // B1 hi | lo: row n = 2 kb + c, K = b, K-major SWIZZLE_128B
     float2 tw[64 * CR_TWP];                           // W4096^(a kb), [kb][a]
-    uint64_t bar[2];
+    float nyq[2][2][2];                               // [tile][frame][column half]: partial Nyquist sums
+    uint64_t bar[4];                                  // stage 1 of tile 0 / 1, stage 2 of tile 0 / 1
     uint32_t tmem_base;
 };
 static_assert(sizeof(CrSmem) + 1024 <= 227 * 1024, "shared memory budget");
@@ -100,7 +101,7 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
         sincospi((double)(a * kb) / 2048.0, &sn, &cs);
         sm.tw[kb * CR_TWP + a] = make_float2((float)cs, (float)-sn);
     }
-    if (tid == 0) { mbar_init(smem_u32(&sm.bar[0]), 1); mbar_init(smem_u32(&sm.bar[1]), 1); fence_mbar_init(); }
+    if (tid == 0) { for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&sm.bar[i]), 1); fence_mbar_init(); }
     if (warp == 0) { tmem_alloc<1>(smem_u32(&sm.tmem_base), 512); tmem_relinquish<1>(); }
     fence_proxy_async();
     tc_fence_before();
@@ -133,8 +134,8 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
     // rows a sits at row rho(a) = a / 2 + 32 (a & 1), so the two rows are lane and lane + 32 (2-way instead of 4-way
     // bank conflicts); epilogue 1 undoes the permutation for free when it picks TMEM columns.  K bytes 8 warp .. + 7.
     const uint32_t fir_off = lane * 128 + ((((uint32_t)warp >> 1) ^ (lane & 7)) << 4) + 8 * (warp & 1);
-    // epilogue roles: TMEM lane quarter, tile, column half
-    const int eq = warp & 3, et = (warp >> 2) & 1, eh = warp >> 3;
+    // epilogue roles: TMEM lane quarter; epilogue 1: frame of the tile and column half; epilogue 2: ka block
+    const int eq = warp & 3, q4 = warp >> 2, eh = q4 >> 1, ch = q4 & 1;
     // the NR = WA - 1 + CR_FR samples of input columns (2 lane, 2 lane + 1) + 64 (4 warp + bi) that group gg needs; rows
     // outside the stream read as zero (the first groups when M < WA and the last group of a stream take that path)
     auto load_col = [&](int gg, int bi, float2 (&row)[NR]) {
@@ -202,6 +203,9 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
         }
         fence_proxy_async();
         __syncthreads();
+        // The two tiles of a group are pipelined against the tensor pipe: ALL warps run epilogue 1 of tile 0 while the
+        // stage-1 MMAs of tile 1 execute, epilogue 1 of tile 1 while the stage-2 MMAs of tile 0 execute, epilogue 2 of
+        // tile 0 while the stage-2 MMAs of tile 1 execute; only the stage-1 MMAs of tile 0 are waited for in full.
         // ---- stage 1 (transposed): D1^T[t] = B1 * A1[t]^T -> TMEM columns 128 t .. 128 t + 127 = (frame, a)
         if (tid == 0) {
             tc_fence_after();
@@ -213,56 +217,55 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
                 for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 128 * t, d_bl + 2 * k, d_a + t * TILE + 2 * k, idesc1, 1);
 #pragma unroll
                 for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 128 * t, d_bh + 2 * k, d_a + t * TILE + 2 * k, idesc1, 1);
+                umma_commit(smem_u32(&sm.bar[t]));
             }
-            umma_commit(smem_u32(&sm.bar[0]));
         }
-        mbar_wait(smem_u32(&sm.bar[0]), it & 1u);
-        tc_fence_after();
-        // ---- epilogue 1: warp (eq, et, eh) reads TMEM lanes 32 eq .. + 31 = (kb = 16 eq + lane / 2, c = lane & 1) and the
-        //      64 columns a = 0 .. 63 of frame 2 et + eh; the partner lane (lane ^ 1) holds the other part of G[a][kb].
-        //      G' = G * w:  Re = Gr wr - Gi wi,  Im = Gi wr + Gr wi  ->  own * wr + partner * (c ? wi : -wi).
-        {
-            const int kb = 16 * eq + (lane >> 1), c = lane & 1;
-            const float sgn = c ? 1.f : -1.f;
-            const long long f = f0 + 2 * et + eh;
-            const uint32_t row = eh * 64 + kb;
-            uint8_t* const blk = &sm.a[et][c][0][0];
-            const float4* twr = reinterpret_cast<const float4*>(sm.tw + kb * CR_TWP);
-            // TMEM column rho of this frame holds a = 2 rho (rho < 32) or 2 (rho - 32) + 1: even a in ve, odd a in vo
-            // TMEM column rho of this frame holds a = 2 rho (rho < 32) or 2 (rho - 32) + 1: even a in ve, odd a in vo
-            uint32_t ve[32], vo[32];
-            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 * eh, ve);
-            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 * eh + 32, vo);
-            tmem_ld_wait();
-            float nyq = 0.f;
 #pragma unroll
-            for (int j8 = 0; j8 < 8; ++j8) {                               // a = 8 j8 .. 8 j8 + 7
-                uint32_t hw[4], lw[4];
-#pragma unroll
-                for (int i2 = 0; i2 < 4; ++i2) {
-                    const int i = 4 * j8 + i2;                             // a = 2 i, 2 i + 1
-                    const float4 w = twr[i];
-                    const float v0 = __uint_as_float(ve[i]), v1 = __uint_as_float(vo[i]);
-                    const float p0 = __shfl_xor_sync(0xffffffffu, v0, 1), p1 = __shfl_xor_sync(0xffffffffu, v1, 1);
-                    nyq += v0 - v1;
-                    const float o0 = fmaf(p0, sgn * w.y, v0 * w.x), o1 = fmaf(p1, sgn * w.w, v1 * w.z);
-                    cr_split(o0, o1, hw[i2], lw[i2]);
-                }
-                const uint32_t off = cr_sw128(row, 16 * j8);
-                *reinterpret_cast<uint4*>(blk + off) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
-                *reinterpret_cast<uint4*>(blk + CR_TILE + off) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
-            }
-            // k = 2048: X = sum_a (-1)^a G[a][0] (real; the lane holding (kb = 0, re) has all 64 terms)
-            if (eq == 0 && lane == 0 && f < F) out[((long long)s * F + f) * CR_NK + CR_P / 2] = make_float2(nyq, 0.f);
-        }
-        fence_proxy_async();
-        tc_fence_before();
-        __syncthreads();
-        // ---- stage 2: D_R[t] = Re(G')[t] * B1[0..63]^T -> columns 128 t .. + 63,  D_I[t] = Im(G')[t] * B1[0..63]^T -> + 64 .. + 127
-        if (tid == 0) {
+        for (int t = 0; t < 2; ++t) {
+            mbar_wait(smem_u32(&sm.bar[t]), it & 1u);
             tc_fence_after();
+            // ---- epilogue 1 of tile t: warp (eq, eh, ch) reads TMEM lanes 32 eq .. + 31 = (kb = 16 eq + lane / 2,
+            //      c = lane & 1) and the columns a = 32 ch .. 32 ch + 31 of frame 2 t + eh; the partner lane (lane ^ 1)
+            //      holds the other part of G[a][kb].  G' = G * w:  Re = Gr wr - Gi wi,  Im = Gi wr + Gr wi  ->
+            //      own * wr + partner * (c ? wi : -wi).
+            {
+                const int kb = 16 * eq + (lane >> 1), c = lane & 1;
+                const float sgn = c ? 1.f : -1.f;
+                const uint32_t row = eh * 64 + kb;
+                uint8_t* const blk = &sm.a[t][c][0][0];
+                const float4* twr = reinterpret_cast<const float4*>(sm.tw + kb * CR_TWP) + 16 * ch;
+                // TMEM column rho of this frame holds a = 2 rho (rho < 32) or 2 (rho - 32) + 1: even a in ve, odd a in vo
+                uint32_t ve[16], vo[16];
+                tmem_ld16(tmem + ((uint32_t)(eq * 32) << 16) + 128 * t + 64 * eh + 16 * ch, ve);
+                tmem_ld16(tmem + ((uint32_t)(eq * 32) << 16) + 128 * t + 64 * eh + 32 + 16 * ch, vo);
+                tmem_ld_wait();
+                float nyq = 0.f;
 #pragma unroll
-            for (int t = 0; t < 2; ++t)
+                for (int j4 = 0; j4 < 4; ++j4) {                           // a = 8 j8 .. 8 j8 + 7, j8 = 4 ch + j4
+                    uint32_t hw[4], lw[4];
+#pragma unroll
+                    for (int i2 = 0; i2 < 4; ++i2) {
+                        const int i = 4 * j4 + i2;                         // a = 32 ch + 2 i, + 1
+                        const float4 w = twr[i];
+                        const float v0 = __uint_as_float(ve[i]), v1 = __uint_as_float(vo[i]);
+                        const float p0 = __shfl_xor_sync(0xffffffffu, v0, 1), p1 = __shfl_xor_sync(0xffffffffu, v1, 1);
+                        nyq += v0 - v1;
+                        const float o0 = fmaf(p0, sgn * w.y, v0 * w.x), o1 = fmaf(p1, sgn * w.w, v1 * w.z);
+                        cr_split(o0, o1, hw[i2], lw[i2]);
+                    }
+                    const uint32_t off = cr_sw128(row, 16 * (4 * ch + j4));
+                    *reinterpret_cast<uint4*>(blk + off) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+                    *reinterpret_cast<uint4*>(blk + CR_TILE + off) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+                }
+                // k = 2048: X = sum_a (-1)^a G[a][0] (real; the lanes holding (kb = 0, re) have 32 terms each)
+                if (eq == 0 && lane == 0) sm.nyq[t][eh][ch] = nyq;
+            }
+            fence_proxy_async();
+            tc_fence_before();
+            __syncthreads();
+            // ---- stage 2 of tile t: D_R = Re(G') * B1[0..63]^T -> columns 128 t .. + 63,  D_I = Im(G') * B1[0..63]^T -> + 64 .. + 127
+            if (tid == 0) {
+                tc_fence_after();
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     const uint64_t da = d_a + t * TILE + c * BLOCK;
@@ -274,23 +277,29 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
 #pragma unroll
                     for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bl + 2 * k, idesc2, 1);
                 }
-            umma_commit(smem_u32(&sm.bar[1]));
+                umma_commit(smem_u32(&sm.bar[2 + t]));
+            }
+            if (tid < 2) {                                                 // Nyquist bins of the tile's two frames
+                const long long f = f0 + 2 * t + tid;
+                if (f < F) out[((long long)s * F + f) * CR_NK + CR_P / 2] = make_float2(sm.nyq[t][tid][0] + sm.nyq[t][tid][1], 0.f);
+            }
         }
-        mbar_wait(smem_u32(&sm.bar[1]), it & 1u);
-        tc_fence_after();
-        // ---- epilogue 2: warp (eq, et, eh) reads rows 32 eq .. + 31 = (frame 2 et + eq / 2, kb = 32 (eq & 1) + lane) and
-        //      ka = 16 eh .. 16 eh + 15.  D_R = (C_r, -S_r), D_I = (C_i, -S_i):  X = (C_r + S_i, C_i - S_r).
+        // ---- epilogue 2: warp (eq, q4) reads rows 32 eq .. + 31 = (frame 2 t + eq / 2, kb = 32 (eq & 1) + lane) and
+        //      ka = 8 q4 .. 8 q4 + 7.  D_R = (C_r, -S_r), D_I = (C_i, -S_i):  X = (C_r + S_i, C_i - S_r).
         //      For a fixed ka the 32 lanes hold 32 consecutive channels: 256 contiguous bytes per warp store.
-        {
-            const long long f = f0 + 2 * et + (eq >> 1);
-            float2* const orow = out + ((long long)s * F + f) * CR_NK + 32 * (eq & 1) + lane + 64 * 16 * eh;
-            uint32_t vr[32], vi[32];
-            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 32 * eh, vr);
-            tmem_ld32(tmem + ((uint32_t)(eq * 32) << 16) + 128 * et + 64 + 32 * eh, vi);
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            mbar_wait(smem_u32(&sm.bar[2 + t]), it & 1u);
+            tc_fence_after();
+            const long long f = f0 + 2 * t + (eq >> 1);
+            float2* const orow = out + ((long long)s * F + f) * CR_NK + 32 * (eq & 1) + lane + 64 * 8 * q4;
+            uint32_t vr[16], vi[16];
+            tmem_ld16(tmem + ((uint32_t)(eq * 32) << 16) + 128 * t + 16 * q4, vr);
+            tmem_ld16(tmem + ((uint32_t)(eq * 32) << 16) + 128 * t + 64 + 16 * q4, vi);
             tmem_ld_wait();
             if (f < F) {
 #pragma unroll
-                for (int i = 0; i < 16; ++i)
+                for (int i = 0; i < 8; ++i)
                     orow[64 * i] = make_float2(__uint_as_float(vr[2 * i]) - __uint_as_float(vi[2 * i + 1]),
                                                __uint_as_float(vr[2 * i + 1]) + __uint_as_float(vi[2 * i]));
             }
