@@ -152,8 +152,8 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
     };
     // Loads run one column ahead of the FMAs: column bi + 1 is requested before column bi is computed, and column 0 of
     // the NEXT group right after this group's subfilter stage, so it is in flight during the MMA waits and epilogues.
-    float2 pre[NR];
-    if ((int)blockIdx.x < total_groups) load_col(blockIdx.x, 0, pre);
+    float2 pre[NR], pre1[NR];
+    if ((int)blockIdx.x < total_groups) { load_col(blockIdx.x, 0, pre); load_col(blockIdx.x, 1, pre1); }
     uint32_t it = 0;
     for (int g = blockIdx.x; g < total_groups; g += gridDim.x, ++it) {
         const int s = g / groups_per_stream;
@@ -164,12 +164,14 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
             uint32_t hprev[CR_FR], lprev[CR_FR];
             float2 rows[2][NR];
 #pragma unroll
-            for (int j = 0; j < NR; ++j) rows[0][j] = pre[j];
+            for (int j = 0; j < NR; ++j) { rows[0][j] = pre[j]; rows[1][j] = pre1[j]; }
 #pragma unroll
             for (int bi = 0; bi < CR_BPW; ++bi) {
                 uint32_t tv[16];
                 tmem_ld16(tap_addr + bi * 16, tv);
-                if (bi + 1 < CR_BPW) load_col(g, bi + 1, rows[(bi + 1) & 1]);
+                // columns 0 and 1 were requested during the previous group's epilogues; column bi + 1 >= 2 goes into the
+                // buffer that column bi - 1 has just left
+                if (bi >= 1 && bi + 1 < CR_BPW) load_col(g, bi + 1, rows[(bi + 1) & 1]);
                 float2 (&row)[NR] = rows[bi & 1];
                 tmem_ld_wait();
 #pragma unroll
@@ -191,7 +193,7 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
                     }
                 }
             }
-            if (g + (int)gridDim.x < total_groups) load_col(g + (int)gridDim.x, 0, pre);
+            if (g + (int)gridDim.x < total_groups) { load_col(g + (int)gridDim.x, 0, pre); load_col(g + (int)gridDim.x, 1, pre1); }
 #pragma unroll
             for (int fl = 0; fl < CR_FR; ++fl) {
                 uint8_t* const dst = &sm.a[fl >> 1][0][0][0] + (fl & 1) * 64 * 128 + fir_off;
