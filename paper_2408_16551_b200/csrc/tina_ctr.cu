@@ -193,7 +193,23 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
                     }
                 }
             }
-            if (g + (int)gridDim.x < total_groups) { load_col(g + (int)gridDim.x, 0, pre); load_col(g + (int)gridDim.x, 1, pre1); }
+            if (g + (int)gridDim.x < total_groups) {
+                load_col(g + (int)gridDim.x, 0, pre);
+                load_col(g + (int)gridDim.x, 1, pre1);
+                // columns 2 and 3 of the next group: pulled into L2 now, loaded into registers inside its subfilter stage
+                const int gn = g + (int)gridDim.x;
+                const long long r0 = (long long)(gn % groups_per_stream) * CR_FR + M - WA;
+                if (r0 >= 0 && r0 + NR <= NBLK) {
+                    const float* xg = x + (long long)(gn / groups_per_stream) * stream_stride + r0 * CR_P + 2 * lane + 64 * (CR_BPW * warp + 2);
+                    if ((lane & 15) == 0) {
+#pragma unroll
+                        for (int j = 0; j < NR; ++j) {
+                            asm volatile("prefetch.global.L2 [%0];" :: "l"(xg + j * CR_P));
+                            asm volatile("prefetch.global.L2 [%0];" :: "l"(xg + j * CR_P + 64));
+                        }
+                    }
+                }
+            }
 #pragma unroll
             for (int fl = 0; fl < CR_FR; ++fl) {
                 uint8_t* const dst = &sm.a[fl >> 1][0][0][0] + (fl & 1) * 64 * 128 + fir_off;
