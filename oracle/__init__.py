@@ -47,6 +47,8 @@ def _load():
     ll, vp, ci = ctypes.c_longlong, ctypes.c_void_p, ctypes.c_int
     lib.oracle_fir.argtypes = [vp, vp, vp, ll, ll, ll]
     lib.oracle_fir.restype = ci
+    lib.oracle_fir_multi.argtypes = [vp, vp, vp, ll, ll, ll]
+    lib.oracle_fir_multi.restype = ci
     lib.oracle_unfold.argtypes = [vp, vp, ll, ll]
     lib.oracle_unfold.restype = ci
     lib.oracle_dft.argtypes = [vp, vp, ll, ll, ci]
@@ -96,6 +98,22 @@ def fir(x, taps) -> np.ndarray:
     if rc:
         raise ValueError(f"oracle_fir rc={rc}")
     return y[0] if one_d else y
+
+
+def fir_multi(x, taps) -> np.ndarray:
+    """Eq. (15) with per-channel taps ("multiple FIR filters").
+    x: [C, L] float32, taps: [C, K] float32 -> float64 [C, L-K+1]."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    taps = np.ascontiguousarray(taps, dtype=np.float32)
+    if x.ndim != 2 or taps.ndim != 2 or taps.shape[0] != x.shape[0]:
+        raise ValueError("need x [C, L] and taps [C, K]")
+    C, L = x.shape
+    K = taps.shape[1]
+    y = np.empty((C, L - K + 1), dtype=np.float64)
+    rc = _load().oracle_fir_multi(_ptr(x), _ptr(taps), _ptr(y), C, L, K)
+    if rc:
+        raise ValueError(f"oracle_fir_multi rc={rc}")
+    return y
 
 
 def unfold(x, J: int) -> np.ndarray:

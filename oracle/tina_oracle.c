@@ -77,6 +77,29 @@ int oracle_fir(const float *x, const float *a, double *y,
     return 0;
 }
 
+/* Eq. (15), with one tap vector PER CHANNEL -- the "multiple FIR filters"
+ * that the PFB's subfilter stage combines (Eq. (20): branch p is
+ * filtered with its own h_p).  Valid mode as above:
+ *   y[c][j] = sum_{k=0}^{K-1} a[c][k] * x[c][j + K-1 - k],  j in [0, L-K+1).
+ * x: [C][L] float32, a: [C][K] float32, y: [C][L-K+1] float64.              */
+int oracle_fir_multi(const float *x, const float *a, double *y,
+                     long long C, long long L, long long K)
+{
+    if (!x || !a || !y || C < 1 || K < 1 || L < K) return 1;
+    const long long Lo = L - K + 1;
+    long long c;
+#pragma omp parallel for schedule(static)
+    for (c = 0; c < C; ++c) {
+        for (long long j = 0; j < Lo; ++j) {
+            double acc = 0.0;
+            for (long long k = 0; k < K; ++k)
+                acc += (double)a[c * K + k] * (double)x[c * L + (j + K - 1 - k)];
+            y[c * Lo + j] = acc;
+        }
+    }
+    return 0;
+}
+
 /* Eq. (17): Y(i,j) = X(i+j), output (I-J+1) x J.               */
 int oracle_unfold(const float *x, double *y, long long I, long long J)
 {

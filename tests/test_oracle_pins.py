@@ -71,6 +71,34 @@ def test_fir_single_tap_and_shared_taps(oracle):
         assert np.array_equal(y[c], oracle.fir(x[c], a))
 
 
+def test_fir_multi_per_channel_taps(oracle):
+    """Per-channel taps (PAPER.md:233 'multiple FIR filters'; Eq. (15) per channel).  Pins that do
+    not re-type the formula: (i) channel c's impulse response is ITS tap row, in order; (ii) each
+    channel equals numpy.convolve with its own taps; (iii) rows of taps are not mixed up: a channel
+    whose taps are all zero gives zeros; (iv) the PFB subfilter stage (Eq. (20)) is ONE fir_multi
+    call over the P branches with taps w[p::P] (the statement of PAPER.md:233)."""
+    rng = np.random.default_rng(31)
+    C, K, L = 5, 7, 90
+    a = rng.standard_normal((C, K)).astype(np.float32)
+    a[3] = 0.0
+    x = np.zeros((C, 2 * K - 1), np.float32)
+    x[:, K - 1] = 1.0
+    assert np.array_equal(oracle.fir_multi(x, a), a.astype(np.float64))
+    x = ti.noise_real(rng, C * L).reshape(C, L)
+    y = oracle.fir_multi(x, a)
+    assert y.shape == (C, L - K + 1)
+    for c in range(C):
+        assert np.allclose(y[c], np.convolve(x[c].astype(np.float64), a[c].astype(np.float64), "valid"),
+                           rtol=0, atol=1e-12)
+    assert np.array_equal(y[3], np.zeros(L - K + 1))
+    P, M, F = 8, 3, 11
+    c4 = _small_case(P, M, F, real=True, seed=12)
+    _, ysub = oracle.pfb(c4.x[0], P, M, c4.window, return_subfiltered=True)
+    branches = np.ascontiguousarray(c4.x[0][: (F + M - 1) * P].reshape(F + M - 1, P).T)   # [P][NB]
+    taps = np.ascontiguousarray(c4.window.reshape(M, P).T)                                # [P][M] = w[p::P]
+    assert np.allclose(oracle.fir_multi(branches, taps).T, ysub, rtol=0, atol=1e-12)
+
+
 # ---------------------------------------------------------------- DFT / IDFT
 def test_dft4_textbook_golden(oracle):
     rows = _rows(os.path.join(GOLDEN, "dft4_textbook.txt"))
