@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- headline benchmark of libtina: fused PFB at P=1024, M=16 (BASELINE.json config 4).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4|c5|c5bf16|c2|c3|c1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload c4|c5|c5bf16|c5fp16|c2|c3|c3multi|c1|c4fir|c4fft|c5fft|peaks]
 
 One "step" = one pass of the whole hot path (subfilter stage + DFT contraction, one
 tina_pfb_batched call) over one batch of synthetic input shaped like config 4:
@@ -66,6 +67,10 @@ def workload_spec(name: str):
         return dict(call="dft", B=65536, N=256)
     if name == "c3":
         return dict(call="fir", C=64, L=1 << 20, K=64)
+    if name == "c3multi":   # config-3 shape with one tap vector per channel (tina_fir_multi)
+        return dict(call="fir_multi", C=64, L=1 << 20, K=64)
+    if name == "peaks":     # measured arithmetic ceilings (tina_probe_peak), no workload
+        return dict(call="peaks")
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -157,7 +162,7 @@ def make_inputs(w, seed_offset: int = 0):
         return case
     if w["call"] == "dft":
         return ti.config2(w["B"], w["N"])
-    return ti.config3(w["C"], w["L"], w["K"])
+    return ti.config3(w["C"], w["L"], w["K"])   # fir and fir_multi
 
 
 def cpu_oracle_rate(w, budget_s: float = 15.0):
@@ -183,8 +188,78 @@ def cpu_oracle_rate(w, budget_s: float = 15.0):
         return n * N / dt / 1e9, cores, f"{n} signals of N={N}", dt
     C, L, K = 8, 1 << 20, w["K"]
     x, taps, _ = ti.config3(C, L, K)
+    if w["call"] == "fir_multi":
+        tm = np.ascontiguousarray(np.tile(taps, (C, 1)))
+        t0 = time.perf_counter(); oracle.fir_multi(x, tm); dt = time.perf_counter() - t0
+        return C * L / dt / 1e9, cores, f"{C} channels of L={L}, K={K}, per-channel taps", dt
     t0 = time.perf_counter(); oracle.fir(x, taps); dt = time.perf_counter() - t0
     return C * L / dt / 1e9, cores, f"{C} channels of L={L}, K={K}", dt
+
+
+def cpu_numpy_rate(w, repeats: int = 5, budget_s: float = 25.0):
+    """The NumPy-style vectorised CPU PFB of oracle/numpy_pfb.py (the stand-in for the paper's "naive
+    implementation written in NumPy (on CPU)"; protocol PAPER.md:208, :214: data resident,
+    best of `repeats`), complex64 / float32, numpy.fft for the Fourier stage.  c4 is timed as ONE stream
+    (the eight streams are independent and identical in cost; the rate is per sample, so no scaling is
+    needed).  Returns a dict, or None for workloads it does not define (FIR)."""
+    from oracle import numpy_pfb
+    if w["call"] == "dft":
+        x = ti.config2(min(w["B"], 16384), w["N"])
+        fn, n_samp, sample = (lambda: np.fft.ifft(np.fft.fft(x, axis=1), axis=1).astype(np.complex64)), x.size, \
+            f"{x.shape[0]} signals of N={w['N']}, numpy.fft forward + inverse"
+    elif w["call"] in ("pfb", "pfb_fft", "pfb_fir"):
+        P, M, F = w["P"], w["M"], w["F"]
+        case = ti.pfb_case(P, M, F, real=w["real"], streams=1, seed=3)
+        x, win = case.x[0], case.window
+        if w["call"] == "pfb_fir":
+            fn = lambda: numpy_pfb.pfb_subfilter(x, P, M, win)
+        else:
+            fn = lambda: numpy_pfb.pfb(x, P, M, win)
+        n_samp, sample = x.size, f"one stream of {F} frames (P={P}, M={M}), complex64/float32, numpy.fft"
+    else:
+        return None
+    best, t_all = None, time.perf_counter()
+    for i in range(repeats):
+        t0 = time.perf_counter(); fn(); dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+        if time.perf_counter() - t_all > budget_s:
+            break
+    try:
+        from threadpoolctl import threadpool_info
+        blas_threads = max([d.get("num_threads", 1) for d in threadpool_info()] or [1])
+    except Exception:
+        blas_threads = None
+    return {"value": n_samp / best / 1e9, "unit": UNIT, "kind": "numpy", "cores": 1,
+            "host_cores": len(os.sched_getaffinity(0)), "blas_threads": blas_threads,
+            "numpy": np.__version__, "best_of": i + 1, "seconds": best, "sample": sample,
+            "note": "numpy.fft (pocketfft) and the slice multiply-accumulates run on one thread"}
+
+
+def tina_env():
+    """Every TINA_* variable set in the environment (recorded in the JSON line)."""
+    return {k: v for k, v in sorted(os.environ.items()) if k.startswith("TINA_")}
+
+
+REFUSED_ENV = ("TINA_DEBUG_SKIP", "TINA_KSPLIT", "TINA_A_SLOTS", "TINA_B_ENTRIES", "TINA_CL4", "TINA_PROF", "TINA_BUILD_DEV")
+
+
+def run_peaks(args):
+    """--workload peaks: bare-loop ceilings of this device (burst = ~20 ms region, sustained = ~2 s)."""
+    import torch
+    import paper_2408_16551_b200 as tina
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    names = {0: "ffma_fp32", 1: "ffma2_fp32", 2: "tcgen05_tf32", 3: "tcgen05_bf16"}
+    out = {}
+    for which, name in names.items():
+        base = 4096 if which < 2 else 2048
+        tf, ms = tina.probe_peak(which, base)
+        per_ms = base / ms
+        burst = max(tina.probe_peak(which, int(per_ms * 20))[0] for _ in range(5))
+        sampler = ClockSampler(0); sampler.start(); time.sleep(0.1); t0 = time.time()
+        sus, sus_ms = tina.probe_peak(which, int(per_ms * 2000))
+        clocks = sampler.stop(t0, time.time())
+        out[name] = {"burst_tflops": burst, "sustained_tflops": sus, "sustained_ms": sus_ms, "clocks": clocks}
+    print(json.dumps({"metric": "measured_peaks", "peaks": out, "measured_peaks_json": load_peaks()}), flush=True)
 
 
 def run_reference(args, w):
@@ -212,6 +287,9 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+L2_BYTES = 126e6
+
+
 def run_ours(args, w):
     import torch
     import torch.distributed as dist
@@ -223,11 +301,17 @@ def run_ours(args, w):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- libtina has no CPU fallback")
+    env = tina_env()
+    refused = [k for k in REFUSED_ENV if k in os.environ]
+    tina.lib()
+    if refused or tina.build_is_dev():
+        # knobs that skip work or change the accuracy contract: a number measured with them is not a measurement
+        print(f"bench.py: refusing to run with {refused or 'a -DTINA_DEV build of libtina.so'}", file=sys.stderr)
+        raise SystemExit(2)
     torch.cuda.set_device(local_rank)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    tina.lib()
 
     flops, byts, samples, frames = useful_flops_and_bytes(w)
     peaks = load_peaks()
@@ -236,63 +320,94 @@ def run_ours(args, w):
     # ---- inputs resident in HBM (each rank its own seeded batch: frames are independent, so
     #      ranks shard the units with no data-path collective -> weak scaling) --------------
     data = make_inputs(w, seed_offset=rank)
-    if w["call"] == "pfb":
-        x_host = torch.from_numpy(data.x)
-        w_host = torch.from_numpy(data.window)
-        xd, wd = x_host.cuda(), w_host.cuda()
-        NK = w["P"] // 2 + 1 if w["real"] else w["P"]
-        out = torch.empty((w["S"], w["F"], NK), dtype=torch.complex64, device="cuda")
-        step = lambda: tina.pfb(xd, w["P"], w["M"], wd, prec=w["prec"], out=out)
-    elif w["call"] == "pfb_fft":
-        xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()
-        out = torch.empty((w["S"], w["F"], w["P"] // 2 + 1 if w["real"] else w["P"]), dtype=torch.complex64, device="cuda")
-        step = lambda: tina.pfb_fft(xd, w["P"], w["M"], wd, out=out)
-    elif w["call"] == "pfb_fir":
-        xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()
-        out = torch.empty((w["S"], w["F"], w["P"]), dtype=xd.dtype, device="cuda")
-        step = lambda: tina.pfb_fir(xd, w["P"], w["M"], wd, out=out)
-    elif w["call"] == "dft":
-        xd = torch.from_numpy(data).cuda()
-        out = torch.empty_like(xd); back = torch.empty_like(xd)
-        def step():
-            tina.dft(xd, out=out); tina.dft(out, inverse=True, out=back)
-        flops *= 2; byts *= 2
-    else:
+    x_host = w_host = None
+    NK = None
+
+    def make_set():
+        """One set of device buffers + the step that runs on them."""
+        nonlocal x_host, w_host, NK
+        if w["call"] == "pfb":
+            x_host, w_host = torch.from_numpy(data.x), torch.from_numpy(data.window)
+            xd, wd = x_host.cuda(), w_host.cuda()
+            NK = w["P"] // 2 + 1 if w["real"] else w["P"]
+            out = torch.empty((w["S"], w["F"], NK), dtype=torch.complex64, device="cuda")
+            return lambda: tina.pfb(xd, w["P"], w["M"], wd, prec=w["prec"], out=out)
+        if w["call"] == "pfb_fft":
+            xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()
+            out = torch.empty((w["S"], w["F"], w["P"] // 2 + 1 if w["real"] else w["P"]), dtype=torch.complex64, device="cuda")
+            return lambda: tina.pfb_fft(xd, w["P"], w["M"], wd, out=out)
+        if w["call"] == "pfb_fir":
+            xd, wd = torch.from_numpy(data.x).cuda(), torch.from_numpy(data.window).cuda()
+            out = torch.empty((w["S"], w["F"], w["P"]), dtype=xd.dtype, device="cuda")
+            return lambda: tina.pfb_fir(xd, w["P"], w["M"], wd, out=out)
+        if w["call"] == "dft":
+            xd = torch.from_numpy(data).cuda()
+            out = torch.empty_like(xd); back = torch.empty_like(xd)
+            def step():
+                tina.dft(xd, out=out); tina.dft(out, inverse=True, out=back)
+            return step
         xh, taps, _ = data
-        xd, td = torch.from_numpy(xh).cuda(), torch.from_numpy(taps).cuda()
+        xd = torch.from_numpy(xh).cuda()
         out = torch.empty((w["C"], w["L"] - w["K"] + 1), dtype=torch.float32, device="cuda")
-        step = lambda: tina.fir(xd, td, out=out)
+        if w["call"] == "fir_multi":
+            td = torch.from_numpy(np.ascontiguousarray(np.tile(taps, (w["C"], 1)))).cuda()
+            return lambda: tina.fir_multi(xd, td, out=out)
+        td = torch.from_numpy(taps).cuda()
+        return lambda: tina.fir(xd, td, out=out)
+
+    if w["call"] == "dft":
+        flops *= 2; byts *= 2
+    # Working sets smaller than ~8x L2 are timed twice: HOT (the same buffers every step) and COLD (rotating
+    # over >= 4 distinct buffer sets totalling > 2x L2, so no step finds its data in L2).  HBM fractions and
+    # `value` are quoted from the cold run (SURVEY.md section 8(d), PAPER.md:208, :214).
+    set_bytes = 3 * 8.0 * w["B"] * w["N"] if w["call"] == "dft" else byts      # dft: x, out and back buffers
+    rotate = set_bytes < 8 * L2_BYTES
+    n_sets = int(min(512, max(4, np.ceil(2.5 * L2_BYTES / set_bytes)))) if rotate else 1
+    steps_of = [make_set() for _ in range(n_sets)]
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
+    def timed(n_steps, pick):
+        """CUDA events on the launching stream: whole region + every step."""
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.time()
+        e0.record(stream)
+        for i, (a, b) in enumerate(evs):
+            a.record(stream); pick(i)(); b.record(stream)
+        e1.record(stream)
+        barrier()
+        t1 = time.time()
+        per = [a.elapsed_time(b) for a, b in evs]
+        return e0.elapsed_time(e1), per, t0, t1
+
+    n_warm = max(args.warmup, 3)
+    for i in range(max(n_warm, n_sets)):
+        steps_of[i % n_sets]()
     barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
         time.sleep(0.15)
     launches0 = tina.launch_count()
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    t_wall0 = time.time()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for a, b in evs:
-        a.record(stream); step(); b.record(stream)
-    e1.record(stream)
-    barrier()
-    t_wall1 = time.time()
+    total_ms, per_step, t_wall0, t_wall1 = timed(args.steps, lambda i: steps_of[i % n_sets])
     launches = tina.launch_count() - launches0
-    total_ms = e0.elapsed_time(e1)
-    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    kern_ms, kern_min = float(np.mean(per_step)), float(np.min(per_step))
     total_ms = shard.max_over_ranks(total_ms, device="cuda")
     ms_per_step = total_ms / args.steps
     value = world * samples / (ms_per_step * 1e-3) / 1e9
-    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    hot = None
+    if rotate:
+        h_total, h_per, _, _ = timed(args.steps, lambda i: steps_of[0])
+        hot = {"ms_per_step": h_total / args.steps, "ms_mean": float(np.mean(h_per)), "ms_min": float(np.min(h_per)),
+               "value": world * samples / (h_total / args.steps * 1e-3) / 1e9}
+    issued_ratio = tina.last_issued_ratio() if hasattr(tina, "last_issued_ratio") else None
+    variant = tina.last_kernel() if hasattr(tina, "last_kernel") else None
 
     # ---- e2e: host buffers through the C ABI (H2D + kernel + D2H inside the timed region) --
     e2e = None
@@ -323,39 +438,61 @@ def run_ours(args, w):
     if os.path.exists(tpath):
         with open(tpath) as fh:
             traffic = json.load(fh).get(args.workload)
-    # the peak to compare with: the burst figure for a short, unthrottled region; the sustained one when
-    # the region is long or the power cap was active during it (clocks well below max)
+    # Which measured peak applies: the burst figure for a short, unthrottled region; the sustained one when the
+    # region is long or the power cap was active during it.  BOTH fractions are printed every time.
     throttled = bool(clocks) and ("sw_power_cap" in clocks.get("reasons", []) or
                                   (clocks.get("sm_mhz") and clocks.get("sm_max_mhz") and clocks["sm_mhz"] < 0.85 * clocks["sm_max_mhz"]))
     sustained = total_ms > 1500.0 or throttled
     if tensor_bound:
-        peak = peaks["bf16_tflops_sustained" if sustained else "bf16_tflops"]
+        pk_b, pk_s = peaks["bf16_tflops"], peaks["bf16_tflops_sustained"]
+        peak = pk_s if sustained else pk_b
         achieved = flops / (kern_ms * 1e-3) / 1e12
         passes = 3 if w.get("prec", 0) == 0 else 1
+        # issued tensor flops per useful flop: `passes` bf16 products per useful one (error-compensated bf16x3),
+        # times the fraction of the Fourier matrix the kernel contracts against (0.5 when every distinct column
+        # pair k / P-k is contracted once; reported by the library for the kernel that ran)
+        ratio = passes * (issued_ratio if issued_ratio else 1.0)
         roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_source": f"{peaks['_source']} bf16 {'sustained' if sustained else 'burst'}",
-                "issued_passes": passes, "issued_frac": passes * achieved / peak,
+                "useful_flops": flops, "issued_flops": flops * ratio, "issued_passes": passes,
+                "issued_per_useful": ratio, "frac_useful_ceiling": 1.0 / ratio,
+                "frac_useful": achieved / peak, "frac_issued": ratio * achieved / peak, "issued_frac": ratio * achieved / peak,
+                "peak_burst": pk_b, "peak_sustained": pk_s,
+                "frac_useful_burst": achieved / pk_b, "frac_useful_sustained": achieved / pk_s,
+                "frac_issued_burst": ratio * achieved / pk_b, "frac_issued_sustained": ratio * achieved / pk_s,
                 "hbm_gbs_achieved": byts / (kern_ms * 1e-3) / 1e9, "hbm_frac": byts / (kern_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
     else:
         achieved = byts / (kern_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": f"{peaks['_source']} copy"}
+                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": f"{peaks['_source']} copy",
+                "algorithmic_bytes": byts, "frac_nominal_8tbs": achieved / 8000.0}
     roof["kernel_ms"] = kern_ms
+    roof["kernel_ms_min"] = kern_min
+    roof["kernel"] = variant
 
     cpu_val, cores, sample, _ = cpu_oracle_rate(w) if world == 1 else (None, None, None, None)
+    cpu_np = cpu_numpy_rate(w) if world == 1 else None
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": n_warm,
+        "ms_per_step": ms_per_step, "ms_mean": kern_ms, "ms_min": kern_min,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": ("bf16x3->f32" if w.get("prec", 0) == 0 else ("bf16" if w.get("prec", 0) == 1 else "f16")) if (tensor_bound or w["call"] == "pfb_fft") else "f32",
         "data": "synthetic", "spectra_per_s": world * frames / (ms_per_step * 1e-3),
         "config": {"workload": args.workload, **{k: v for k, v in w.items() if k != "call"},
-                   "l2": "inputs and outputs each exceed the 126 MB L2; no explicit flush",
+                   "l2": (f"cold: rotating over {n_sets} distinct buffer sets ({n_sets * set_bytes / 1e6:.0f} MB > 2x L2); the hot "
+                          "(same buffers) timing is in `hot`") if rotate else
+                         "inputs and outputs each exceed the 126 MB L2; no explicit flush",
                    "path": {0: "none", 1: "cuda-core", 2: "tcgen05"}[tina.last_path()],
                    "parallelism": f"frame-sharded replicas x{world}, no collective"},
-        "roofline": roof, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": roof, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "tina_env": env,
     }
+    if hot is not None:
+        line["hot"] = hot
     if cpu_val is not None:
-        line["cpu_baseline"] = {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        line["cpu_baseline"] = {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                "note": "float64 direct sums (the parity oracle): not a performance baseline"}
+    if cpu_np is not None:
+        line["cpu_baseline_numpy"] = cpu_np
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -370,6 +507,8 @@ def main():
     ap.add_argument("--workload", default="c4")
     args = ap.parse_args()
     w = workload_spec(args.workload)
+    if w["call"] == "peaks":
+        return run_peaks(args)
     if args.impl == "reference":
         run_reference(args, w)
     else:

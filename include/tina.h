@@ -13,7 +13,14 @@
  *
  * Errors: integer status only; nothing is written to the outputs on error; no exceptions,
  * no exit(), no CPU fallback, no other backend.  tina_last_error() gives thread-local text.
- * Thread-safety: the plan cache is behind a mutex; everything else is re-entrant.
+ * Thread-safety: the plan cache, the per-device state (SM count, shared-memory opt-ins, scratch) and
+ * the option block are behind mutexes; every device entry point may be called concurrently from
+ * several host threads and on several devices of one process (state is kept per CUDA device; the
+ * current device at call time is the one used).  The `_host` entry point serialises per device.
+ * Environment: TINA_* variant switches (TINA_SHARE, TINA_NT256, TINA_NO_OUT_TMA, TINA_FIR_SIMT,
+ * TINA_CT_NO_WS, TINA_CTR_WS, TINA_NO_SYM) select between kernels that compute the same result under the
+ * same contract; they are read once (tina_reload_options() re-reads them).  Knobs that skip work or
+ * change the accuracy contract exist only in development builds (-DTINA_DEV, tina_build_is_dev()).
  *
  * Notation (0-based everywhere; PAPER.md = /root/reference/PAPER.md):
  *   P  channels / polyphase branches        M  taps per branch
@@ -62,6 +69,17 @@ typedef enum {
 tina_status tina_fir(const float* x, const float* taps, float* y,
                      int C, long long L, int M, void* stream);
 
+/* FIR with one tap vector PER CHANNEL: the "multiple FIR filters" that the PFB's subfilter stage
+ * combines (Eq. (20): branch p is filtered with its own h_p), each
+ * channel being Eq. (15) in valid mode:
+ *     y[c][j] = sum_{k=0}^{M-1} taps[c][k] * x[c][j + M-1 - k],   j in [0, L-M+1)
+ *   x    [C][L]       float32 (device)      taps [C][M] float32, row c = channel c's taps (device)
+ *   y    [C][L-M+1]   float32 (device), must not overlap x
+ * Supported: C >= 1, 1 <= M <= 4096, L >= M; runs on the CUDA-core register-window kernel (fp32 FMA).
+ * Errors as tina_fir.                                                                              */
+tina_status tina_fir_multi(const float* x, const float* taps, float* y,
+                           int C, long long L, int M, void* stream);
+
 /* ---------------------------------------------------------------------------------------
  * DFT / inverse DFT as a dense contraction against the Fourier matrix,
  * Eq. (12) / Eq. (14):
@@ -76,8 +94,9 @@ tina_status tina_dft(const void* x, void* out, long long B, int N, int inverse,
 
 /* ---------------------------------------------------------------------------------------
  * Polyphase filter bank: subfilter stage Eq. (20) followed by a P-point DFT
- * across the branches, fused in one kernel (the subfiltered signals never
- * touch HBM):
+ * across the branches, fused in one kernel for M <= 16 (the subfiltered signals
+ * never touch HBM; for 16 < M <= 64 the subfilter stage runs as its own kernel into a stream-ordered
+ * temporary of S*F*P samples, followed by the contraction -- two launches):
  *     y[f][p] = sum_{m=0}^{M-1} window[m P + p] * x[(f + M-1 - m) P + p]
  *     out[f][k] = sum_{p=0}^{P-1} y[f][p] * exp(-2 pi i p k / P)
  * with x_p(n') = x[n' P + p], h_p(m) = window[m P + p], frame f <-> n' = f + M-1.
@@ -153,12 +172,28 @@ const char* tina_status_string(tina_status s);   /* static storage              
 const char* tina_last_error(void);               /* thread-local detail text, "" if none    */
 tina_status tina_clear_plan_cache(void);         /* frees cached twiddles / staging buffers */
 int         tina_version(void);                  /* major*10000 + minor*100 + patch         */
+tina_status tina_reload_options(void);           /* re-read the TINA_* variant switches     */
+int         tina_build_is_dev(void);             /* 1: built with -DTINA_DEV (debug knobs)  */
+
+/* Measured arithmetic ceilings of the device (bare loops, no memory traffic; the denominators of the
+ * rooflines bench.py reports -- SURVEY.md section 8(d)).  which: 0 = fp32 fma.rn.f32 on the CUDA cores,
+ * 1 = packed fma.rn.f32x2, 2 = tcgen05.mma kind::tf32, 3 = tcgen05.mma kind::f16 with bf16 operands
+ * (M = 128, N = 256 per instruction, operands in shared memory).  Runs `iters` loop iterations per thread
+ * (FMA) or MMA groups per SM (tensor) after a short warm-up, SYNCHRONISES, and returns TFLOP/s in *tflops
+ * and the elapsed milliseconds in *ms (host pointers; ms may be NULL).                                  */
+tina_status tina_probe_peak(int which, int iters, double* tflops, double* ms, void* stream);
 
 /* Introspection used by the tests and bench.py: number of kernel launches the library has
  * enqueued since process start (monotonic), and which path the last device call used
  * (0 = none yet, 1 = generic CUDA-core, 2 = tcgen05 tensor-core).                           */
 long long   tina_launch_count(void);
 int         tina_last_path(void);
+/* Name of the kernel variant the last device call launched (static storage), and the tensor-core flops that
+ * kernel issues PER PASS divided by the method's useful flops (8 P^2 per complex frame, 2 P^2 + 4 P per real
+ * frame): 1.0 for the plain dense contraction, 0.5 where each distinct column pair of the Fourier matrix is
+ * contracted once.  bench.py multiplies it by the number of bf16 passes (3 for TINA_PREC_FP32).          */
+const char* tina_last_kernel(void);
+double      tina_last_issued_ratio(void);
 
 #ifdef __cplusplus
 }

@@ -16,9 +16,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libtina.so")
 _lib = None
 
-EXPORTS = ["tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
+EXPORTS = ["tina_fir", "tina_fir_multi", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
            "tina_pfb_batched_host", "tina_pfb_num_frames", "tina_status_string", "tina_last_error",
-           "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path",
+           "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path", "tina_reload_options", "tina_build_is_dev", "tina_probe_peak", "tina_last_kernel", "tina_last_issued_ratio",
            "tina_mul", "tina_add", "tina_sum", "tina_matmul"]
 
 
@@ -38,6 +38,8 @@ def lib() -> ctypes.CDLL:
     L = ctypes.CDLL(_LIB_PATH)
     ll, vp, ci = ctypes.c_longlong, ctypes.c_void_p, ctypes.c_int
     L.tina_fir.argtypes = [vp, vp, vp, ci, ll, ci, vp]
+    L.tina_fir_multi.argtypes = [vp, vp, vp, ci, ll, ci, vp]
+    L.tina_fir_multi.restype = ci
     L.tina_unfold.argtypes = [vp, vp, ll, ci, vp]
     L.tina_dft.argtypes = [vp, vp, ll, ci, ci, ci, vp]
     L.tina_pfb.argtypes = [vp, ll, ci, ci, vp, ci, ci, vp, vp]
@@ -52,8 +54,13 @@ def lib() -> ctypes.CDLL:
     for f in ("tina_mul", "tina_add", "tina_sum", "tina_matmul"):
         getattr(L, f).restype = ci
     for f in ("tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
-              "tina_pfb_batched_host", "tina_clear_plan_cache", "tina_version", "tina_last_path"):
+              "tina_pfb_batched_host", "tina_clear_plan_cache", "tina_version", "tina_last_path", "tina_reload_options",
+              "tina_build_is_dev"):
         getattr(L, f).restype = ci
+    L.tina_probe_peak.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
+    L.tina_probe_peak.restype = ci
+    L.tina_last_kernel.restype = ctypes.c_char_p
+    L.tina_last_issued_ratio.restype = ctypes.c_double
     L.tina_pfb_num_frames.argtypes = [ll, ci, ci]
     L.tina_pfb_num_frames.restype = ll
     L.tina_launch_count.restype = ll
@@ -88,6 +95,21 @@ def _dev(t, dtype, what):
     return t
 
 
+def _out(out, shape, dtype, device, what="out"):
+    """Allocate the result, or check a caller-supplied one: dtype, device, contiguity AND shape
+    (a too-small buffer would be overrun by the kernels)."""
+    import torch
+    shape = tuple(int(v) for v in shape)
+    if out is None:
+        return torch.empty(shape, dtype=dtype, device=device)
+    _dev(out, dtype, what)
+    if out.device != device:
+        raise ValueError(f"{what}: on {out.device}, inputs on {device}")
+    if tuple(out.shape) != shape:
+        raise ValueError(f"{what}: expected shape {shape}, got {tuple(out.shape)}")
+    return out
+
+
 def pfb_num_frames(n_samples: int, P: int, M: int) -> int:
     return int(lib().tina_pfb_num_frames(n_samples, P, M))
 
@@ -100,8 +122,36 @@ def last_path() -> int:
     return int(lib().tina_last_path())
 
 
+def last_kernel() -> str:
+    return lib().tina_last_kernel().decode()
+
+
+def last_issued_ratio() -> float:
+    return float(lib().tina_last_issued_ratio())
+
+
 def clear_plan_cache() -> None:
     _check(lib().tina_clear_plan_cache())
+
+
+PEAK_FFMA, PEAK_FFMA2, PEAK_TF32, PEAK_BF16 = 0, 1, 2, 3
+
+
+def probe_peak(which: int, iters: int, stream=None):
+    """tina_probe_peak: (TFLOP/s, ms) of a bare FMA / tcgen05.mma loop on the current device."""
+    tf, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(lib().tina_probe_peak(which, iters, ctypes.byref(tf), ctypes.byref(ms), _stream_ptr(stream)))
+    return tf.value, ms.value
+
+
+def reload_options() -> None:
+    """Re-read the TINA_* variant switches from the environment (they are read once otherwise)."""
+    _check(lib().tina_reload_options())
+
+
+def build_is_dev() -> bool:
+    """True if libtina.so was compiled with -DTINA_DEV (work-skipping debug knobs present)."""
+    return bool(lib().tina_build_is_dev())
 
 
 def version() -> int:
@@ -117,10 +167,23 @@ def fir(x, taps, out=None, stream=None):
         raise ValueError("x must be [C, L], taps [M]")
     C, L = x.shape
     M = taps.shape[0]
-    if out is None:
-        out = torch.empty((C, max(L - M + 1, 0)), dtype=torch.float32, device=x.device)
-    _dev(out, torch.float32, "out")
+    out = _out(out, (C, max(L - M + 1, 0)), torch.float32, x.device)
     _check(lib().tina_fir(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream)))
+    return out
+
+
+def fir_multi(x, taps, out=None, stream=None):
+    """tina_fir_multi: x [C, L] float32 CUDA, taps [C, M] float32 CUDA (row c = channel c's taps)
+    -> y [C, L-M+1] float32."""
+    import torch
+    x = _dev(x, torch.float32, "x")
+    taps = _dev(taps, torch.float32, "taps")
+    if x.dim() != 2 or taps.dim() != 2 or taps.shape[0] != x.shape[0]:
+        raise ValueError("x must be [C, L], taps [C, M]")
+    C, L = x.shape
+    M = taps.shape[1]
+    out = _out(out, (C, max(L - M + 1, 0)), torch.float32, x.device)
+    _check(lib().tina_fir_multi(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream)))
     return out
 
 
@@ -131,9 +194,7 @@ def unfold(x, J: int, out=None, stream=None):
     if x.dim() != 1:
         raise ValueError("x must be 1-D")
     I = x.shape[0]
-    if out is None:
-        out = torch.empty((max(I - J + 1, 0), J), dtype=torch.float32, device=x.device)
-    _dev(out, torch.float32, "out")
+    out = _out(out, (max(I - J + 1, 0), J), torch.float32, x.device)
     _check(lib().tina_unfold(x.data_ptr(), out.data_ptr(), I, J, _stream_ptr(stream)))
     return out
 
@@ -143,9 +204,7 @@ def _ew(fn, a, b, out, stream):
     a, b = _dev(a, torch.float32, "a"), _dev(b, torch.float32, "b")
     if a.shape != b.shape:
         raise ValueError("a and b must have the same shape")
-    if out is None:
-        out = torch.empty_like(a)
-    _dev(out, torch.float32, "out")
+    out = _out(out, a.shape, torch.float32, a.device)
     _check(fn(a.data_ptr(), b.data_ptr(), out.data_ptr(), a.numel(), _stream_ptr(stream)))
     return out
 
@@ -170,9 +229,7 @@ def summation(x, out=None, stream=None):
     if x.dim() != 2:
         raise ValueError("x must be 1-D or 2-D")
     rows, n = x.shape
-    if out is None:
-        out = torch.empty((rows,), dtype=torch.float32, device=x.device)
-    _dev(out, torch.float32, "out")
+    out = _out(out, (rows,), torch.float32, x.device)
     _check(lib().tina_sum(x.data_ptr(), rows, n, out.data_ptr(), _stream_ptr(stream)))
     return out[0] if one_d else out
 
@@ -185,9 +242,7 @@ def matmul(x, y, out=None, stream=None):
         raise ValueError("need x [M, L] and y [L, N]")
     M, L = x.shape
     N = y.shape[1]
-    if out is None:
-        out = torch.empty((M, N), dtype=torch.float32, device=x.device)
-    _dev(out, torch.float32, "out")
+    out = _out(out, (M, N), torch.float32, x.device)
     _check(lib().tina_matmul(x.data_ptr(), y.data_ptr(), out.data_ptr(), M, L, N, _stream_ptr(stream)))
     return out
 
@@ -199,9 +254,7 @@ def dft(x, inverse: bool = False, prec: int = PREC_FP32, out=None, stream=None):
     if x.dim() != 2:
         raise ValueError("x must be [B, N]")
     B, N = x.shape
-    if out is None:
-        out = torch.empty_like(x)
-    _dev(out, torch.complex64, "out")
+    out = _out(out, x.shape, torch.complex64, x.device)
     _check(lib().tina_dft(x.data_ptr(), out.data_ptr(), B, N, int(bool(inverse)), prec, _stream_ptr(stream)))
     return out
 
@@ -233,10 +286,10 @@ def pfb(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=None)
     import torch
     squeeze = x.dim() == 1
     x, kind, S, n, F = _pfb_args(x, P, M, window)
+    if squeeze and out is not None and out.dim() == 2:
+        out = out[None]
     NK = P if kind == COMPLEX else P // 2 + 1
-    if out is None:
-        out = torch.empty((S, max(F, 0), NK), dtype=torch.complex64, device=x.device)
-    _dev(out, torch.complex64, "out")
+    out = _out(out, (S, max(F, 0), NK), torch.complex64, x.device)
     _check(lib().tina_pfb_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind, prec,
                                   out.data_ptr(), _stream_ptr(stream)))
     return out[0] if squeeze else out
@@ -247,10 +300,10 @@ def pfb_fft(x, P: int, M: int, window, out=None, stream=None):
     import torch
     squeeze = x.dim() == 1
     x, kind, S, n, F = _pfb_args(x, P, M, window)
+    if squeeze and out is not None and out.dim() == 2:
+        out = out[None]
     NK = P if kind == COMPLEX else P // 2 + 1
-    if out is None:
-        out = torch.empty((S, max(F, 0), NK), dtype=torch.complex64, device=x.device)
-    _dev(out, torch.complex64, "out")
+    out = _out(out, (S, max(F, 0), NK), torch.complex64, x.device)
     _check(lib().tina_pfb_fft_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind,
                                       out.data_ptr(), _stream_ptr(stream)))
     return out[0] if squeeze else out
@@ -261,9 +314,9 @@ def pfb_fir(x, P: int, M: int, window, out=None, stream=None):
     import torch
     squeeze = x.dim() == 1
     x, kind, S, n, F = _pfb_args(x, P, M, window)
-    if out is None:
-        out = torch.empty((S, max(F, 0), P), dtype=x.dtype, device=x.device)
-    _dev(out, x.dtype, "out")
+    if squeeze and out is not None and out.dim() == 2:
+        out = out[None]
+    out = _out(out, (S, max(F, 0), P), x.dtype, x.device)
     _check(lib().tina_pfb_fir_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind,
                                       out.data_ptr(), _stream_ptr(stream)))
     return out[0] if squeeze else out
@@ -274,16 +327,22 @@ def pfb_host(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=
     import torch
     if x.dim() == 1:
         x = x[None, :]
-    if x.is_cuda or window.is_cuda:
+    if x.is_cuda or window.is_cuda or (out is not None and out.is_cuda):
         raise TypeError("pfb_host takes host tensors")
     kind = COMPLEX if x.dtype == torch.complex64 else REAL
     if kind == REAL and x.dtype != torch.float32:
         raise TypeError("x must be complex64 or float32")
+    if x.dim() != 2 or not x.is_contiguous():
+        raise ValueError("x must be a contiguous [S, n_samples] (or [n_samples]) tensor")
+    if window.dtype != torch.float32 or not window.is_contiguous() or window.numel() != P * M:
+        raise ValueError("window must be a contiguous float32 tensor with P*M entries")
     S, n = x.shape
     F = pfb_num_frames(n, P, M)
     NK = P if kind == COMPLEX else P // 2 + 1
     if out is None:
         out = torch.empty((S, max(F, 0), NK), dtype=torch.complex64, pin_memory=True)
+    elif out.dtype != torch.complex64 or not out.is_contiguous() or tuple(out.shape) != (S, max(F, 0), NK):
+        raise ValueError(f"out must be a contiguous complex64 host tensor of shape {(S, max(F, 0), NK)}")
     _check(lib().tina_pfb_batched_host(x.data_ptr(), S, n, P, M, window.data_ptr(), kind, prec,
                                        out.data_ptr(), _stream_ptr(stream)))
     return out

@@ -5,11 +5,12 @@ from __future__ import annotations
 import os
 import shutil
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtina.so")
-SOURCES = ["tina_api.cu", "tina_simt.cu", "tina_umma.cu", "tina_ct.cu", "tina_ctr.cu", "tina_arith.cu"]
+SOURCES = ["tina_api.cu", "tina_simt.cu", "tina_umma.cu", "tina_ct.cu", "tina_ctr.cu", "tina_arith.cu", "tina_peaks.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 
@@ -42,10 +43,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     flags = list(NVCC_FLAGS)
     if verbose:
         flags += ["-Xptxas", "-v"]
-    for src in SOURCES:
+    if os.environ.get("TINA_BUILD_DEV"):
+        flags += ["-DTINA_DEV"]       # development build: role-skipping / ring-depth / in-kernel profiling knobs
+
+    def compile_one(src):
         obj = os.path.join(CSRC, src.replace(".cu", ".o"))
         subprocess.run([nvcc, *flags, "-c", os.path.join(CSRC, src), "-o", obj], check=True)
-        objs.append(obj)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as ex:
+        objs = list(ex.map(compile_one, SOURCES))
     tmp = LIB + f".tmp{os.getpid()}"
     subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs, "-cudart", "static", "-lpthread", "-ldl"], check=True)
     os.replace(tmp, LIB)

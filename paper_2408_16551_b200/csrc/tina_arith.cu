@@ -13,13 +13,8 @@ namespace {
 
 int sm_count()
 {
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
-    }
-    return n;
+    DevCtx* ctx = nullptr;
+    return dev_ctx(&ctx) == TINA_OK ? ctx->n_sm : 148;      // grid sizing only
 }
 
 template <bool MUL>
@@ -157,7 +152,7 @@ tina_status arith_ew(const float* a, const float* b, float* o, long long n, bool
     if (mul) ew_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(a, b, o, n, vec);
     else ew_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(a, b, o, n, vec);
     count_launch();
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("ew_kernel");
     return check_cuda(cudaGetLastError(), "ew_kernel launch");
 }
 
@@ -171,7 +166,7 @@ tina_status arith_sum(const float* x, long long rows, long long n, float* out, c
     if (gx > need) gx = need;
     if (gx < 1) gx = 1;
     const long long chunk = ((n + gx - 1) / gx + 255) / 256 * 256;
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("sum_kernel");
     if (gx == 1) {
         sum_kernel<<<dim3(1, (unsigned)rows), 256, 0, st>>>(x, n, chunk > 0 ? chunk : 256, nullptr, out);
         count_launch();
@@ -196,7 +191,7 @@ tina_status arith_matmul(const float* x, const float* y, float* z, long long M, 
     if (gy > 65535) return fail(TINA_ERR_UNSUPPORTED, "tina_matmul: M too large");
     matmul_kernel<<<dim3((unsigned)gx, (unsigned)gy), 256, 0, st>>>(x, y, z, M, L, N);
     count_launch();
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("matmul_kernel");
     return check_cuda(cudaGetLastError(), "matmul_kernel launch");
 }
 

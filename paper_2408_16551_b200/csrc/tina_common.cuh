@@ -5,6 +5,8 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <map>
+#include <mutex>
 
 #include "../../include/tina.h"
 
@@ -18,23 +20,74 @@ enum Path { kPathNone = 0, kPathSimt = 1, kPathUmma = 2 };
 
 extern std::atomic<long long> g_launches;
 extern std::atomic<int> g_last_path;
+extern std::atomic<const char*> g_last_kernel;        // name of the kernel variant the last device call launched
+extern std::atomic<double> g_last_issued_ratio;       // tensor flops issued per pass / useful flops of that call
 
 void set_error(const char* fmt, ...);
 tina_status fail(tina_status s, const char* fmt, ...);
 tina_status check_cuda(cudaError_t e, const char* what);
 
+// ---- run-time options (environment, read ONCE; tina_reload_options() re-reads them) --------------
+// Every option selects between variants that compute the SAME result within the same contract.
+// The knobs that change the amount of work or the accuracy contract (TINA_DEBUG_SKIP, TINA_KSPLIT,
+// ring depths, TINA_CL4, TINA_PROF) exist only in builds compiled with -DTINA_DEV.
+struct Options {
+    bool nt256 = false;        // TINA_NT256: 256-column passes with two TMEM stages (dense kernel)
+    bool share = false;        // TINA_SHARE: clusters of four share the subfilter stage (dense kernel)
+    bool no_out_tma = false;   // TINA_NO_OUT_TMA: real-kind epilogue through registers instead of TMA stores
+    bool fir_simt = false;     // TINA_FIR_SIMT: tina_fir on the CUDA-core kernel even where the Toeplitz path applies
+    bool ct_no_ws = false;     // TINA_CT_NO_WS: factorised complex kernel without warp specialisation
+    bool ctr_ws = false;       // TINA_CTR_WS: warp-specialised factorised real kernel
+    bool no_sym = false;       // TINA_NO_SYM: complex dense contraction without the k <-> P-k column pairing
+    // -DTINA_DEV only (always 0 / false otherwise):
+    int debug_skip = 0, ksplit = 0, a_slots = 0, b_entries = 0, cl4 = 0;
+    bool prof = false;
+};
+const Options& options();
+void reload_options();
+
+// ---- per-device state: SM count, kernels whose >48 KB dynamic shared memory opt-in has been set ---
+struct DevCtx {
+    int dev = -1;
+    int n_sm = 0;
+    std::mutex mu;
+    std::map<const void*, int> smem_attr;   // kernel -> bytes opted in on this device
+    std::map<const void*, int> occupancy;   // kernel -> resident CTAs per SM (cached query)
+    void* tz_ring = nullptr;                // Toeplitz scratch of tina_fir (tina_umma.cu)
+    std::atomic<unsigned> tz_next{0};
+    // tina_pfb_batched_host: staging buffers, internal streams and events (tina_api.cu)
+    void* stage_p[3] = {nullptr, nullptr, nullptr};
+    size_t stage_n[3] = {0, 0, 0};
+    cudaStream_t s_in = nullptr, s_cmp = nullptr, s_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_in[64] = {}, ev_cmp[64] = {};
+    std::mutex host_mu;                     // serialises tina_pfb_batched_host on this device
+};
+// context of the CURRENT device (cudaGetDevice), created on first use; the registry is mutex-guarded
+tina_status dev_ctx(DevCtx** out);
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (device, kernel)
+tina_status ensure_smem(DevCtx* ctx, const void* func, int bytes, const char* what);
+void dev_ctx_release_all();                 // frees per-device scratch (tina_clear_plan_cache)
+
+inline void note_kernel(const char* name, double issued_ratio = 1.0)
+{
+    g_last_kernel.store(name, std::memory_order_relaxed);
+    g_last_issued_ratio.store(issued_ratio, std::memory_order_relaxed);
+}
 inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 // ---- generic CUDA-core path (tina_simt.cu) ------------------------------------------
 tina_status simt_fir(const float* x, const float* taps, float* y, int C, long long L, int M,
-                     cudaStream_t st);
+                     cudaStream_t st, bool per_channel = false);
 tina_status simt_unfold(const float* x, float* y, long long I, int J, cudaStream_t st);
 // PFB / DFT on CUDA cores: window == nullptr means M == 1 with unit taps (plain DFT).
 tina_status simt_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window,
                      bool real, bool inverse, void* out, cudaStream_t st);
 tina_status simt_pfb_fir(const void* x, int S, long long n_samples, int P, int M,
                          const float* window, bool real, void* y, cudaStream_t st);
+
+// ---- measured arithmetic ceilings (tina_peaks.cu) -----------------------------------
+tina_status probe_peak(int which, int iters, double* tflops, double* ms_out, cudaStream_t st);
 
 // ---- tcgen05 tensor-core path (tina_umma.cu) ----------------------------------------
 bool umma_supported(int P, bool real);

@@ -492,26 +492,13 @@ tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float
     if (!w32) return ps;
     const long long gps = (F + CT_FR - 1) / CT_FR;
     if (gps * S > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb_fft: too many frames");
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaError_t e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ct_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CtSmem) + 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ct_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CtSmem) + 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ct_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CtSmem) + 1024);
-        if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "pfb_ct_kernel setup"); }
-    }
+    DevCtx* ctx = nullptr;
+    if ((ps = dev_ctx(&ctx)) != TINA_OK) return ps;
+    const int n_sm = ctx->n_sm;
     const int total = (int)(gps * S);
-    if (!getenv("TINA_CT_NO_WS")) {                         // warp-specialised variant: one 640-thread CTA per SM
-        static bool ws_ready = false;
-        if (!ws_ready) {
-            cudaError_t e = cudaFuncSetAttribute(pfb_ctws_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WsSmem) + 1024);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctws_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WsSmem) + 1024);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctws_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WsSmem) + 1024);
-            if (e != cudaSuccess) return check_cuda(e, "pfb_ctws_kernel setup");
-            ws_ready = true;
-        }
+    if (!options().ct_no_ws) {                              // warp-specialised variant: one 640-thread CTA per SM
+        const void* kw = M <= 4 ? (const void*)pfb_ctws_kernel<4> : M <= 8 ? (const void*)pfb_ctws_kernel<8> : (const void*)pfb_ctws_kernel<16>;
+        if ((ps = ensure_smem(ctx, kw, (int)sizeof(WsSmem) + 1024, "pfb_ctws_kernel setup")) != TINA_OK) return ps;
         const int grid = total < n_sm ? total : n_sm;
         const size_t smem = sizeof(WsSmem) + 1024;
         const float2* xf = static_cast<const float2*>(x);
@@ -520,8 +507,12 @@ tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float
         else if (M <= 8) pfb_ctws_kernel<8><<<grid, WS_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
         else pfb_ctws_kernel<16><<<grid, WS_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
         count_launch();
-        g_last_path = kPathUmma;
+        g_last_path = kPathUmma; note_kernel("pfb_ctws_kernel");
         return check_cuda(cudaGetLastError(), "pfb_ctws_kernel launch");
+    }
+    {
+        const void* kc = M <= 4 ? (const void*)pfb_ct_kernel<4> : M <= 8 ? (const void*)pfb_ct_kernel<8> : (const void*)pfb_ct_kernel<16>;
+        if ((ps = ensure_smem(ctx, kc, (int)sizeof(CtSmem) + 1024, "pfb_ct_kernel setup")) != TINA_OK) return ps;
     }
     const int per_sm = 2;                                   // 256 threads, 89 KB shared memory, 128 TMEM columns per CTA
     const int grid = total < n_sm * per_sm ? total : n_sm * per_sm;
@@ -532,7 +523,7 @@ tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float
     else if (M <= 8) pfb_ct_kernel<8><<<grid, CT_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
     else pfb_ct_kernel<16><<<grid, CT_THREADS, smem, st>>>(xf, n_samples, window, w32, of, F, NBLK, M, (int)gps, total);
     count_launch();
-    g_last_path = kPathUmma;
+    g_last_path = kPathUmma; note_kernel("pfb_ct_kernel");
     return check_cuda(cudaGetLastError(), "pfb_ct_kernel launch");
 }
 

@@ -639,39 +639,33 @@ tina_status ctr_pfb(const void* x, int S, long long n_samples, int M, const floa
     const long long NBLK = n_samples / CR_P, F = NBLK - M + 1;
     const long long gps = (F + CR_FR - 1) / CR_FR;
     if (gps * S > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb_fft: too many frames");
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaError_t e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctr_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CrSmem) + 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctr_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CrSmem) + 1024);
-        if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "pfb_ctr_kernel setup"); }
-    }
+    DevCtx* ctx = nullptr;
+    tina_status ps = dev_ctx(&ctx);
+    if (ps != TINA_OK) return ps;
+    const int n_sm = ctx->n_sm;
     const int total = (int)(gps * S);
     const int grid = total < n_sm ? total : n_sm;           // one CTA per SM (all 512 TMEM columns)
     const float* xf = static_cast<const float*>(x);
     float2* of = static_cast<float2*>(out);
-    if (getenv("TINA_CTR_WS")) {                            // warp-specialised variant: one 640-thread CTA per SM
-        static bool ws_ready = false;
+    if (options().ctr_ws) {                                 // warp-specialised variant: one 640-thread CTA per SM
         const size_t wsmem = sizeof(CwSmem) + 1024;
-        if (!ws_ready) {
-            cudaError_t e = cudaFuncSetAttribute(pfb_ctrws_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(pfb_ctrws_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem);
-            if (e != cudaSuccess) return check_cuda(e, "pfb_ctrws_kernel setup");
-            ws_ready = true;
-        }
+        const void* kw = M <= 4 ? (const void*)pfb_ctrws_kernel<4> : (const void*)pfb_ctrws_kernel<8>;
+        if ((ps = ensure_smem(ctx, kw, (int)wsmem, "pfb_ctrws_kernel setup")) != TINA_OK) return ps;
         if (M <= 4) pfb_ctrws_kernel<4><<<grid, CW_THREADS, wsmem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
         else pfb_ctrws_kernel<8><<<grid, CW_THREADS, wsmem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
         count_launch();
-        g_last_path = kPathUmma;
+        g_last_path = kPathUmma; note_kernel("pfb_ctrws_kernel");
         return check_cuda(cudaGetLastError(), "pfb_ctrws_kernel launch");
     }
     const size_t smem = sizeof(CrSmem) + 1024;
+    {
+        const void* kc = M <= 4 ? (const void*)pfb_ctr_kernel<4> : (const void*)pfb_ctr_kernel<8>;
+        if ((ps = ensure_smem(ctx, kc, (int)smem, "pfb_ctr_kernel setup")) != TINA_OK) return ps;
+    }
     if (M <= 4) pfb_ctr_kernel<4><<<grid, CR_THREADS, smem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
     else pfb_ctr_kernel<8><<<grid, CR_THREADS, smem, st>>>(xf, n_samples, window, of, F, NBLK, M, (int)gps, total);
     count_launch();
-    g_last_path = kPathUmma;
+    g_last_path = kPathUmma; note_kernel("pfb_ctr_kernel");
     return check_cuda(cudaGetLastError(), "pfb_ctr_kernel launch");
 }
 

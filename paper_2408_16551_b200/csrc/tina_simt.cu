@@ -72,7 +72,7 @@ __device__ __forceinline__ void cp_async4(float* dst_smem, const float* src, boo
 template <int LD>
 __global__ void __launch_bounds__(FIR_THREADS)
 fir_kernel(const float* __restrict__ x, const float* __restrict__ taps, float* __restrict__ y,
-           long long L, int M, long long Lo, int tiles_per_chan, int total_tiles)
+           long long L, int M, long long Lo, int tiles_per_chan, int total_tiles, int taps_stride)
 {
     extern __shared__ __align__(16) float smem[];
     const int Mp = (M + 15) & ~15;                     // taps padded to a multiple of 16 (zeros)
@@ -91,10 +91,20 @@ fir_kernel(const float* __restrict__ x, const float* __restrict__ taps, float* _
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    for (int i = threadIdx.x; i < Mp; i += FIR_THREADS) s_taps[i] = (i < M) ? __ldg(taps + (M - 1 - i)) : 0.f;
-    int tile = blockIdx.x, buf = 0;
+    // taps_stride == 0: one tap vector for every channel (loaded once); otherwise channel c filters with
+    // taps + c * taps_stride, reloaded whenever the tile's channel changes (every read of s_taps for the
+    // previous tile lies before the __syncthreads() that follows its s_out writes)
+    int tile = blockIdx.x, buf = 0, cur_chan = -1;
     if (tile < total_tiles) stage(tile, s_buf0);
     for (; tile < total_tiles; tile += gridDim.x, buf ^= 1) {
+    {
+        const int c = taps_stride ? tile / tiles_per_chan : 0;
+        if (c != cur_chan) {
+            const float* tc = taps + (long long)c * taps_stride;
+            for (int i = threadIdx.x; i < Mp; i += FIR_THREADS) s_taps[i] = (i < M) ? __ldg(tc + (M - 1 - i)) : 0.f;
+            cur_chan = c;
+        }
+    }
     float* s_x = s_buf0 + buf * 16 * LD;
     const int nxt = tile + gridDim.x;
     if (nxt < total_tiles) { stage(nxt, s_buf0 + (buf ^ 1) * 16 * LD); asm volatile("cp.async.wait_group 1;" ::: "memory"); }
@@ -157,40 +167,45 @@ fir_kernel(const float* __restrict__ x, const float* __restrict__ taps, float* _
 }
 
 tina_status simt_fir(const float* x, const float* taps, float* y, int C, long long L, int M,
-                     cudaStream_t st)
+                     cudaStream_t st, bool per_channel)
 {
+    const int taps_stride = per_channel ? M : 0;
     const long long Lo = L - M + 1;
     const long long tiles = (Lo + FIR_TILE - 1) / FIR_TILE;
     if (tiles * C > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_fir: C*L too large for one grid");
     const int Mp = (M + 15) & ~15;
     const bool small = Mp <= 512;
     const size_t smem = sizeof(float) * ((size_t)Mp + 3 * 16 * (size_t)(small ? FIR_LD_SMALL : FIR_LD_LARGE));
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaError_t e = cudaFuncSetAttribute(fir_kernel<FIR_LD_LARGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(fir_kernel<FIR_LD_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "fir_kernel setup"); }
-    }
+    DevCtx* ctx = nullptr;
+    tina_status cs = dev_ctx(&ctx);
+    if (cs != TINA_OK) return cs;
+    const int n_sm = ctx->n_sm;
+    const void* kern = small ? (const void*)fir_kernel<FIR_LD_SMALL> : (const void*)fir_kernel<FIR_LD_LARGE>;
+    if ((cs = ensure_smem(ctx, kern, small ? 64 * 1024 : 120 * 1024, "fir_kernel setup")) != TINA_OK) return cs;
     const long long total = tiles * C;
-    // resident CTAs per SM (registers / shared memory): a persistent grid must not exceed one wave
-    static int occ_small = 0, occ_large = 0;
-    int& occ = small ? occ_small : occ_large;
-    if (!occ) {
-        cudaError_t e = small ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fir_kernel<FIR_LD_SMALL>, FIR_THREADS, smem)
-                              : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fir_kernel<FIR_LD_LARGE>, FIR_THREADS, smem);
-        if (e != cudaSuccess || occ < 1) { occ = 0; return check_cuda(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor(fir_kernel)"); }
+    // resident CTAs per SM (registers / shared memory): a persistent grid must not exceed one wave.  The query
+    // depends on the dynamic shared memory size, i.e. on Mp: cached per (device, kernel, Mp).
+    int occ = 0;
+    {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        const void* key = reinterpret_cast<const char*>(kern) + Mp;       // distinct key per padded tap count
+        auto it = ctx->occupancy.find(key);
+        if (it != ctx->occupancy.end()) occ = it->second;
+        else {
+            cudaError_t e = small ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fir_kernel<FIR_LD_SMALL>, FIR_THREADS, smem)
+                                  : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fir_kernel<FIR_LD_LARGE>, FIR_THREADS, smem);
+            if (e != cudaSuccess || occ < 1) return check_cuda(e != cudaSuccess ? e : cudaErrorLaunchOutOfResources, "cudaOccupancyMaxActiveBlocksPerMultiprocessor(fir_kernel)");
+            ctx->occupancy[key] = occ;
+        }
     }
     const int per_sm = occ;
     const unsigned grid = (unsigned)(total < (long long)n_sm * per_sm ? total : (long long)n_sm * per_sm);
     if (small)
-        fir_kernel<FIR_LD_SMALL><<<grid, FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles, (int)total);
+        fir_kernel<FIR_LD_SMALL><<<grid, FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles, (int)total, taps_stride);
     else
-        fir_kernel<FIR_LD_LARGE><<<grid, FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles, (int)total);
+        fir_kernel<FIR_LD_LARGE><<<grid, FIR_THREADS, smem, st>>>(x, taps, y, L, M, Lo, (int)tiles, (int)total, taps_stride);
     count_launch();
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("fir_kernel");
     return check_cuda(cudaGetLastError(), "fir_kernel launch");
 }
 
@@ -299,14 +314,11 @@ tina_status simt_pfb(const void* x, int S, long long n_samples, int P, int M, co
     const long long tiles = (F + TF - 1) / TF;
     if (tiles * S > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: too many tiles");
     const size_t smem = sizeof(float) * (2 * (size_t)P + (size_t)TF * P * elem);
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(pfb_simt_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(pfb_simt_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e != cudaSuccess) return check_cuda(e, "cudaFuncSetAttribute(pfb_simt_kernel)");
-        attr_done = true;
-    }
+    DevCtx* ctx = nullptr;
+    tina_status cs = dev_ctx(&ctx);
+    if (cs != TINA_OK) return cs;
+    const void* kern = real ? (const void*)pfb_simt_kernel<true> : (const void*)pfb_simt_kernel<false>;
+    if ((cs = ensure_smem(ctx, kern, 200 * 1024, "cudaFuncSetAttribute(pfb_simt_kernel)")) != TINA_OK) return cs;
     const float scale = inverse ? (float)(1.0 / (double)P) : 1.f;
     if (real)
         pfb_simt_kernel<true><<<(unsigned)(tiles * S), PFB_SIMT_THREADS, smem, st>>>(
@@ -315,7 +327,7 @@ tina_status simt_pfb(const void* x, int S, long long n_samples, int P, int M, co
         pfb_simt_kernel<false><<<(unsigned)(tiles * S), PFB_SIMT_THREADS, smem, st>>>(
             x, n_samples, P, M, window, F, TF, (int)tiles, inverse ? 1 : 0, scale, out);
     count_launch();
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("pfb_simt_kernel");
     return check_cuda(cudaGetLastError(), "pfb_simt_kernel launch");
 }
 
@@ -389,7 +401,7 @@ tina_status simt_pfb_fir(const void* x, int S, long long n_samples, int P, int M
         pfb_fir_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(
             (const float2*)x, stride2, P2, M, window, F, (float2*)y, total, (int)runs);
     count_launch();
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("pfb_fir_kernel");
     return check_cuda(cudaGetLastError(), "pfb_fir_kernel launch");
 }
 
@@ -416,7 +428,7 @@ tina_status simt_unfold(const float* x, float* y, long long I, int J, cudaStream
     if (blocks > 148LL * 32) blocks = 148LL * 32;
     unfold_kernel<<<(unsigned)blocks, 256, 0, st>>>(x, y, total, J);
     count_launch();
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("unfold_kernel");
     return check_cuda(cudaGetLastError(), "unfold_kernel launch");
 }
 

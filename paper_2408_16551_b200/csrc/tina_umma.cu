@@ -364,8 +364,17 @@ __device__ __forceinline__ void arrive_leader(uint32_t bar, uint32_t rank_in_pai
     if (CG == 1 || rank_in_pair == 0) mbar_arrive(bar); else mbar_arrive_cluster(bar, leader);
 }
 
-// cycle counter for the optional in-kernel profile (TINA_PROF=1); a constant when profiling is off
+// Development-only instrumentation (-DTINA_DEV): TINA_DEBUG_SKIP role-skipping bits and the TINA_PROF
+// in-kernel cycle counters.  The default build compiles both out: no knob can skip work.
+#ifdef TINA_DEV
+#define TINA_DBG(bit) (prm.debug & (bit))
 #define PF_NOW() (prm.prof ? clock64() : 0LL)
+#define PF_ON() (prm.prof != nullptr)
+#else
+#define TINA_DBG(bit) 0
+#define PF_NOW() 0LL
+#define PF_ON() false
+#endif
 
 // =====================================================================================
 // The fused kernel.  MT = compile-time tap count the sliding window is unrolled for
@@ -447,7 +456,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             const uint32_t bar = smem_u32(&ctl->b_full[b.idx]);
                             const uint32_t dst = smem_u32(b_ring + b.idx * B_ENTRY);
                             const int row = part * N + n0 + nh * NSUB + (int)rank * (nw / CG);
-                            if (prm.debug & 8) { if (rank == 0) mbar_arrive(bar); }
+                            if (TINA_DBG(8)) { if (rank == 0) mbar_arrive(bar); }
                             else if (CG == 1) {
                                 mbar_expect_tx(bar, b_box_bytes);
                                 tma_load_2d(dst, &tmap_b, bar, kc * KC, row);
@@ -518,14 +527,14 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     if (lane == 0) {
                         const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + bi * B_ENTRY));
                         uint32_t acc = kc > kc_begin;
-                        if (prm.debug & 4) { } else
+                        if (TINA_DBG(4)) { } else
                         if (parts > 1) {
                             const uint64_t ad = smem_desc_sw128(a_lo);
 #pragma unroll
                             for (int k = 0; k < KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
                         }
                         const uint64_t ad = smem_desc_sw128(a_hi);
-                        if (!(prm.debug & 4))
+                        if (!TINA_DBG(4))
 #pragma unroll
                         for (int k = 0; k < KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
                         commit_cg<CG>(smem_u32(&ctl->b_empty[bi]), pair_mask);
@@ -539,7 +548,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                         if (lane == 0) {
                             const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + bi * B_ENTRY));
                             const uint64_t ad = smem_desc_sw128(a_hi);
-                            if (!(prm.debug & 4))
+                            if (!TINA_DBG(4))
 #pragma unroll
                             for (int k = 0; k < KC / 16; ++k) umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
                             commit_cg<CG>(smem_u32(&ctl->b_empty[bi]), pair_mask);
@@ -560,7 +569,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             t.advance(n_acc);
             }
         }
-        if (prm.prof && lane == 0 && h == 0) {
+        if (PF_ON() && lane == 0 && h == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
             pp[0] = PF_NOW() - pf_tot; pp[1] = pf_a; pp[2] = pf_b; pp[3] = pf_t;
         }
@@ -585,7 +594,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             const int s = tile / prm.tiles_per_stream;
             const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + q * 32;
             float* obase = prm.out + (long long)s * prm.out_stream_stride + row0 * prm.out_row + n0;
-            const int rows_valid = (prm.debug & 2) ? 0 : (int)min(32LL, prm.F - row0);   // <= 0: nothing to store
+            const int rows_valid = TINA_DBG(2) ? 0 : (int)min(32LL, prm.F - row0);   // <= 0: nothing to store
             for (int ks = 0; ks < prm.k_splits; ++ks) {
                 const uint32_t blk0 = n_acc == 2 ? t.idx : 0;
                 // wait for the 256-column TMEM block that column cb starts (called before its first tcgen05.ld)
@@ -612,7 +621,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     float* const orow = obase + (long long)lane * prm.out_row;               // this lane's output row
                     for (int cb = 0; cb < nt; cb += 32) {
                         tmem_ld_wait();
-                        if (REAL && lane < rows_valid && !(prm.debug & 2)) {
+                        if (REAL && lane < rows_valid && !TINA_DBG(2)) {
                             if (n0 + cb == 0) {
                                 // columns 0 / 1 carry Re X[0] and Re X[P/2]; Im X[0] = Im X[P/2] = 0
                                 float2* ny = reinterpret_cast<float2*>(orow + prm.P);
@@ -652,7 +661,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                         if (cb + 32 < nt && !last_of_block) tmem_ld32(taddr + cb + 32, r);
                         fence_proxy_async();
                         __syncwarp();
-                        if (lane == 0 && !(prm.debug & 2)) {
+                        if (lane == 0 && !TINA_DBG(2)) {
                             if (!REAL) {
                                 if (ks == 0) tma_store_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
                                 else         tma_reduce_add_3d(&tmap_out, tile_s, n0 + cb, (int)row0, s);
@@ -700,7 +709,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     const long long e0 = row0 * prm.out_row + n0;
                     long long n_run = prm.out_len - e0;                        // valid elements of the run
                     if (n_run > 32LL * 128) n_run = 32LL * 128;
-                    if (n_run > 0 && !(prm.debug & 2)) {
+                    if (n_run > 0 && !TINA_DBG(2)) {
                         float* g = obase;                                        // address of l = 0
                         const int run = (int)n_run;
                         const int head = min(run, (int)(((16u - ((uint32_t)(uintptr_t)g & 15u)) & 15u) >> 2));
@@ -801,7 +810,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             }
         }
         if (prm.out_tma && lane == 0) bulk_wait<0>();            // staging tiles must outlive their TMA reads
-        if (prm.prof && q == 0 && lane == 0) {
+        if (PF_ON() && q == 0 && lane == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
             pp[8] = PF_NOW() - pe_tot; pp[9] = pe_w; pp[10] = pe_ld; pp[11] = pe_sts; pp[12] = pe_st; pp[13] = pe_fo; pp[14] = pe_sy;
         }
@@ -840,7 +849,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                        (x_len == 0 || (f0 + FPW + M - 2) * K + prm.K <= x_len);
         };
         auto load = [&](int kk) {
-            if (prm.debug & 1) return;
+            if (TINA_DBG(1)) return;
             if (interior) fir_load<MT, REAL, false>(rg, window, P, M, K, nblk, xs + kk * KC, kk * KC + 2 * lane, f0);
             else          fir_load<MT, REAL, true>(rg, window, P, M, K, nblk, xs + kk * KC, kk * KC + 2 * lane, f0, x_len);
         };
@@ -863,7 +872,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             const uint32_t slot_i = n % n_a, slot_ph = (n / n_a) & 1u;
             pq_x = PF_NOW(); mbar_wait(smem_u32(&ctl->a_empty[slot_i]), slot_ph ^ 1); pq_w += PF_NOW() - pq_x;
             pq_x = PF_NOW();
-            if (!(prm.debug & 1))
+            if (!TINA_DBG(1))
                 fir_compute_store<MT>(rg, a_ring_s + slot_i * a_slot_bytes, swz, split, 0, prm.fp16 != 0);
             if (have2) {
                 if (w2 != w) set_tile(w2);
@@ -889,7 +898,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             pq_f += PF_NOW() - pq_x;
             w = w2; kc = kc2; n = n2; have = have2;
         }
-        if (prm.prof && pw == 0 && lane == 0) {
+        if (PF_ON() && pw == 0 && lane == 0) {
             unsigned long long* pp = prm.prof + blockIdx.x * 16;
             pp[4] = PF_NOW() - pq_tot; pp[5] = pq_w; pp[6] = pq_c; pp[7] = pq_f;
         }
@@ -910,16 +919,12 @@ bool umma_supported(int P, bool real)
 }
 
 template <int MT, bool REAL, bool SHARE>
-static tina_status launch_umma(const CUtensorMap& tmap, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
+static tina_status launch_umma(DevCtx* ctx, const CUtensorMap& tmap, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
                                const UmmaParams& prm, int grid, cudaStream_t st)
 {
     auto kern = pfb_umma_kernel<MT, REAL, UMMA_CG, SHARE>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UMMA_SMEM_BYTES);
-        if (e != cudaSuccess) return check_cuda(e, "cudaFuncSetAttribute(pfb_umma_kernel)");
-        attr_done = true;
-    }
+    tina_status as = ensure_smem(ctx, reinterpret_cast<const void*>(kern), (int)UMMA_SMEM_BYTES, "cudaFuncSetAttribute(pfb_umma_kernel)");
+    if (as != TINA_OK) return as;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(UMMA_THREADS);
@@ -933,21 +938,30 @@ static tina_status launch_umma(const CUtensorMap& tmap, const CUtensorMap& tmap_
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     UmmaParams prm2 = prm;
-    const bool prof = getenv("TINA_PROF") != nullptr;
-    if (prof) { cudaMalloc(&prm2.prof, (size_t)grid * 16 * 8); cudaMemsetAsync(prm2.prof, 0, (size_t)grid * 16 * 8, st); }
+#ifdef TINA_DEV
+    const bool prof = options().prof;
+    if (prof) {
+        cudaError_t pe = cudaMalloc(&prm2.prof, (size_t)grid * 16 * 8);
+        if (pe == cudaSuccess) pe = cudaMemsetAsync(prm2.prof, 0, (size_t)grid * 16 * 8, st);
+        if (pe != cudaSuccess) { if (prm2.prof) cudaFree(prm2.prof); return check_cuda(pe, "TINA_PROF counter buffer"); }
+    }
+#endif
     cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tmap, tmap_out, tmap_out2, prm2);
+#ifdef TINA_DEV
     if (prof) {
         std::vector<unsigned long long> h((size_t)grid * 16);
-        cudaStreamSynchronize(st);
-        cudaMemcpy(h.data(), prm2.prof, h.size() * 8, cudaMemcpyDeviceToHost);
+        cudaError_t pe = cudaStreamSynchronize(st);
+        if (pe == cudaSuccess) pe = cudaMemcpy(h.data(), prm2.prof, h.size() * 8, cudaMemcpyDeviceToHost);
         cudaFree(prm2.prof);
+        if (pe != cudaSuccess) return check_cuda(pe, "TINA_PROF counter read-back");
         double acc[16] = {0};
         for (int b = 0; b < grid; b += UMMA_CG) for (int i = 0; i < 16; ++i) acc[i] += (double)h[(size_t)b * 16 + i] / (grid / UMMA_CG);   // leaders: even ranks
         fprintf(stderr, "[tina prof] leader CTA mean cycles: mma tot %.0f a_full %.0f b_full %.0f t_empty %.0f | prod tot %.0f a_empty %.0f work %.0f fence %.0f | epi tot %.0f t_full %.0f ldwait %.0f sts %.0f lds+stg %.0f fetch %.0f sync %.0f\n",
                 acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], acc[7], acc[8], acc[9], acc[10], acc[11], acc[12], acc[13], acc[14]);
     }
+#endif
     count_launch();
-    g_last_path = kPathUmma;
+    g_last_path = kPathUmma; note_kernel("pfb_umma_kernel");
     if (e != cudaSuccess) return check_cuda(e, "pfb_umma_kernel launch");
     return check_cuda(cudaGetLastError(), "pfb_umma_kernel launch");
 }
@@ -977,6 +991,10 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     const Plan* plan = nullptr;
     tina_status ps = get_plan(P, real, inverse, parts, fp16, st, &plan);
     if (ps != TINA_OK) return ps;
+    DevCtx* ctx = nullptr;
+    if ((ps = dev_ctx(&ctx)) != TINA_OK) return ps;
+    const Options& opt = options();
+    const int n_sm = ctx->n_sm;
 
     UmmaParams prm;
     prm.x = static_cast<const float*>(x);
@@ -994,50 +1012,40 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     prm.out_len = 0;
     prm.out_scalar = 0;
     prm.a_ring_bytes = A_RING_BYTES; prm.b_ring_bytes = B_RING_BYTES; prm.stage_bytes = EPI_STAGE_BYTES;
+#ifdef TINA_DEV
     {   // experiment knobs: ring depths (A slots of 32 KB, B half-tile entries of 16 KB)
-        const char* ea = getenv("TINA_A_SLOTS"); const char* eb = getenv("TINA_B_ENTRIES");
-        if (ea) prm.a_ring_bytes = atoi(ea) * 2 * A_PART_BYTES;
-        if (eb) prm.b_ring_bytes = atoi(eb) * (B_ENTRY_BYTES / UMMA_CG);
+        if (opt.a_slots) prm.a_ring_bytes = opt.a_slots * 2 * A_PART_BYTES;
+        if (opt.b_entries) prm.b_ring_bytes = opt.b_entries * (B_ENTRY_BYTES / UMMA_CG);
         if ((size_t)prm.a_ring_bytes + prm.b_ring_bytes + 4 * prm.stage_bytes + sizeof(SmemCtl) > UMMA_SMEM_BYTES)
             return fail(TINA_ERR_UNSUPPORTED, "ring sizes exceed shared memory");
     }
+#endif
     prm.P = P;
     prm.M = M;
     prm.tiles_per_stream = (int)((F + BM * UMMA_CG - 1) / (BM * UMMA_CG));
     // Column pass width: all 512 TMEM columns (one accumulator stage, both MMA-issuing warps busy).  256-column
     // passes (two TMEM stages, epilogue overlapped) measured slower at config 2 because only one warp issues.
-    prm.nt_pass = getenv("TINA_NT256") ? 256 : NT_MAX;
+    prm.nt_pass = opt.nt256 ? 256 : NT_MAX;
     prm.n_passes = (K + prm.nt_pass - 1) / prm.nt_pass;
     // SHARE (clusters of four, FIR computed once per two column passes) needs an even number of passes
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaError_t e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess || n_sm < 1) { n_sm = 0; return check_cuda(e, "cudaDeviceGetAttribute(SM count)"); }
-    }
     // Measured on B200 (c4 / c5): equal or slightly slower than independent pairs (only 33 clusters of four are
     // co-resident on 148 SMs and the twiddle ring becomes the limiter), so it is opt-in: TINA_SHARE=1.
-    const bool share = prm.n_passes % 2 == 0 && n_sm >= 4 && getenv("TINA_SHARE") != nullptr && !getenv("TINA_NO_SHARE");
+    const bool share = prm.n_passes % 2 == 0 && n_sm >= 4 && opt.share;
     const long long total = (long long)S * prm.tiles_per_stream * (share ? prm.n_passes / 2 : prm.n_passes);
     if (total > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: too many tiles");
     prm.total_work = (int)total;
     prm.parts = parts;
     prm.fp16 = fp16 ? 1 : 0;
     prm.prof = nullptr;
-    { const char* dbg = getenv("TINA_DEBUG_SKIP"); prm.debug = dbg ? atoi(dbg) : 0; }
-    { const char* ksm = getenv("TINA_KSPLIT"); const int kmax = ksm ? atoi(ksm) : KSPLIT_MAX; prm.k_splits = (K + kmax - 1) / kmax; }
+    prm.debug = opt.debug_skip;                                   // 0 unless -DTINA_DEV
+    { const int kmax = opt.ksplit > 0 ? opt.ksplit : KSPLIT_MAX; prm.k_splits = (K + kmax - 1) / kmax; }
     prm.kc_per_split = ((K / KC) + prm.k_splits - 1) / prm.k_splits;
 
     const int cl_size = share ? 4 : UMMA_CG;
     int n_cl = n_sm / cl_size;
     if (share) {
         // clusters of four do not tile every GPC (16 / 18 / 20 SMs): launch only as many as are co-resident
-        static int max_cl4 = 0;
-        if (!max_cl4) {
-            const char* e4 = getenv("TINA_CL4");
-            max_cl4 = e4 ? atoi(e4) : 33;
-        }
+        const int max_cl4 = opt.cl4 > 0 ? opt.cl4 : 33;
         if (n_cl > max_cl4) n_cl = max_cl4;
     }
     const int grid = cl_size * (prm.total_work < n_cl ? prm.total_work : n_cl);
@@ -1052,7 +1060,7 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     memset(&tmap_out, 0, sizeof(tmap_out));
     memset(&tmap_out2, 0, sizeof(tmap_out2));
     prm.out_tma = real ? ((S == 1 || F % 2 == 0) && F >= 2) : 1;
-    if (getenv("TINA_NO_OUT_TMA") && real) prm.out_tma = 0;
+    if (opt.no_out_tma && real) prm.out_tma = 0;
     if (prm.out_tma) {
         EncodeTiledFn enc = encode_fn();
         if (!enc) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
@@ -1086,10 +1094,10 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     }
 
 #define TINA_LAUNCH(MT_)                                                                           \
-    (real ? (share ? launch_umma<MT_, true, true>(plan->tmap, tmap_out, tmap_out2, prm, grid, st)                  \
-                   : launch_umma<MT_, true, false>(plan->tmap, tmap_out, tmap_out2, prm, grid, st))                \
-          : (share ? launch_umma<MT_, false, true>(plan->tmap, tmap_out, tmap_out2, prm, grid, st)                 \
-                   : launch_umma<MT_, false, false>(plan->tmap, tmap_out, tmap_out2, prm, grid, st)))
+    (real ? (share ? launch_umma<MT_, true, true>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st)                  \
+                   : launch_umma<MT_, true, false>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st))                \
+          : (share ? launch_umma<MT_, false, true>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st)                 \
+                   : launch_umma<MT_, false, false>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st)))
     if (!window) return TINA_LAUNCH(0);
     if (M <= 4) return TINA_LAUNCH(4);
     if (M <= 8) return TINA_LAUNCH(8);
@@ -1165,7 +1173,7 @@ bool umma_pfb_fir(const void* x, int S, long long n_samples, int P, int M, const
     else TINA_FIRWIN(16);
 #undef TINA_FIRWIN
     count_launch();
-    g_last_path = kPathSimt;
+    g_last_path = kPathSimt; note_kernel("pfb_fir_win_kernel");
     *status = check_cuda(cudaGetLastError(), "pfb_fir_win_kernel launch");
     return true;
 }
@@ -1204,7 +1212,7 @@ __global__ void toeplitz_kernel(__nv_bfloat16* __restrict__ tz, const float* __r
 bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, int M, cudaStream_t st,
               tina_status* status)
 {
-    if (M > 193 || (L & 1) || getenv("TINA_FIR_SIMT")) return false;
+    if (M > 193 || (L & 1) || options().fir_simt) return false;
     const long long Lo = L - M + 1;
     const int Kp = (FIR_T + M - 1 + KC - 1) / KC * KC;
     const long long R = (Lo + FIR_T - 1) / FIR_T;                    // output blocks (A rows) per channel
@@ -1215,20 +1223,17 @@ bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, i
     // call, in stream order; eight calls may be in flight on different streams before a buffer is reused)
     constexpr int kRing = 8;
     constexpr size_t kTzBytes = (size_t)2 * FIR_T * 320 * sizeof(__nv_bfloat16);
-    static __nv_bfloat16* tz_ring = nullptr;
-    static std::atomic<unsigned> tz_next{0};
-    static int n_sm = 0;
+    DevCtx* ctx = nullptr;
+    if ((*status = dev_ctx(&ctx)) != TINA_OK) return true;
+    const int n_sm = ctx->n_sm;
     {
-        std::lock_guard<std::mutex> lk(g_plan_mu);
-        if (!tz_ring) {
-            int dev = 0;
-            cudaGetDevice(&dev);
-            cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tz_ring), kRing * kTzBytes);
-            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-            if (e != cudaSuccess) { tz_ring = nullptr; *status = check_cuda(e, "cudaMalloc(toeplitz)"); return true; }
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        if (!ctx->tz_ring) {
+            cudaError_t e = cudaMalloc(&ctx->tz_ring, kRing * kTzBytes);
+            if (e != cudaSuccess) { ctx->tz_ring = nullptr; *status = check_cuda(e, "cudaMalloc(toeplitz)"); return true; }
         }
     }
-    __nv_bfloat16* tz = reinterpret_cast<__nv_bfloat16*>(reinterpret_cast<char*>(tz_ring) + (tz_next.fetch_add(1) % kRing) * kTzBytes);
+    __nv_bfloat16* tz = reinterpret_cast<__nv_bfloat16*>(static_cast<char*>(ctx->tz_ring) + (ctx->tz_next.fetch_add(1) % kRing) * kTzBytes);
     toeplitz_kernel<<<(FIR_T * Kp + 255) / 256, 256, 0, st>>>(tz, taps, M, Kp);
     count_launch();
     CUtensorMap tmap, zero1, zero2;
@@ -1269,7 +1274,7 @@ bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, i
         prm.k_splits = 1; prm.kc_per_split = Kp / KC;
         const int n_cl = n_sm / UMMA_CG;
         const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
-        rs = launch_umma<0, false, false>(tmap, zero1, zero2, prm, grid, st);
+        rs = launch_umma<0, false, false>(ctx, tmap, zero1, zero2, prm, grid, st);
     }
     *status = rs;
     return true;

@@ -112,6 +112,48 @@ def pfb_case(P: int, M: int, n_frames: int, real: bool = False, streams: int = 1
     return PfbCase(name, x, w, P, M, real, n_frames, bins)
 
 
+ADVERSARIAL_KINDS = ("constant", "dc_offset", "big_tone", "scale_up", "scale_down", "big_tap")
+
+
+def adversarial_case(kind: str, P: int, M: int, n_frames: int, real: bool = False, streams: int = 1,
+                     seed: int = 0) -> PfbCase:
+    """Inputs chosen to stress data-dependent mechanisms of an implementation (operand splitting,
+    accumulator rounding) -- still only draws and closed-form signals, no filtering or transforms:
+      constant    x = 1 (real) or 1 + 0.5i (complex): every product has the same sign
+      dc_offset   100 + N(0,1)
+      big_tone    one bin-centred tone / cosine of amplitude 1e4 over unit noise
+      scale_up    N(0,1) * 1e20          scale_down  N(0,1) * 1e-20
+      big_tap     random window with one tap 1e4 times the rest (data N(0,1))
+    The window is random and asymmetric (as in the small parity shapes) except where stated."""
+    if kind not in ADVERSARIAL_KINDS:
+        raise ValueError(kind)
+    rng = np.random.default_rng(seed)
+    case = pfb_case(P, M, n_frames, real=real, streams=streams, seed=seed + 1,
+                    window=random_taps(rng, P * M))
+    x = case.x
+    if kind == "constant":
+        x[...] = 1.0 if real else np.complex64(1.0 + 0.5j)
+    elif kind == "dc_offset":
+        x += np.float32(100.0)
+    elif kind == "big_tone":
+        k0 = int(rng.integers(1, P // 2))
+        n = np.arange(P, dtype=np.float64)
+        ph = 2.0 * np.pi * ((k0 * n) % P) / P + 0.3
+        period = 1e4 * (np.cos(ph) if real else np.exp(1j * ph))
+        period = period.astype(x.dtype)
+        for s in range(streams):
+            x[s] = (x[s].reshape(-1, P) + period[None, :]).reshape(-1)
+    elif kind == "scale_up":
+        x *= np.float32(1e20)
+    elif kind == "scale_down":
+        x *= np.float32(1e-20)
+    elif kind == "big_tap":
+        j = int(rng.integers(0, P * M))
+        case.window[j] *= np.float32(1e4)
+    case.name = f"adv_{kind}"
+    return case
+
+
 # ---- the five BASELINE.json configs -------------------------------------------------
 
 def config1() -> PfbCase:
