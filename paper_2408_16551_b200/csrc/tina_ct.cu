@@ -7,7 +7,10 @@
 //     G[f][a][kb]  = sum_b y[f][a + 32 b] W32^(b kb)                        (32-point DFTs, stage 1)
 //     G'[f][a][kb] = G[f][a][kb] * W1024^(a kb)                             (twiddle)
 //     X[f][kb + 32 ka] = sum_a G'[f][a][kb] W32^(a ka)                      (32-point DFTs, stage 2)
-// Both stages are 128 x 64 x 64 real-block GEMMs on tcgen05 (bf16x3, fp32 accumulate in TMEM) against
+// Both stages are 128 x 64 x 64 real-block GEMMs on tcgen05 (bf16 hi / lo operands, ALL FOUR products
+// lo*lo, lo*hi, hi*hi, hi*lo, fp32 accumulate in TMEM: two chained stages double the split error of one,
+// and an input dominated by one branch -- a window with one huge tap -- does not average it away: measured
+// 1.02e-5 with three products; the tensor pipe has slack here) against
 // the SAME 64 x 64 matrix, with the subfilter stage (Eq. (20)) as producer of the first A tile and the
 // twiddle + transpose done by the first epilogue straight into the second A tile: nothing round-trips
 // through HBM, and the tensor work drops from 8 P^2 to 8 P (32 + 32) flops per frame, which makes the
@@ -188,7 +191,9 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
 #pragma unroll
             for (int t = 0; t < CT_NT; ++t) {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, k > 0);
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bl + 2 * k, idesc, k > 0);   // lo x lo
+#pragma unroll
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, 1);
 #pragma unroll
                 for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_ah + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, 1);
 #pragma unroll
@@ -222,7 +227,9 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
 #pragma unroll
             for (int t = 0; t < CT_NT; ++t) {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, k > 0);
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bl + 2 * k, idesc, k > 0);   // lo x lo
+#pragma unroll
+                for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_al + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, 1);
 #pragma unroll
                 for (int k = 0; k < 4; ++k) umma_bf16<1>(tmem + 64 * t, d_ah + t * TILE_DESC + 2 * k, d_bh + 2 * k, idesc, 1);
 #pragma unroll
@@ -446,7 +453,9 @@ pfb_ctws_kernel(const float2* __restrict__ x, long long stream_stride, const flo
                     const uint32_t dcol = tmem + 128 * slot + 64 * t;
                     const uint64_t da = d_ah + t * TILE_DESC;
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + PART_DESC + 2 * k, d_bh + 2 * k, idesc, k > 0);
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + PART_DESC + 2 * k, d_bl + 2 * k, idesc, k > 0);   // lo x lo
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + PART_DESC + 2 * k, d_bh + 2 * k, idesc, 1);
 #pragma unroll
                     for (int k = 0; k < 4; ++k) umma_bf16<1>(dcol, da + 2 * k, d_bh + 2 * k, idesc, 1);
 #pragma unroll

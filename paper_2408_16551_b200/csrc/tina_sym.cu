@@ -1,0 +1,539 @@
+// tina_sym.cu -- the fused PFB / DFT kernel for the COMPLEX kind with every distinct column pair of the
+// Fourier matrix contracted once.
+//
+// Eq. (12) for a complex frame y = yr + i yi and the bins k and P-k:
+//     X[k]   = sum_p y[p] (c - i s),   X[P-k] = sum_p y[p] (c + i s),   c = cos(2 pi p k / P), s = sin(2 pi p k / P)
+// The two bins share the four real sums
+//     U = sum_p yr c,   V = sum_p yi s,   W = sum_p yi c,   Z = sum_p yr s
+//     X[k] = (U + V) + i (W - Z),        X[P-k] = (U - V) + i (W + Z)
+// so the dense contraction against the P x P Fourier matrix needs the real products  yr * [C | S]  and
+// yi * [C | S]  for k in [0, P/2) only: 4 P^2 tensor flops per frame and pass instead of the 8 P^2 of the real
+// 2P x 2P block form (tina_umma.cu), half the twiddle bytes, and contraction length P instead of 2P (one
+// accumulation chain at P = 1024).  It is still the dense contraction of Eq. (12)-(13) -- no factorisation of P;
+// bench.py keeps counting 8 P^2 useful flops and reports the issued count.  Bin 0 has s = 0, so its sine column
+// carries (-1)^p instead and delivers the unpaired Nyquist bin X[P/2].
+//
+// Structure (same roles as tina_umma.cu; CTA pair, tcgen05.mma.cta_group::2, M = 256):
+//   A slot   = [yr hi | yr lo | yi hi | yi lo], 128 frames x 64 contraction elements each (bf16, K-major
+//              SWIZZLE_128B): the FIR producers de-interleave the complex samples with 16-bit stores
+//   B entry  = 64 contraction elements x 256 matrix rows (128 bins x (cos, sin)), half per CTA, hi / lo
+//   TMEM     = D1 (columns 0-255) = yr * [C|S] = (U, Z) per bin,  D2 (columns 256-511) = yi * [C|S] = (W, V)
+//   MMA      = warp 13 issues the yr products into D1, warp 15 the yi products into D2, against the SAME B entry
+//   epilogue = tcgen05.ld of 16 bins from D1 and D2, the +- combine in registers, a forward 32 x 32 staging
+//              tile (bins k ..) and a mirrored one (the aligned group of bins P-k-16 .., in reverse), both stored by TMA
+#include "tina_umma.cuh"
+
+#include <cstring>
+
+namespace tina {
+
+using namespace ptx;
+
+constexpr int SY_BINS = 128;                              // bins per pass: D1 + D2 = 4 x 128 = 512 TMEM columns
+constexpr int SY_A_RING = 128 * 1024;                     // 2 slots of 64 KB (bf16x3) or 4 of 32 KB (single pass)
+constexpr int SY_B_ENTRY = B_ENTRY_BYTES / UMMA_CG;       // 16 KB per CTA
+constexpr int SY_B_ENTRIES = 4;
+constexpr int SY_STAGE = 8192;                            // per epilogue warp: forward + mirrored 32 x 32 fp32 tiles
+constexpr size_t SY_SMEM_BYTES = SY_A_RING + SY_B_ENTRIES * SY_B_ENTRY + 4 * SY_STAGE + sizeof(SmemCtl);
+static_assert(SY_SMEM_BYTES <= 232448, "exceeds the 227 KB shared memory opt-in limit");
+
+struct SymParams {
+    const float* x;            // [S][stream_stride] floats (interleaved complex64)
+    const float* window;       // [M][P] or nullptr (plain DFT batch)
+    float* out;                // [S][F][2P] floats
+    long long stream_stride;   // floats between streams of x
+    long long F, NBLK;
+    int P, M;
+    int tiles_per_stream, n_passes, total_work;
+    int parts;                 // 2: bf16x3, 1: single pass
+    int fp16;
+    int k_splits, kc_per_split;
+    int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 16 no mirrored-tile stores, 32 no forward-tile stores
+};
+
+#ifdef TINA_DEV
+#define SY_DBG(bit) (prm.debug & (bit))
+#else
+#define SY_DBG(bit) 0
+#endif
+
+__device__ __forceinline__ void sts16(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared.b16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+
+// Polyphase MAC of the FPW frames held in registers (as fir_compute_store), the complex result DE-INTERLEAVED:
+// real parts into the yr tiles, imaginary parts into the yi tiles, each split into bf16 hi / lo.
+// `cell` = byte offset (in a 16 KB tile) of this lane's 2-byte cell in row 0 of the warp's slab for each swizzle
+// phase; tile order in the slot: [yr hi | yr lo | yi hi | yi lo] (single pass: [yr | yi]).
+template <int MT>
+__device__ __forceinline__ void fir_compute_store_sym(const FirRegs<MT>& rg, uint32_t slot, const uint32_t (&cell)[8],
+                                                      uint32_t sub_xor, bool split, bool fp16)
+{
+    constexpr int WA = FirRegs<MT>::WA;
+    constexpr int FG = 8;
+    const uint32_t im_off = split ? 2u * A_PART_BYTES : (uint32_t)A_PART_BYTES;
+#pragma unroll
+    for (int i0 = 0; i0 < FPW; i0 += FG) {
+        float2 y[FG];
+        if (MT > 0) {
+#pragma unroll
+            for (int g = 0; g < FG; ++g) y[g] = fmul2(rg.tap[0], rg.row[i0 + g + WA - 1]);
+#pragma unroll
+            for (int m = 1; m < WA; ++m)
+#pragma unroll
+                for (int g = 0; g < FG; ++g) y[g] = ffma2(rg.tap[m], rg.row[i0 + g + WA - 1 - m], y[g]);
+        } else {
+#pragma unroll
+            for (int g = 0; g < FG; ++g) y[g] = rg.row[i0 + g];
+        }
+#pragma unroll
+        for (int g = 0; g < FG; ++g) {
+            const int i = i0 + g;
+            uint32_t hb;
+            if (fp16) { const __half2 hh = __floats2half2_rn(y[g].x, y[g].y); hb = *reinterpret_cast<const uint32_t*>(&hh); }
+            else { const __nv_bfloat162 hi = __floats2bfloat162_rn(y[g].x, y[g].y); hb = *reinterpret_cast<const uint32_t*>(&hi); }
+            const uint32_t addr = slot + (cell[i & 7] ^ sub_xor) + (uint32_t)i * 128u;
+            sts16(addr, hb);
+            sts16(addr + im_off, hb >> 16);
+            if (split) {
+                const float lx = y[g].x - __uint_as_float(hb << 16);
+                const float ly = y[g].y - __uint_as_float(hb & 0xffff0000u);
+                const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
+                const uint32_t lb = *reinterpret_cast<const uint32_t*>(&lo);
+                sts16(addr + A_PART_BYTES, lb);
+                sts16(addr + im_off + A_PART_BYTES, lb >> 16);
+            }
+        }
+    }
+}
+
+template <int MT>
+__global__ void __launch_bounds__(UMMA_THREADS, 1)
+pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_out,
+               const __grid_constant__ CUtensorMap tmap_out2, const SymParams prm)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    if ((smem_u32(smem) & 1023u) != 0) __trap();                // the swizzled tiles need 1024-byte alignment
+    uint8_t* a_ring = smem;
+    uint8_t* b_ring = smem + SY_A_RING;
+    uint8_t* stage = b_ring + SY_B_ENTRIES * SY_B_ENTRY;
+    SmemCtl* ctl = reinterpret_cast<SmemCtl*>(stage + 4 * SY_STAGE);
+
+    constexpr int CG = UMMA_CG;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int parts = prm.parts;
+    const uint32_t a_slot_bytes = 2u * parts * A_PART_BYTES;
+    const uint32_t n_a = (uint32_t)SY_A_RING / a_slot_bytes;            // 2 (bf16x3) or 4 (single pass)
+    const int P = prm.P;
+    const int n_kc = P / KC;
+    const int half = P >> 1;                                           // bins 0 .. P/2 - 1 are contracted
+    const uint32_t rank = cluster_ctarank();                           // rank in the CTA pair; 0 = leader
+    constexpr uint32_t leader = 0;
+    constexpr uint16_t pair_mask = 3;
+    const int cl = blockIdx.x / CG, n_cl = gridDim.x / CG;
+    const int npg = prm.n_passes;
+    const uint32_t b_box_bytes = (uint32_t)(P < NSUB ? P : NSUB) / CG * KC * 2;   // bytes one TMA box delivers
+
+    if (warp == TMA_WARP && lane == 0) {
+        prefetch_tmap(&tmap_b);
+        prefetch_tmap(&tmap_out);
+        prefetch_tmap(&tmap_out2);
+        for (int i = 0; i < 8; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), 2); }
+        for (int i = 0; i < SY_B_ENTRIES; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 2); }
+        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
+        fence_mbar_init();
+    }
+    if (warp == ALLOC_WARP) {
+        tmem_alloc<CG>(smem_u32(&ctl->tmem_base), 512);
+        tmem_relinquish<CG>();
+    }
+    tc_fence_before();
+    cluster_sync();
+    tc_fence_after();
+    const uint32_t tmem_base = ctl->tmem_base;
+
+    if (warp == TMA_WARP) {
+        // ============================ TMA producer: [C|S] tiles, hi then lo per chunk ===============
+        if (lane == 0) {
+            RingPos b;
+            for (int w = cl; w < prm.total_work; w += n_cl) {
+                const int k0 = (w % npg) * SY_BINS;
+                const int nw = 2 * min(SY_BINS, half - k0);               // matrix rows of this pass
+                for (int kc = 0; kc < n_kc; ++kc)
+                    for (int part = 0; part < parts; ++part) {
+                        mbar_wait<64>(smem_u32(&ctl->b_empty[b.idx]), b.phase ^ 1);
+                        const uint32_t bar = smem_u32(&ctl->b_full[b.idx]);
+                        const uint32_t dst = smem_u32(b_ring + b.idx * SY_B_ENTRY);
+                        const int row = part * P + 2 * k0 + (int)rank * (nw / CG);
+                        if (rank == 0) mbar_expect_tx(bar, 2 * b_box_bytes);
+                        tma_load_2d_cg2(dst, &tmap_b, mapa_u32(bar, leader), kc * KC, row);
+                        b.advance(SY_B_ENTRIES);
+                    }
+            }
+        }
+    } else if (warp == MMA_WARP || warp == MMA_WARP2) {
+        // ============================ MMA issuers ===========================================
+        // warp 13 (h = 0): yr tiles -> D1;  warp 15 (h = 1): yi tiles -> D2.  Both consume the same B entries
+        // (b_empty takes one commit from each) and the same A slot (a_empty likewise).  Only the leader CTA
+        // issues; the peer's warp 13 forwards "my A tile is ready" to the leader's barrier.
+        const int h = warp == MMA_WARP ? 0 : 1;
+        if (rank != 0 && h == 0) {
+            RingPos a;
+            for (int w = cl; w < prm.total_work; w += n_cl)
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                    if (lane == 0) mbar_arrive_cluster(smem_u32(&ctl->a_full[a.idx]), leader);
+                    __syncwarp();
+                    a.advance(n_a);
+                }
+        }
+        if (rank == 0) {
+            RingPos a, b;
+            uint32_t te_phase = 0;
+            const uint32_t d = tmem_base + (uint32_t)h * 256u;
+            for (int w = cl; w < prm.total_work; w += n_cl) {
+                const int k0 = (w % npg) * SY_BINS;
+                const int nw = 2 * min(SY_BINS, half - k0);
+                const uint32_t idesc = idesc_bf16(BM * CG, nw, prm.fp16 != 0);
+                for (int ks = 0; ks < prm.k_splits; ++ks) {
+                    const int kc_begin = ks * prm.kc_per_split, kc_end = min(n_kc, kc_begin + prm.kc_per_split);
+                    for (int kc = kc_begin; kc < kc_end; ++kc) {
+                        mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                        tc_fence_after();
+                        const uint32_t a_hi = smem_u32(a_ring + a.idx * a_slot_bytes) + (uint32_t)h * (uint32_t)parts * A_PART_BYTES;
+                        const uint32_t a_lo = a_hi + A_PART_BYTES;
+                        if (kc == kc_begin) {
+                            // first write into this accumulator: wait until the epilogue has drained it
+                            mbar_wait(smem_u32(&ctl->t_empty[h]), te_phase ^ 1u);
+                            te_phase ^= 1u;
+                            tc_fence_after();
+                        }
+                        // ---- B_hi: (A_lo x B_hi) then (A_hi x B_hi)
+                        mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase);
+                        tc_fence_after();
+                        if (lane == 0) {
+                            const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * SY_B_ENTRY));
+                            uint32_t acc = kc > kc_begin;
+                            if (parts > 1) {
+                                const uint64_t ad = smem_desc_sw128(a_lo);
+#pragma unroll
+                                for (int k = 0; k < KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                            }
+                            const uint64_t ad = smem_desc_sw128(a_hi);
+#pragma unroll
+                            for (int k = 0; k < KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                            commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]), pair_mask);
+                        }
+                        __syncwarp();
+                        b.advance(SY_B_ENTRIES);
+                        // ---- B_lo: (A_hi x B_lo)
+                        if (parts > 1) {
+                            mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase);
+                            tc_fence_after();
+                            if (lane == 0) {
+                                const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * SY_B_ENTRY));
+                                const uint64_t ad = smem_desc_sw128(a_hi);
+#pragma unroll
+                                for (int k = 0; k < KC / 16; ++k) umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
+                                commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]), pair_mask);
+                            }
+                            __syncwarp();
+                            b.advance(SY_B_ENTRIES);
+                        }
+                        if (lane == 0) {
+                            commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
+                            if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[h]), pair_mask);
+                        }
+                        __syncwarp();
+                        a.advance(n_a);
+                    }
+                }
+            }
+        }
+    } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
+        // ============================ epilogue ==============================================
+        // Lane = frame (TMEM lane); a step takes 32 accumulator columns = 16 bins kb .. kb+15 from D1 (U, Z) and
+        // D2 (W, V).  Forward tile: bins kb .. kb+15, stored by TMA at column 2 kb.  The mirrored bins P-kb-j are
+        // one bin off any 16-byte-aligned tile (TMA needs 16-byte-aligned box starts), so the mirrored tile is
+        // the ALIGNED group P-kb-16 .. P-kb-1 = the mirrors of j = 1 .. 16, j = 16 being the first bin of the next
+        // step (two extra TMEM columns are read for it).  What does not fit that scheme is stored from registers,
+        // 8 bytes per row: the mirror of a pass's first bin (j = 0; none for bin 0, whose "mirror" is bin 0 itself),
+        // the mirror of j = 15 in the pass's last step (whose tile goes out 28 floats wide through a second map,
+        // because j = 16 belongs to the next pass), and the Nyquist bin.
+        const int q = warp - EPI_WARP0;
+        const uint32_t sb_f = smem_u32(stage) + (uint32_t)q * SY_STAGE, sb_m = sb_f + 4096u;
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+        const uint32_t rowoff = (uint32_t)lane * 128u, sw = (uint32_t)lane & 7u;
+        uint32_t tf_phase = 0;
+        for (int w = cl; w < prm.total_work; w += n_cl) {
+            const int tile = w / npg;
+            const int k0 = (w % npg) * SY_BINS;
+            const int ncol = 2 * min(SY_BINS, half - k0);
+            const int s = tile / prm.tiles_per_stream;
+            const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + q * 32;
+            const bool row_ok = lane < (int)min(32LL, prm.F - row0);
+            float* const orow = prm.out + ((long long)s * prm.F + row0 + lane) * (2LL * P);
+            for (int ks = 0; ks < prm.k_splits; ++ks) {
+                if (ks > 0 && lane == 0) bulk_wait<0>();          // the previous chain's stores to this tile are complete
+                mbar_wait<256>(smem_u32(&ctl->t_full[0]), tf_phase);
+                mbar_wait<256>(smem_u32(&ctl->t_full[1]), tf_phase);
+                tf_phase ^= 1u;
+                tc_fence_after();
+                // one bin (complex value) straight from registers: plain store for the first chain, fp32 add at L2 after
+                auto put = [&](int bin, float re, float im) {
+                    if (row_ok && !SY_DBG(16)) {
+                        float2* g = reinterpret_cast<float2*>(orow + 2 * bin);
+                        if (ks > 0) atomicAdd(g, make_float2(re, im)); else *g = make_float2(re, im);
+                    }
+                };
+                uint32_t r1[32], r2[32], e1[2] = {0u, 0u}, e2[2] = {0u, 0u};
+                tmem_ld32(taddr, r1);
+                tmem_ld32(taddr + 256u, r2);
+                if (32 < ncol) { tmem_ld2(taddr + 32u, e1); tmem_ld2(taddr + 256u + 32u, e2); }
+                for (int cb = 0; cb < ncol; cb += 32) {
+                    const int kb = k0 + (cb >> 1);
+                    const bool last = cb + 32 >= ncol;
+                    tmem_ld_wait();
+                    if (last) {
+                        // both accumulators have been read out completely: hand them back to the MMA warps
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) {
+                            arrive_leader<CG>(smem_u32(&ctl->t_empty[0]), rank, leader);
+                            arrive_leader<CG>(smem_u32(&ctl->t_empty[1]), rank, leader);
+                        }
+                    }
+#define SY_F(v) __uint_as_float(v)
+                    if (kb == 0) {
+                        // bin 0: its sine column carries (-1)^p, i.e. r1[1] + i r2[1] = X[P/2] (unpaired)
+                        put(half, SY_F(r1[1]), SY_F(r2[1]));
+                        r1[1] = 0u; r2[1] = 0u;                  // V = Z = 0 for bin 0: X[0] = U + i W
+                    } else if (cb == 0) {
+                        put(P - kb, SY_F(r1[0]) - SY_F(r2[1]), SY_F(r2[0]) + SY_F(r1[1]));          // mirror of j = 0
+                    }
+                    if (last) put(P - kb - 15, SY_F(r1[30]) - SY_F(r2[31]), SY_F(r2[30]) + SY_F(r1[31]));   // mirror of j = 15
+                    if (lane == 0) bulk_wait_read<1>();           // the forward tile of the previous step has been read
+                    __syncwarp();
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) {
+                        const float U0 = SY_F(r1[4 * g]), Z0 = SY_F(r1[4 * g + 1]), U1 = SY_F(r1[4 * g + 2]), Z1 = SY_F(r1[4 * g + 3]);
+                        const float W0 = SY_F(r2[4 * g]), V0 = SY_F(r2[4 * g + 1]), W1 = SY_F(r2[4 * g + 2]), V1 = SY_F(r2[4 * g + 3]);
+                        sts128(sb_f + rowoff + (((uint32_t)g ^ sw) << 4), __float_as_uint(U0 + V0), __float_as_uint(W0 - Z0),
+                               __float_as_uint(U1 + V1), __float_as_uint(W1 - Z1));
+                    }
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) {
+                        if (SY_DBG(32)) { }
+                        else if (ks == 0) tma_store_3d(&tmap_out, sb_f, 2 * kb, (int)row0, s);
+                        else              tma_reduce_add_3d(&tmap_out, sb_f, 2 * kb, (int)row0, s);
+                        bulk_commit();
+                        bulk_wait_read<1>();                      // the mirrored tile of the previous step has been read
+                    }
+                    __syncwarp();
+                    // mirrored tile: position t <-> bin P-kb-16+t <-> j = 16 - t; 16-byte chunk c holds j = 16-2c, 15-2c
+                    // = accumulator columns 32-4c .. 33-4c and 30-4c .. 31-4c (columns 32, 33 = e1 / e2)
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const float Ua = SY_F(c ? r1[32 - 4 * c] : e1[0]), Za = SY_F(c ? r1[33 - 4 * c] : e1[1]);
+                        const float Wa = SY_F(c ? r2[32 - 4 * c] : e2[0]), Va = SY_F(c ? r2[33 - 4 * c] : e2[1]);
+                        const float Ub = SY_F(r1[30 - 4 * c]), Zb = SY_F(r1[31 - 4 * c]);
+                        const float Wb = SY_F(r2[30 - 4 * c]), Vb = SY_F(r2[31 - 4 * c]);
+                        if (!last)
+                            sts128(sb_m + rowoff + (((uint32_t)c ^ sw) << 4), __float_as_uint(Ua - Va), __float_as_uint(Wa + Za),
+                                   __float_as_uint(Ub - Vb), __float_as_uint(Wb + Zb));
+                        else if (c > 0)                              // last step of the pass: dense rows of 28 floats, positions 2 .. 15
+                            sts128(sb_m + (uint32_t)lane * 112u + (uint32_t)(c - 1) * 16u, __float_as_uint(Ua - Va), __float_as_uint(Wa + Za),
+                                   __float_as_uint(Ub - Vb), __float_as_uint(Wb + Zb));
+                    }
+#undef SY_F
+                    if (!last) {
+                        tmem_ld32(taddr + cb + 32, r1);
+                        tmem_ld32(taddr + 256u + cb + 32, r2);
+                        if (cb + 64 < ncol) { tmem_ld2(taddr + cb + 64, e1); tmem_ld2(taddr + 256u + cb + 64, e2); }
+                    }
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) {
+                        if (SY_DBG(16)) { }
+                        else if (!last) {
+                            const int cm = 2 * (P - kb - 16);
+                            if (ks == 0) tma_store_3d(&tmap_out, sb_m, cm, (int)row0, s);
+                            else         tma_reduce_add_3d(&tmap_out, sb_m, cm, (int)row0, s);
+                        } else {
+                            const int cm = 2 * (P - kb - 14);
+                            if (ks == 0) tma_store_3d(&tmap_out2, sb_m, cm, (int)row0, s);
+                            else         tma_reduce_add_3d(&tmap_out2, sb_m, cm, (int)row0, s);
+                        }
+                        bulk_commit();
+                    }
+                }
+            }
+        }
+        if (lane == 0) bulk_wait<0>();                            // staging tiles must outlive their TMA reads
+    } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
+        // ============================ FIR producers =========================================
+        // A chunk is 64 complex columns = two sub-steps of 32 (one complex sample per lane, 16 frames per
+        // warp, as in tina_umma.cu).  Software pipeline over the flattened (work item, chunk, sub-step)
+        // sequence: the loads of the next sub-step are issued right after the arithmetic of this one.
+        const int pw = warp - PROD_WARP0;
+        const uint32_t a_ring_s = smem_u32(a_ring);
+        // byte offset of this lane's 2-byte cell in row 0 of the warp's slab, per swizzle phase (row & 7), for
+        // sub-step 0: complex column lane -> 16-byte chunk lane >> 3, stored at chunk ^ (row & 7); sub-step 1 is
+        // chunk + 4, i.e. the same offset with bit 6 flipped
+        uint32_t cell[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            cell[j] = (uint32_t)(pw * FPW) * 128u + ((((uint32_t)lane >> 3) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 7u) * 2u;
+        constexpr int WA = MT > 0 ? MT : 1;
+        const float* const window = prm.window;
+        const int M = prm.M;
+        const long long K = 2LL * P, nblk = prm.NBLK;
+        const bool split = parts > 1;
+        FirRegs<MT> rg;
+        int w = cl, st = 0;                                   // st = 2 * kc + sub
+        const int n_st = 2 * n_kc;
+        uint32_t n = 0;                                       // chunk counter over this CTA's whole sequence
+        const float* xs = nullptr;
+        long long f0 = 0;
+        bool interior = false;
+        auto set_tile = [&](int ww) {
+            const int tile = ww / npg;
+            const int s = tile / prm.tiles_per_stream;
+            f0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + pw * FPW;
+            xs = prm.x + (long long)s * prm.stream_stride + 2 * lane;
+            interior = (f0 + M - WA >= 0) && (f0 + FPW + M - 1 <= nblk);
+        };
+        auto load = [&](int sst) {
+            const int c0 = sst * KC + 2 * lane;                // first float column of this lane in the sub-step
+            if (interior) fir_load<MT, false, false>(rg, window, P, M, K, nblk, xs + sst * KC, c0, f0);
+            else          fir_load<MT, false, true>(rg, window, P, M, K, nblk, xs + sst * KC, c0, f0);
+        };
+        bool have = w < prm.total_work;
+        if (have) { set_tile(w); load(st); }
+        while (have) {
+            int w2 = w, st2 = st + 1;
+            if (st2 == n_st) { st2 = 0; w2 += n_cl; }
+            const bool have2 = w2 < prm.total_work;
+            const uint32_t slot_i = n % n_a, slot_ph = (n / n_a) & 1u;
+            const int sub = st & 1;
+            if (sub == 0) mbar_wait(smem_u32(&ctl->a_empty[slot_i]), slot_ph ^ 1);
+            fir_compute_store_sym<MT>(rg, a_ring_s + slot_i * a_slot_bytes, cell, sub ? 64u : 0u, split, prm.fp16 != 0);
+            if (have2) {
+                if (w2 != w) set_tile(w2);
+                load(st2);
+            }
+            if (sub == 1) {
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[slot_i]));
+                ++n;
+            }
+            w = w2; st = st2; have = have2;
+        }
+    }
+
+    tc_fence_before();
+    cluster_sync();                                           // the peer's smem / barriers stay live until both are done
+    if (warp == ALLOC_WARP) tmem_dealloc<CG>(tmem_base, 512);
+}
+
+// =====================================================================================
+// Host side
+// =====================================================================================
+bool sym_supported(int P) { return P >= 64 && P <= kMaxP && P % 64 == 0; }
+
+template <int MT>
+static tina_status launch_sym(DevCtx* ctx, const CUtensorMap& tmap, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
+                              const SymParams& prm, int grid, cudaStream_t st)
+{
+    auto kern = pfb_sym_kernel<MT>;
+    tina_status as = ensure_smem(ctx, reinterpret_cast<const void*>(kern), (int)SY_SMEM_BYTES, "cudaFuncSetAttribute(pfb_sym_kernel)");
+    if (as != TINA_OK) return as;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(UMMA_THREADS);
+    cfg.dynamicSmemBytes = SY_SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = UMMA_CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tmap, tmap_out, tmap_out2, prm);
+    count_launch();
+    g_last_path = kPathUmma;
+    note_kernel("pfb_sym_kernel", 0.5);
+    if (e != cudaSuccess) return check_cuda(e, "pfb_sym_kernel launch");
+    return check_cuda(cudaGetLastError(), "pfb_sym_kernel launch");
+}
+
+// complex kind, P % 64 == 0, window == nullptr (DFT batch) or M <= 16
+tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool inverse,
+                    tina_precision prec, void* out, cudaStream_t st)
+{
+    const long long NBLK = n_samples / P;
+    const long long F = NBLK - M + 1;
+    const int parts = prec == TINA_PREC_FP32 ? 2 : 1;
+    const bool fp16 = prec == TINA_PREC_FP16;
+    const Plan* plan = nullptr;
+    tina_status ps = get_plan(P, false, inverse, parts, fp16, st, &plan, true);
+    if (ps != TINA_OK) return ps;
+    DevCtx* ctx = nullptr;
+    if ((ps = dev_ctx(&ctx)) != TINA_OK) return ps;
+
+    SymParams prm;
+    memset(&prm, 0, sizeof(prm));
+    prm.x = static_cast<const float*>(x);
+    prm.window = window;
+    prm.out = static_cast<float*>(out);
+    prm.stream_stride = 2 * n_samples;
+    prm.F = F;
+    prm.NBLK = NBLK;
+    prm.P = P;
+    prm.M = M;
+    prm.tiles_per_stream = (int)((F + BM * UMMA_CG - 1) / (BM * UMMA_CG));
+    prm.n_passes = (P / 2 + SY_BINS - 1) / SY_BINS;
+    const long long total = (long long)S * prm.tiles_per_stream * prm.n_passes;
+    if (total > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: too many tiles");
+    prm.total_work = (int)total;
+    prm.parts = parts;
+    prm.fp16 = fp16 ? 1 : 0;
+    prm.k_splits = (P + KSPLIT_MAX - 1) / KSPLIT_MAX;             // accumulation chains of <= 1024
+    prm.kc_per_split = ((P / KC) + prm.k_splits - 1) / prm.k_splits;
+    prm.debug = options().debug_skip;                             // 0 unless -DTINA_DEV
+    const int n_cl = ctx->n_sm / UMMA_CG;
+    const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
+
+    // Output maps over [S][F][2P] floats: 32 x 32 swizzled boxes, and 28-float-wide dense boxes for the mirrored
+    // tile of a pass's last step (see the epilogue).
+    CUtensorMap tmap_out, tmap_out2;
+    memset(&tmap_out, 0, sizeof(tmap_out));
+    memset(&tmap_out2, 0, sizeof(tmap_out2));
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    {
+        const cuuint32_t estr[3] = {1, 1, 1};
+        const cuuint64_t dims[3] = {(cuuint64_t)2 * P, (cuuint64_t)F, (cuuint64_t)S};
+        const cuuint64_t strides[2] = {(cuuint64_t)2 * P * sizeof(float), (cuuint64_t)F * 2 * P * sizeof(float)};
+        const cuuint32_t box[3] = {32, 32, 1};
+        CUresult r = enc(&tmap_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        const cuuint32_t box2[3] = {28, 32, 1};
+        if (r == CUDA_SUCCESS)
+            r = enc(&tmap_out2, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims, strides, box2, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(out) failed (%d)", (int)r);
+    }
+    if (!window) return launch_sym<0>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
+    if (M <= 4) return launch_sym<4>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
+    if (M <= 8) return launch_sym<8>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
+    return launch_sym<16>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
+}
+
+}  // namespace tina
