@@ -18,7 +18,7 @@
  * several host threads and on several devices of one process (state is kept per CUDA device; the
  * current device at call time is the one used).  The `_host` entry point serialises per device.
  * Environment: TINA_* variant switches (TINA_SHARE, TINA_NT256, TINA_NO_OUT_TMA, TINA_FIR_SIMT,
- * TINA_CT_NO_WS, TINA_CTR_WS, TINA_NO_SYM) select between kernels that compute the same result under the
+ * TINA_CT_NO_WS, TINA_CTR_WS, TINA_NO_SYM, TINA_SYM_V1) select between kernels that compute the same result under the
  * same contract; they are read once (tina_reload_options() re-reads them).  Knobs that skip work or
  * change the accuracy contract exist only in development builds (-DTINA_DEV, tina_build_is_dev()).
  *

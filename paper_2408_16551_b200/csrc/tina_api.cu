@@ -52,6 +52,7 @@ static void load_options_locked()
     o.ct_no_ws = on("TINA_CT_NO_WS");
     o.ctr_ws = on("TINA_CTR_WS");
     o.no_sym = on("TINA_NO_SYM");
+    o.sym_v1 = on("TINA_SYM_V1");
 #ifdef TINA_DEV
     auto num = [](const char* n) { const char* v = getenv(n); return v ? atoi(v) : 0; };
     o.debug_skip = num("TINA_DEBUG_SKIP");

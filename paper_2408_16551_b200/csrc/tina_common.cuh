@@ -39,6 +39,7 @@ struct Options {
     bool ct_no_ws = false;     // TINA_CT_NO_WS: factorised complex kernel without warp specialisation
     bool ctr_ws = false;       // TINA_CTR_WS: warp-specialised factorised real kernel
     bool no_sym = false;       // TINA_NO_SYM: complex dense contraction without the k <-> P-k column pairing
+    bool sym_v1 = false;       // TINA_SYM_V1: column-paired contraction with register-window producers (no TMA input staging)
     // -DTINA_DEV only (always 0 / false otherwise):
     int debug_skip = 0, ksplit = 0, a_slots = 0, b_entries = 0, cl4 = 0;
     bool prof = false;

@@ -139,6 +139,13 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, uint
                  "[%0], [%1, {%3, %4}], [%2];"
                  ::"r"(dst), "l"(tmap), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
+// 3-D tiled load global -> shared, completion on an mbarrier of this CTA
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const void* tmap, uint32_t bar, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes "
+                 "[%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(dst), "l"(tmap), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
 // cta_group::2 form: data lands in this CTA's smem, completion may signal the peer's barrier
 __device__ __forceinline__ void tma_load_2d_cg2(uint32_t dst, const void* tmap, uint32_t bar, int c0, int c1)
 {
@@ -270,6 +277,17 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr)
     d |= (uint64_t)(1024 >> 4) << 32;                 // SBO = 1024 B       bits [32,46)
     d |= (uint64_t)1 << 46;                           // descriptor version bits [46,48)
     d |= (uint64_t)2 << 61;                           // SWIZZLE_128B       bits [61,64)
+    return d;
+}
+// Same for the 64-byte-swizzled layout: rows of 64 B (32 bf16), 8-row groups of 512 B (SBO), base 512-B aligned.
+__device__ __forceinline__ uint64_t smem_desc_sw64(uint32_t saddr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)(512 >> 4) << 32;                  // SBO = 512 B
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)4 << 61;                           // SWIZZLE_64B
     return d;
 }
 // Instruction descriptor for kind::f16 with bf16 A/B (both K-major), fp32 D.

@@ -24,6 +24,7 @@
 #include "tina_umma.cuh"
 
 #include <cstring>
+#include <vector>
 
 namespace tina {
 
@@ -49,12 +50,17 @@ struct SymParams {
     int fp16;
     int k_splits, kc_per_split;
     int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 16 no mirrored-tile stores, 32 no forward-tile stores
+    unsigned long long* prof;  // -DTINA_DEV only (TINA_PROF): [grid][16] cycle counters
 };
 
 #ifdef TINA_DEV
 #define SY_DBG(bit) (prm.debug & (bit))
+#define SY_NOW() (prm.prof ? clock64() : 0LL)
+#define SY_PROF 1
 #else
 #define SY_DBG(bit) 0
+#define SY_NOW() 0LL
+#define SY_PROF 0
 #endif
 
 __device__ __forceinline__ void sts16(uint32_t addr, uint32_t v)
@@ -66,13 +72,15 @@ __device__ __forceinline__ void sts16(uint32_t addr, uint32_t v)
 // real parts into the yr tiles, imaginary parts into the yi tiles, each split into bf16 hi / lo.
 // `cell` = byte offset (in a 16 KB tile) of this lane's 2-byte cell in row 0 of the warp's slab for each swizzle
 // phase; tile order in the slot: [yr hi | yr lo | yi hi | yi lo] (single pass: [yr | yi]).
-template <int MT>
-__device__ __forceinline__ void fir_compute_store_sym(const FirRegs<MT>& rg, uint32_t slot, const uint32_t (&cell)[8],
-                                                      uint32_t sub_xor, bool split, bool fp16)
+template <int MT, bool SPLIT>
+__device__ __forceinline__ void fir_compute_store_sym(const FirRegs<MT>& rg, const uint32_t (&cell)[8], bool fp16)
 {
+    // cell[j]: shared-memory address of this lane's 2-byte cell in row 0 of the warp's slab of the yr hi tile, for
+    // swizzle phase j (slot base, sub-step and lane already folded in): everything below is an immediate offset
     constexpr int WA = FirRegs<MT>::WA;
     constexpr int FG = 8;
-    const uint32_t im_off = split ? 2u * A_PART_BYTES : (uint32_t)A_PART_BYTES;
+    constexpr uint32_t im_off = SPLIT ? 2u * A_PART_BYTES : (uint32_t)A_PART_BYTES;
+    constexpr bool split = SPLIT;
 #pragma unroll
     for (int i0 = 0; i0 < FPW; i0 += FG) {
         float2 y[FG];
@@ -91,9 +99,9 @@ __device__ __forceinline__ void fir_compute_store_sym(const FirRegs<MT>& rg, uin
         for (int g = 0; g < FG; ++g) {
             const int i = i0 + g;
             uint32_t hb;
-            if (fp16) { const __half2 hh = __floats2half2_rn(y[g].x, y[g].y); hb = *reinterpret_cast<const uint32_t*>(&hh); }
+            if (!SPLIT && fp16) { const __half2 hh = __floats2half2_rn(y[g].x, y[g].y); hb = *reinterpret_cast<const uint32_t*>(&hh); }
             else { const __nv_bfloat162 hi = __floats2bfloat162_rn(y[g].x, y[g].y); hb = *reinterpret_cast<const uint32_t*>(&hi); }
-            const uint32_t addr = slot + (cell[i & 7] ^ sub_xor) + (uint32_t)i * 128u;
+            const uint32_t addr = cell[i & 7] + (uint32_t)i * 128u;
             sts16(addr, hb);
             sts16(addr + im_off, hb >> 16);
             if (split) {
@@ -108,7 +116,148 @@ __device__ __forceinline__ void fir_compute_store_sym(const FirRegs<MT>& rg, uin
     }
 }
 
-template <int MT>
+struct EpiCtx {
+    uint32_t t_full0, t_full1, t_empty0, t_empty1;   // shared-memory addresses of the accumulator barriers
+    uint32_t stage, tmem_base, rank;
+    int cl, n_cl;
+};
+
+// Epilogue of one lane quarter q (a warp): see the comment inside.  Shared by both kernels of this file.
+__device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtensorMap* tmap_out, const CUtensorMap* tmap_out2,
+                                             const EpiCtx& e, const int q, const int lane)
+{
+    constexpr int CG = UMMA_CG;
+    const int P = prm.P, half = P >> 1, npg = prm.n_passes;
+    // ============================ epilogue ==============================================
+    // Lane = frame (TMEM lane); a step takes 32 accumulator columns = 16 bins kb .. kb+15 from D1 (U, Z) and
+    // D2 (W, V).  Forward tile: bins kb .. kb+15, stored by TMA at column 2 kb.  The mirrored bins P-kb-j are
+    // one bin off any 16-byte-aligned tile (TMA needs 16-byte-aligned box starts), so the mirrored tile is
+    // the ALIGNED group P-kb-16 .. P-kb-1 = the mirrors of j = 1 .. 16, j = 16 being the first bin of the next
+    // step (two extra TMEM columns are read for it).  What does not fit that scheme is stored from registers,
+    // 8 bytes per row: the mirror of a pass's first bin (j = 0; none for bin 0, whose "mirror" is bin 0 itself),
+    // the mirror of j = 15 in the pass's last step (whose tile goes out 28 floats wide through a second map,
+    // because j = 16 belongs to the next pass), and the Nyquist bin.
+            const uint32_t sb_f = e.stage + (uint32_t)q * SY_STAGE, sb_m = sb_f + 4096u;
+    const uint32_t taddr = e.tmem_base + ((uint32_t)(q * 32) << 16);
+    const uint32_t rowoff = (uint32_t)lane * 128u, sw = (uint32_t)lane & 7u;
+    uint32_t tf_phase = 0;
+    long long pe_w = 0, pe_d = 0, pe_x, pe_tot = SY_NOW();
+    for (int w = e.cl; w < prm.total_work; w += e.n_cl) {
+        const int tile = w / npg;
+        const int k0 = (w % npg) * SY_BINS;
+        const int ncol = 2 * min(SY_BINS, half - k0);
+        const int s = tile / prm.tiles_per_stream;
+        const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + e.rank * BM + q * 32;
+        const bool row_ok = lane < (int)min(32LL, prm.F - row0);
+        float* const orow = prm.out + ((long long)s * prm.F + row0 + lane) * (2LL * P);
+        for (int ks = 0; ks < prm.k_splits; ++ks) {
+            if (ks > 0 && lane == 0) bulk_wait<0>();          // the previous chain's stores to this tile are complete
+            pe_x = SY_NOW();
+            mbar_wait<256>(e.t_full0, tf_phase);
+            mbar_wait<256>(e.t_full1, tf_phase);
+            pe_w += SY_NOW() - pe_x; pe_x = SY_NOW();
+            tf_phase ^= 1u;
+            tc_fence_after();
+            // one bin (complex value) straight from registers: plain store for the first chain, fp32 add at L2 after
+            auto put = [&](int bin, float re, float im) {
+                if (row_ok && !SY_DBG(16)) {
+                    float2* g = reinterpret_cast<float2*>(orow + 2 * bin);
+                    if (ks > 0) atomicAdd(g, make_float2(re, im)); else *g = make_float2(re, im);
+                }
+            };
+            uint32_t r1[32], r2[32], e1[2] = {0u, 0u}, e2[2] = {0u, 0u};
+            tmem_ld32(taddr, r1);
+            tmem_ld32(taddr + 256u, r2);
+            if (32 < ncol) { tmem_ld2(taddr + 32u, e1); tmem_ld2(taddr + 256u + 32u, e2); }
+            for (int cb = 0; cb < ncol; cb += 32) {
+                const int kb = k0 + (cb >> 1);
+                const bool last = cb + 32 >= ncol;
+                tmem_ld_wait();
+                if (last) {
+                    // both accumulators have been read out completely: hand them back to the MMA warps
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {
+                        arrive_leader<CG>(e.t_empty0, e.rank, 0);
+                        arrive_leader<CG>(e.t_empty1, e.rank, 0);
+                    }
+                    pe_d += SY_NOW() - pe_x;                  // accumulator wait -> release: the exposed drain
+                }
+#define SY_F(v) __uint_as_float(v)
+                if (kb == 0) {
+                    // bin 0: its sine column carries (-1)^p, i.e. r1[1] + i r2[1] = X[P/2] (unpaired)
+                    put(half, SY_F(r1[1]), SY_F(r2[1]));
+                    r1[1] = 0u; r2[1] = 0u;                  // V = Z = 0 for bin 0: X[0] = U + i W
+                } else if (cb == 0) {
+                    put(P - kb, SY_F(r1[0]) - SY_F(r2[1]), SY_F(r2[0]) + SY_F(r1[1]));          // mirror of j = 0
+                }
+                if (last) put(P - kb - 15, SY_F(r1[30]) - SY_F(r2[31]), SY_F(r2[30]) + SY_F(r1[31]));   // mirror of j = 15
+                if (lane == 0) bulk_wait_read<1>();           // the forward tile of the previous step has been read
+                __syncwarp();
+#pragma unroll
+                for (int g = 0; g < 8; ++g) {
+                    const float U0 = SY_F(r1[4 * g]), Z0 = SY_F(r1[4 * g + 1]), U1 = SY_F(r1[4 * g + 2]), Z1 = SY_F(r1[4 * g + 3]);
+                    const float W0 = SY_F(r2[4 * g]), V0 = SY_F(r2[4 * g + 1]), W1 = SY_F(r2[4 * g + 2]), V1 = SY_F(r2[4 * g + 3]);
+                    sts128(sb_f + rowoff + (((uint32_t)g ^ sw) << 4), __float_as_uint(U0 + V0), __float_as_uint(W0 - Z0),
+                           __float_as_uint(U1 + V1), __float_as_uint(W1 - Z1));
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) {
+                    if (SY_DBG(32)) { }
+                    else if (ks == 0) tma_store_3d(tmap_out, sb_f, 2 * kb, (int)row0, s);
+                    else              tma_reduce_add_3d(tmap_out, sb_f, 2 * kb, (int)row0, s);
+                    bulk_commit();
+                    bulk_wait_read<1>();                      // the mirrored tile of the previous step has been read
+                }
+                __syncwarp();
+                // mirrored tile: position t <-> bin P-kb-16+t <-> j = 16 - t; 16-byte chunk c holds j = 16-2c, 15-2c
+                // = accumulator columns 32-4c .. 33-4c and 30-4c .. 31-4c (columns 32, 33 = e1 / e2)
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    const float Ua = SY_F(c ? r1[32 - 4 * c] : e1[0]), Za = SY_F(c ? r1[33 - 4 * c] : e1[1]);
+                    const float Wa = SY_F(c ? r2[32 - 4 * c] : e2[0]), Va = SY_F(c ? r2[33 - 4 * c] : e2[1]);
+                    const float Ub = SY_F(r1[30 - 4 * c]), Zb = SY_F(r1[31 - 4 * c]);
+                    const float Wb = SY_F(r2[30 - 4 * c]), Vb = SY_F(r2[31 - 4 * c]);
+                    if (!last)
+                        sts128(sb_m + rowoff + (((uint32_t)c ^ sw) << 4), __float_as_uint(Ua - Va), __float_as_uint(Wa + Za),
+                               __float_as_uint(Ub - Vb), __float_as_uint(Wb + Zb));
+                    else if (c > 0)                              // last step of the pass: dense rows of 28 floats, positions 2 .. 15
+                        sts128(sb_m + (uint32_t)lane * 112u + (uint32_t)(c - 1) * 16u, __float_as_uint(Ua - Va), __float_as_uint(Wa + Za),
+                               __float_as_uint(Ub - Vb), __float_as_uint(Wb + Zb));
+                }
+#undef SY_F
+                if (!last) {
+                    tmem_ld32(taddr + cb + 32, r1);
+                    tmem_ld32(taddr + 256u + cb + 32, r2);
+                    if (cb + 64 < ncol) { tmem_ld2(taddr + cb + 64, e1); tmem_ld2(taddr + 256u + cb + 64, e2); }
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) {
+                    if (SY_DBG(16)) { }
+                    else if (!last) {
+                        const int cm = 2 * (P - kb - 16);
+                        if (ks == 0) tma_store_3d(tmap_out, sb_m, cm, (int)row0, s);
+                        else         tma_reduce_add_3d(tmap_out, sb_m, cm, (int)row0, s);
+                    } else {
+                        const int cm = 2 * (P - kb - 14);
+                        if (ks == 0) tma_store_3d(tmap_out2, sb_m, cm, (int)row0, s);
+                        else         tma_reduce_add_3d(tmap_out2, sb_m, cm, (int)row0, s);
+                    }
+                    bulk_commit();
+                }
+            }
+        }
+    }
+    if (lane == 0) bulk_wait<0>();                            // staging tiles must outlive their TMA reads
+    if (SY_PROF && prm.prof && q == 0 && lane == 0) {
+        unsigned long long* pp = prm.prof + blockIdx.x * 16 + 8;
+        pp[0] = SY_NOW() - pe_tot; pp[1] = pe_w; pp[2] = pe_d;
+    }
+}
+
+template <int MT, int PARTS>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_out,
                const __grid_constant__ CUtensorMap tmap_out2, const SymParams prm)
@@ -122,8 +271,8 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
 
     constexpr int CG = UMMA_CG;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int parts = prm.parts;
-    const uint32_t a_slot_bytes = 2u * parts * A_PART_BYTES;
+    constexpr int parts = PARTS;                                      // 2: bf16x3 (hi + lo tiles), 1: single pass
+    constexpr uint32_t a_slot_bytes = 2u * parts * A_PART_BYTES;
     const uint32_t n_a = (uint32_t)SY_A_RING / a_slot_bytes;            // 2 (bf16x3) or 4 (single pass)
     const int P = prm.P;
     const int n_kc = P / KC;
@@ -192,6 +341,7 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
             RingPos a, b;
             uint32_t te_phase = 0;
             const uint32_t d = tmem_base + (uint32_t)h * 256u;
+            long long pm_a = 0, pm_b = 0, pm_t = 0, pm_x, pm_tot = SY_NOW();
             for (int w = cl; w < prm.total_work; w += n_cl) {
                 const int k0 = (w % npg) * SY_BINS;
                 const int nw = 2 * min(SY_BINS, half - k0);
@@ -199,18 +349,18 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
                 for (int ks = 0; ks < prm.k_splits; ++ks) {
                     const int kc_begin = ks * prm.kc_per_split, kc_end = min(n_kc, kc_begin + prm.kc_per_split);
                     for (int kc = kc_begin; kc < kc_end; ++kc) {
-                        mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                        pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase); pm_a += SY_NOW() - pm_x;
                         tc_fence_after();
                         const uint32_t a_hi = smem_u32(a_ring + a.idx * a_slot_bytes) + (uint32_t)h * (uint32_t)parts * A_PART_BYTES;
                         const uint32_t a_lo = a_hi + A_PART_BYTES;
                         if (kc == kc_begin) {
                             // first write into this accumulator: wait until the epilogue has drained it
-                            mbar_wait(smem_u32(&ctl->t_empty[h]), te_phase ^ 1u);
+                            pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->t_empty[h]), te_phase ^ 1u); pm_t += SY_NOW() - pm_x;
                             te_phase ^= 1u;
                             tc_fence_after();
                         }
                         // ---- B_hi: (A_lo x B_hi) then (A_hi x B_hi)
-                        mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase);
+                        pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
                         tc_fence_after();
                         if (lane == 0) {
                             const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * SY_B_ENTRY));
@@ -229,7 +379,7 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
                         b.advance(SY_B_ENTRIES);
                         // ---- B_lo: (A_hi x B_lo)
                         if (parts > 1) {
-                            mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase);
+                            pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
                             tc_fence_after();
                             if (lane == 0) {
                                 const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * SY_B_ENTRY));
@@ -250,128 +400,17 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
                     }
                 }
             }
-        }
-    } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
-        // ============================ epilogue ==============================================
-        // Lane = frame (TMEM lane); a step takes 32 accumulator columns = 16 bins kb .. kb+15 from D1 (U, Z) and
-        // D2 (W, V).  Forward tile: bins kb .. kb+15, stored by TMA at column 2 kb.  The mirrored bins P-kb-j are
-        // one bin off any 16-byte-aligned tile (TMA needs 16-byte-aligned box starts), so the mirrored tile is
-        // the ALIGNED group P-kb-16 .. P-kb-1 = the mirrors of j = 1 .. 16, j = 16 being the first bin of the next
-        // step (two extra TMEM columns are read for it).  What does not fit that scheme is stored from registers,
-        // 8 bytes per row: the mirror of a pass's first bin (j = 0; none for bin 0, whose "mirror" is bin 0 itself),
-        // the mirror of j = 15 in the pass's last step (whose tile goes out 28 floats wide through a second map,
-        // because j = 16 belongs to the next pass), and the Nyquist bin.
-        const int q = warp - EPI_WARP0;
-        const uint32_t sb_f = smem_u32(stage) + (uint32_t)q * SY_STAGE, sb_m = sb_f + 4096u;
-        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
-        const uint32_t rowoff = (uint32_t)lane * 128u, sw = (uint32_t)lane & 7u;
-        uint32_t tf_phase = 0;
-        for (int w = cl; w < prm.total_work; w += n_cl) {
-            const int tile = w / npg;
-            const int k0 = (w % npg) * SY_BINS;
-            const int ncol = 2 * min(SY_BINS, half - k0);
-            const int s = tile / prm.tiles_per_stream;
-            const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + rank * BM + q * 32;
-            const bool row_ok = lane < (int)min(32LL, prm.F - row0);
-            float* const orow = prm.out + ((long long)s * prm.F + row0 + lane) * (2LL * P);
-            for (int ks = 0; ks < prm.k_splits; ++ks) {
-                if (ks > 0 && lane == 0) bulk_wait<0>();          // the previous chain's stores to this tile are complete
-                mbar_wait<256>(smem_u32(&ctl->t_full[0]), tf_phase);
-                mbar_wait<256>(smem_u32(&ctl->t_full[1]), tf_phase);
-                tf_phase ^= 1u;
-                tc_fence_after();
-                // one bin (complex value) straight from registers: plain store for the first chain, fp32 add at L2 after
-                auto put = [&](int bin, float re, float im) {
-                    if (row_ok && !SY_DBG(16)) {
-                        float2* g = reinterpret_cast<float2*>(orow + 2 * bin);
-                        if (ks > 0) atomicAdd(g, make_float2(re, im)); else *g = make_float2(re, im);
-                    }
-                };
-                uint32_t r1[32], r2[32], e1[2] = {0u, 0u}, e2[2] = {0u, 0u};
-                tmem_ld32(taddr, r1);
-                tmem_ld32(taddr + 256u, r2);
-                if (32 < ncol) { tmem_ld2(taddr + 32u, e1); tmem_ld2(taddr + 256u + 32u, e2); }
-                for (int cb = 0; cb < ncol; cb += 32) {
-                    const int kb = k0 + (cb >> 1);
-                    const bool last = cb + 32 >= ncol;
-                    tmem_ld_wait();
-                    if (last) {
-                        // both accumulators have been read out completely: hand them back to the MMA warps
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) {
-                            arrive_leader<CG>(smem_u32(&ctl->t_empty[0]), rank, leader);
-                            arrive_leader<CG>(smem_u32(&ctl->t_empty[1]), rank, leader);
-                        }
-                    }
-#define SY_F(v) __uint_as_float(v)
-                    if (kb == 0) {
-                        // bin 0: its sine column carries (-1)^p, i.e. r1[1] + i r2[1] = X[P/2] (unpaired)
-                        put(half, SY_F(r1[1]), SY_F(r2[1]));
-                        r1[1] = 0u; r2[1] = 0u;                  // V = Z = 0 for bin 0: X[0] = U + i W
-                    } else if (cb == 0) {
-                        put(P - kb, SY_F(r1[0]) - SY_F(r2[1]), SY_F(r2[0]) + SY_F(r1[1]));          // mirror of j = 0
-                    }
-                    if (last) put(P - kb - 15, SY_F(r1[30]) - SY_F(r2[31]), SY_F(r2[30]) + SY_F(r1[31]));   // mirror of j = 15
-                    if (lane == 0) bulk_wait_read<1>();           // the forward tile of the previous step has been read
-                    __syncwarp();
-#pragma unroll
-                    for (int g = 0; g < 8; ++g) {
-                        const float U0 = SY_F(r1[4 * g]), Z0 = SY_F(r1[4 * g + 1]), U1 = SY_F(r1[4 * g + 2]), Z1 = SY_F(r1[4 * g + 3]);
-                        const float W0 = SY_F(r2[4 * g]), V0 = SY_F(r2[4 * g + 1]), W1 = SY_F(r2[4 * g + 2]), V1 = SY_F(r2[4 * g + 3]);
-                        sts128(sb_f + rowoff + (((uint32_t)g ^ sw) << 4), __float_as_uint(U0 + V0), __float_as_uint(W0 - Z0),
-                               __float_as_uint(U1 + V1), __float_as_uint(W1 - Z1));
-                    }
-                    fence_proxy_async();
-                    __syncwarp();
-                    if (lane == 0) {
-                        if (SY_DBG(32)) { }
-                        else if (ks == 0) tma_store_3d(&tmap_out, sb_f, 2 * kb, (int)row0, s);
-                        else              tma_reduce_add_3d(&tmap_out, sb_f, 2 * kb, (int)row0, s);
-                        bulk_commit();
-                        bulk_wait_read<1>();                      // the mirrored tile of the previous step has been read
-                    }
-                    __syncwarp();
-                    // mirrored tile: position t <-> bin P-kb-16+t <-> j = 16 - t; 16-byte chunk c holds j = 16-2c, 15-2c
-                    // = accumulator columns 32-4c .. 33-4c and 30-4c .. 31-4c (columns 32, 33 = e1 / e2)
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) {
-                        const float Ua = SY_F(c ? r1[32 - 4 * c] : e1[0]), Za = SY_F(c ? r1[33 - 4 * c] : e1[1]);
-                        const float Wa = SY_F(c ? r2[32 - 4 * c] : e2[0]), Va = SY_F(c ? r2[33 - 4 * c] : e2[1]);
-                        const float Ub = SY_F(r1[30 - 4 * c]), Zb = SY_F(r1[31 - 4 * c]);
-                        const float Wb = SY_F(r2[30 - 4 * c]), Vb = SY_F(r2[31 - 4 * c]);
-                        if (!last)
-                            sts128(sb_m + rowoff + (((uint32_t)c ^ sw) << 4), __float_as_uint(Ua - Va), __float_as_uint(Wa + Za),
-                                   __float_as_uint(Ub - Vb), __float_as_uint(Wb + Zb));
-                        else if (c > 0)                              // last step of the pass: dense rows of 28 floats, positions 2 .. 15
-                            sts128(sb_m + (uint32_t)lane * 112u + (uint32_t)(c - 1) * 16u, __float_as_uint(Ua - Va), __float_as_uint(Wa + Za),
-                                   __float_as_uint(Ub - Vb), __float_as_uint(Wb + Zb));
-                    }
-#undef SY_F
-                    if (!last) {
-                        tmem_ld32(taddr + cb + 32, r1);
-                        tmem_ld32(taddr + 256u + cb + 32, r2);
-                        if (cb + 64 < ncol) { tmem_ld2(taddr + cb + 64, e1); tmem_ld2(taddr + 256u + cb + 64, e2); }
-                    }
-                    fence_proxy_async();
-                    __syncwarp();
-                    if (lane == 0) {
-                        if (SY_DBG(16)) { }
-                        else if (!last) {
-                            const int cm = 2 * (P - kb - 16);
-                            if (ks == 0) tma_store_3d(&tmap_out, sb_m, cm, (int)row0, s);
-                            else         tma_reduce_add_3d(&tmap_out, sb_m, cm, (int)row0, s);
-                        } else {
-                            const int cm = 2 * (P - kb - 14);
-                            if (ks == 0) tma_store_3d(&tmap_out2, sb_m, cm, (int)row0, s);
-                            else         tma_reduce_add_3d(&tmap_out2, sb_m, cm, (int)row0, s);
-                        }
-                        bulk_commit();
-                    }
-                }
+            if (SY_PROF && prm.prof && lane == 0) {
+                unsigned long long* pp = prm.prof + blockIdx.x * 16 + h * 4;
+                pp[0] = SY_NOW() - pm_tot; pp[1] = pm_a; pp[2] = pm_b; pp[3] = pm_t;
             }
         }
-        if (lane == 0) bulk_wait<0>();                            // staging tiles must outlive their TMA reads
+    } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
+        EpiCtx ec;
+        ec.t_full0 = smem_u32(&ctl->t_full[0]); ec.t_full1 = smem_u32(&ctl->t_full[1]);
+        ec.t_empty0 = smem_u32(&ctl->t_empty[0]); ec.t_empty1 = smem_u32(&ctl->t_empty[1]);
+        ec.stage = smem_u32(stage); ec.tmem_base = tmem_base; ec.rank = rank; ec.cl = cl; ec.n_cl = n_cl;
+        sym_epilogue(prm, &tmap_out, &tmap_out2, ec, warp - EPI_WARP0, lane);
     } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ FIR producers =========================================
         // A chunk is 64 complex columns = two sub-steps of 32 (one complex sample per lane, 16 frames per
@@ -382,15 +421,14 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
         // byte offset of this lane's 2-byte cell in row 0 of the warp's slab, per swizzle phase (row & 7), for
         // sub-step 0: complex column lane -> 16-byte chunk lane >> 3, stored at chunk ^ (row & 7); sub-step 1 is
         // chunk + 4, i.e. the same offset with bit 6 flipped
-        uint32_t cell[8];
+        uint32_t cell0[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j)
-            cell[j] = (uint32_t)(pw * FPW) * 128u + ((((uint32_t)lane >> 3) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 7u) * 2u;
+            cell0[j] = a_ring_s + (uint32_t)(pw * FPW) * 128u + ((((uint32_t)lane >> 3) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 7u) * 2u;
         constexpr int WA = MT > 0 ? MT : 1;
         const float* const window = prm.window;
         const int M = prm.M;
         const long long K = 2LL * P, nblk = prm.NBLK;
-        const bool split = parts > 1;
         FirRegs<MT> rg;
         int w = cl, st = 0;                                   // st = 2 * kc + sub
         const int n_st = 2 * n_kc;
@@ -410,6 +448,7 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
             if (interior) fir_load<MT, false, false>(rg, window, P, M, K, nblk, xs + sst * KC, c0, f0);
             else          fir_load<MT, false, true>(rg, window, P, M, K, nblk, xs + sst * KC, c0, f0);
         };
+        long long pq_w = 0, pq_c = 0, pq_f = 0, pq_x, pq_tot = SY_NOW();
         bool have = w < prm.total_work;
         if (have) { set_tile(w); load(st); }
         while (have) {
@@ -418,19 +457,33 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
             const bool have2 = w2 < prm.total_work;
             const uint32_t slot_i = n % n_a, slot_ph = (n / n_a) & 1u;
             const int sub = st & 1;
+            pq_x = SY_NOW();
             if (sub == 0) mbar_wait(smem_u32(&ctl->a_empty[slot_i]), slot_ph ^ 1);
-            fir_compute_store_sym<MT>(rg, a_ring_s + slot_i * a_slot_bytes, cell, sub ? 64u : 0u, split, prm.fp16 != 0);
+            pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
+            {
+                uint32_t cell[8];
+                const uint32_t so = slot_i * a_slot_bytes, sx = sub ? 64u : 0u;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) cell[j] = (cell0[j] ^ sx) + so;     // bit 6 of a 1024-byte-aligned base is clear
+                fir_compute_store_sym<MT, (PARTS > 1)>(rg, cell, prm.fp16 != 0);
+            }
             if (have2) {
                 if (w2 != w) set_tile(w2);
                 load(st2);
             }
+            pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
             if (sub == 1) {
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[slot_i]));
                 ++n;
             }
+            pq_f += SY_NOW() - pq_x;
             w = w2; st = st2; have = have2;
+        }
+        if (SY_PROF && prm.prof && pw == 0 && lane == 0) {
+            unsigned long long* pp = prm.prof + blockIdx.x * 16 + 12;
+            pp[0] = SY_NOW() - pq_tot; pp[1] = pq_w; pp[2] = pq_c; pp[3] = pq_f;
         }
     }
 
@@ -440,15 +493,373 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
 }
 
 // =====================================================================================
+// pfb_symt_kernel: the same contraction with the INPUT WINDOW AND THE TAPS STAGED BY TMA (the north_star
+// sketch): per chunk of 32 complex columns the (128 + MT - 1) x 32 block of input
+// rows and the MT x 32 block of prototype-filter taps are bulk-copied into a two-slot shared-memory ring; the
+// FIR producers read their sliding window from shared memory (no long-latency global loads in the FIR warps,
+// every input row fetched from L2 once per CTA and chunk instead of once per 16-frame warp slab, taps once per
+// CTA instead of once per warp).  To make room the operand tiles are 32 contraction elements wide (64-byte
+// rows, SWIZZLE_64B): A slot = 4 x 8 KB, B entry = 8 KB per CTA, two K = 16 MMAs per tile and product.
+//   shared memory: A ring 64 KB (2 slots; 4 for the single pass) | B ring 48 KB (6 entries = 3 chunks) |
+//                  input ring 2 x 38 KB | epilogue staging 32 KB
+//   warps: 0-7 FIR producers, 8-11 epilogue, 12 TMA (twiddles), 13 / 15 MMA issuers, 14 TMEM allocation + TMA (input)
+// =====================================================================================
+constexpr int ST_KC = 32;                                  // contraction elements (complex columns) per chunk
+constexpr int ST_TILE = BM * ST_KC * 2;                    // 8 KB: 128 rows x 64 B
+constexpr int ST_A_RING = 64 * 1024;
+constexpr int ST_B_ENTRY = (NSUB / UMMA_CG) * ST_KC * 2;   // 8 KB per CTA
+constexpr int ST_B_ENTRIES = 6;
+constexpr int ST_IN_ROWS_MAX = BM + 15;                    // 143 input rows of 256 B
+constexpr int ST_IN_TAPS = ST_IN_ROWS_MAX * 256;           // byte offset of the taps block in an input slot
+constexpr int ST_IN_SLOT = 38 * 1024;                      // 36 608 B of rows + 2 KB of taps, 1024-byte multiple
+constexpr int ST_IN_SLOTS = 2;
+
+struct SmemCtlT {
+    uint64_t a_full[4], a_empty[4];
+    uint64_t b_full[8], b_empty[8];
+    uint64_t in_full[2], in_empty[2];
+    uint64_t t_full[2], t_empty[2];
+    uint32_t tmem_base;
+};
+constexpr size_t ST_SMEM_BYTES = ST_A_RING + ST_B_ENTRIES * ST_B_ENTRY + ST_IN_SLOTS * ST_IN_SLOT + 4 * SY_STAGE + sizeof(SmemCtlT);
+static_assert(ST_SMEM_BYTES <= 232448, "exceeds the 227 KB shared memory opt-in limit");
+
+__device__ __forceinline__ float2 lds_f2(uint32_t addr)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds_f1(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
+template <int MT, int PARTS>
+__global__ void __launch_bounds__(UMMA_THREADS, 1)
+pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_out,
+                const __grid_constant__ CUtensorMap tmap_out2, const __grid_constant__ CUtensorMap tmap_x,
+                const __grid_constant__ CUtensorMap tmap_w, const SymParams prm)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    if ((smem_u32(smem) & 1023u) != 0) __trap();
+    uint8_t* a_ring = smem;
+    uint8_t* b_ring = smem + ST_A_RING;
+    uint8_t* in_ring = b_ring + ST_B_ENTRIES * ST_B_ENTRY;
+    uint8_t* stage = in_ring + ST_IN_SLOTS * ST_IN_SLOT;
+    SmemCtlT* ctl = reinterpret_cast<SmemCtlT*>(stage + 4 * SY_STAGE);
+
+    constexpr int CG = UMMA_CG;
+    constexpr int WA = MT > 0 ? MT : 1;
+    constexpr int IN_ROWS = BM + WA - 1;                               // input rows one CTA needs per chunk
+    constexpr int parts = PARTS;
+    constexpr uint32_t a_slot_bytes = 2u * parts * ST_TILE;            // [yr hi | yr lo | yi hi | yi lo] or [yr | yi]
+    constexpr uint32_t n_a = (uint32_t)ST_A_RING / a_slot_bytes;       // 2 (bf16x3) or 4 (single pass)
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int P = prm.P, M = prm.M;
+    const int n_kc = P / ST_KC;
+    const int half = P >> 1;
+    const uint32_t rank = cluster_ctarank();
+    constexpr uint32_t leader = 0;
+    constexpr uint16_t pair_mask = 3;
+    const int cl = blockIdx.x / CG, n_cl = gridDim.x / CG;
+    const int npg = prm.n_passes;
+    const uint32_t b_box_bytes = (uint32_t)(P < NSUB ? P : NSUB) / CG * ST_KC * 2;
+
+    if (warp == TMA_WARP && lane == 0) {
+        prefetch_tmap(&tmap_b); prefetch_tmap(&tmap_out); prefetch_tmap(&tmap_out2); prefetch_tmap(&tmap_x);
+        if (MT > 0) prefetch_tmap(&tmap_w);
+        for (int i = 0; i < 4; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), 2); }
+        for (int i = 0; i < ST_B_ENTRIES; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 2); }
+        for (int i = 0; i < ST_IN_SLOTS; ++i) { mbar_init(smem_u32(&ctl->in_full[i]), 1); mbar_init(smem_u32(&ctl->in_empty[i]), N_PROD_WARPS); }
+        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
+        fence_mbar_init();
+    }
+    if (warp == ALLOC_WARP) {
+        tmem_alloc<CG>(smem_u32(&ctl->tmem_base), 512);
+        tmem_relinquish<CG>();
+    }
+    tc_fence_before();
+    cluster_sync();
+    tc_fence_after();
+    const uint32_t tmem_base = ctl->tmem_base;
+
+    if (warp == ALLOC_WARP) {
+        // ============================ TMA producer: input rows + taps ========================
+        if (lane == 0) {
+            RingPos in;
+            for (int w = cl; w < prm.total_work; w += n_cl) {
+                const int tile = w / npg;
+                const int s = tile / prm.tiles_per_stream;
+                // first input row of this CTA's window: frame f0 uses rows f0 + M - WA .. f0 + M - 1 (taps m >= M are zero)
+                const int r0 = (tile % prm.tiles_per_stream) * (BM * CG) + (int)rank * BM + M - WA;
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    mbar_wait<64>(smem_u32(&ctl->in_empty[in.idx]), in.phase ^ 1);
+                    const uint32_t bar = smem_u32(&ctl->in_full[in.idx]);
+                    const uint32_t dst = smem_u32(in_ring + in.idx * ST_IN_SLOT);
+                    mbar_expect_tx(bar, (uint32_t)IN_ROWS * 256u + (MT > 0 ? (uint32_t)MT * 128u : 0u));
+                    tma_load_3d(dst, &tmap_x, bar, kc * 2 * ST_KC, r0, s);       // rows outside [0, NB) arrive as zeros
+                    if (MT > 0) tma_load_2d(dst + ST_IN_TAPS, &tmap_w, bar, kc * ST_KC, 0);   // rows >= M arrive as zeros
+                    in.advance(ST_IN_SLOTS);
+                }
+            }
+        }
+    } else if (warp == TMA_WARP) {
+        // ============================ TMA producer: [C|S] tiles, hi then lo per chunk ===============
+        if (lane == 0) {
+            RingPos b;
+            for (int w = cl; w < prm.total_work; w += n_cl) {
+                const int k0 = (w % npg) * SY_BINS;
+                const int nw = 2 * min(SY_BINS, half - k0);
+                for (int kc = 0; kc < n_kc; ++kc)
+                    for (int part = 0; part < parts; ++part) {
+                        mbar_wait<64>(smem_u32(&ctl->b_empty[b.idx]), b.phase ^ 1);
+                        const uint32_t bar = smem_u32(&ctl->b_full[b.idx]);
+                        const uint32_t dst = smem_u32(b_ring + b.idx * ST_B_ENTRY);
+                        const int row = part * P + 2 * k0 + (int)rank * (nw / CG);
+                        if (rank == 0) mbar_expect_tx(bar, 2 * b_box_bytes);
+                        tma_load_2d_cg2(dst, &tmap_b, mapa_u32(bar, leader), kc * ST_KC, row);
+                        b.advance(ST_B_ENTRIES);
+                    }
+            }
+        }
+    } else if (warp == MMA_WARP || warp == MMA_WARP2) {
+        // ============================ MMA issuers (as pfb_sym_kernel, two K = 16 steps per tile) ==========
+        const int h = warp == MMA_WARP ? 0 : 1;
+        if (rank != 0 && h == 0) {
+            RingPos a;
+            for (int w = cl; w < prm.total_work; w += n_cl)
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                    if (lane == 0) mbar_arrive_cluster(smem_u32(&ctl->a_full[a.idx]), leader);
+                    __syncwarp();
+                    a.advance(n_a);
+                }
+        }
+        if (rank == 0) {
+            RingPos a, b;
+            uint32_t te_phase = 0;
+            const uint32_t d = tmem_base + (uint32_t)h * 256u;
+            long long pm_a = 0, pm_b = 0, pm_t = 0, pm_x, pm_tot = SY_NOW();
+            for (int w = cl; w < prm.total_work; w += n_cl) {
+                const int k0 = (w % npg) * SY_BINS;
+                const int nw = 2 * min(SY_BINS, half - k0);
+                const uint32_t idesc = idesc_bf16(BM * CG, nw, prm.fp16 != 0);
+                for (int ks = 0; ks < prm.k_splits; ++ks) {
+                    const int kc_begin = ks * prm.kc_per_split, kc_end = min(n_kc, kc_begin + prm.kc_per_split);
+                    for (int kc = kc_begin; kc < kc_end; ++kc) {
+                        pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase); pm_a += SY_NOW() - pm_x;
+                        tc_fence_after();
+                        const uint32_t a_hi = smem_u32(a_ring + a.idx * a_slot_bytes) + (uint32_t)h * (uint32_t)parts * ST_TILE;
+                        const uint32_t a_lo = a_hi + ST_TILE;
+                        if (kc == kc_begin) {
+                            pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->t_empty[h]), te_phase ^ 1u); pm_t += SY_NOW() - pm_x;
+                            te_phase ^= 1u;
+                            tc_fence_after();
+                        }
+                        pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
+                        tc_fence_after();
+                        if (lane == 0) {
+                            const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + b.idx * ST_B_ENTRY));
+                            uint32_t acc = kc > kc_begin;
+                            if (parts > 1) {
+                                const uint64_t ad = smem_desc_sw64(a_lo);
+#pragma unroll
+                                for (int k = 0; k < ST_KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                            }
+                            const uint64_t ad = smem_desc_sw64(a_hi);
+#pragma unroll
+                            for (int k = 0; k < ST_KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                            commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]), pair_mask);
+                        }
+                        __syncwarp();
+                        b.advance(ST_B_ENTRIES);
+                        if (parts > 1) {
+                            pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
+                            tc_fence_after();
+                            if (lane == 0) {
+                                const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + b.idx * ST_B_ENTRY));
+                                const uint64_t ad = smem_desc_sw64(a_hi);
+#pragma unroll
+                                for (int k = 0; k < ST_KC / 16; ++k) umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
+                                commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]), pair_mask);
+                            }
+                            __syncwarp();
+                            b.advance(ST_B_ENTRIES);
+                        }
+                        if (lane == 0) {
+                            commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
+                            if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[h]), pair_mask);
+                        }
+                        __syncwarp();
+                        a.advance(n_a);
+                    }
+                }
+            }
+            if (SY_PROF && prm.prof && lane == 0) {
+                unsigned long long* pp = prm.prof + blockIdx.x * 16 + h * 4;
+                pp[0] = SY_NOW() - pm_tot; pp[1] = pm_a; pp[2] = pm_b; pp[3] = pm_t;
+            }
+        }
+    } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
+        EpiCtx ec;
+        ec.t_full0 = smem_u32(&ctl->t_full[0]); ec.t_full1 = smem_u32(&ctl->t_full[1]);
+        ec.t_empty0 = smem_u32(&ctl->t_empty[0]); ec.t_empty1 = smem_u32(&ctl->t_empty[1]);
+        ec.stage = smem_u32(stage); ec.tmem_base = tmem_base; ec.rank = rank; ec.cl = cl; ec.n_cl = n_cl;
+        sym_epilogue(prm, &tmap_out, &tmap_out2, ec, warp - EPI_WARP0, lane);
+    } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
+        // ============================ FIR producers =========================================
+        // Warp pw owns frames 16 pw .. 16 pw + 15 of the CTA's tile, lane = complex column of the chunk.  Per
+        // chunk: wait for the staged rows, read the 16 + MT - 1 rows of the sliding window and the MT taps from
+        // shared memory, polyphase MAC in registers (Eq. (20)), split into bf16 hi / lo, de-interleave into the
+        // 64-byte-swizzled yr / yi tiles: row r, 16-byte chunk (lane >> 3) stored at chunk ^ ((r >> 1) & 3).
+        const int pw = warp - PROD_WARP0;
+        const uint32_t a_ring_s = smem_u32(a_ring), in_ring_s = smem_u32(in_ring);
+        uint32_t cell0[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            cell0[j] = a_ring_s + (uint32_t)(pw * FPW) * 64u + ((((uint32_t)lane >> 3) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 7u) * 2u;
+        constexpr uint32_t im_off = (uint32_t)parts * ST_TILE;
+        const uint32_t in_lane = in_ring_s + (uint32_t)(pw * FPW) * 256u + (uint32_t)lane * 8u;
+        const uint32_t tap_lane = in_ring_s + ST_IN_TAPS + (uint32_t)lane * 4u;
+        long long pq_w = 0, pq_c = 0, pq_f = 0, pq_x, pq_tot = SY_NOW();
+        RingPos in, a;
+        for (int w = cl; w < prm.total_work; w += n_cl)
+            for (int kc = 0; kc < n_kc; ++kc) {
+                pq_x = SY_NOW();
+                mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase);
+                pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
+                FirRegs<MT> rg;
+                {
+                    const uint32_t src = in_lane + in.idx * ST_IN_SLOT, tsrc = tap_lane + in.idx * ST_IN_SLOT;
+                    if (MT > 0) {
+#pragma unroll
+                        for (int m = 0; m < WA; ++m) { const float hh = lds_f1(tsrc + (uint32_t)m * 128u); rg.tap[m] = make_float2(hh, hh); }
+                    }
+#pragma unroll
+                    for (int j = 0; j < WA - 1 + FPW; ++j) rg.row[j] = lds_f2(src + (uint32_t)j * 256u);
+                }
+                pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
+                mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
+                pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
+                // polyphase MAC + split + de-interleaved store (as fir_compute_store_sym, 64-byte rows)
+                const uint32_t so = a.idx * a_slot_bytes;
+#pragma unroll
+                for (int i0 = 0; i0 < FPW; i0 += 8) {
+                    float2 yv[8];
+                    if (MT > 0) {
+#pragma unroll
+                        for (int g = 0; g < 8; ++g) yv[g] = fmul2(rg.tap[0], rg.row[i0 + g + WA - 1]);
+#pragma unroll
+                        for (int m = 1; m < WA; ++m)
+#pragma unroll
+                            for (int g = 0; g < 8; ++g) yv[g] = ffma2(rg.tap[m], rg.row[i0 + g + WA - 1 - m], yv[g]);
+                    } else {
+#pragma unroll
+                        for (int g = 0; g < 8; ++g) yv[g] = rg.row[i0 + g];
+                    }
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) {
+                        const int i = i0 + g;
+                        uint32_t hb;
+                        if (parts == 1 && prm.fp16) { const __half2 hh = __floats2half2_rn(yv[g].x, yv[g].y); hb = *reinterpret_cast<const uint32_t*>(&hh); }
+                        else { const __nv_bfloat162 hi = __floats2bfloat162_rn(yv[g].x, yv[g].y); hb = *reinterpret_cast<const uint32_t*>(&hi); }
+                        const uint32_t addr = cell0[(i >> 1) & 3] + so + (uint32_t)i * 64u;
+                        sts16(addr, hb);
+                        sts16(addr + im_off, hb >> 16);
+                        if (parts > 1) {
+                            const float lx = yv[g].x - __uint_as_float(hb << 16);
+                            const float ly = yv[g].y - __uint_as_float(hb & 0xffff0000u);
+                            const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
+                            const uint32_t lb = *reinterpret_cast<const uint32_t*>(&lo);
+                            sts16(addr + ST_TILE, lb);
+                            sts16(addr + im_off + ST_TILE, lb >> 16);
+                        }
+                    }
+                }
+                // the window has been consumed: hand the input slot back to the TMA warp
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
+                in.advance(ST_IN_SLOTS);
+                pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[a.idx]));
+                a.advance(n_a);
+                pq_f += SY_NOW() - pq_x;
+            }
+        if (SY_PROF && prm.prof && pw == 0 && lane == 0) {
+            unsigned long long* pp = prm.prof + blockIdx.x * 16 + 12;
+            pp[0] = SY_NOW() - pq_tot; pp[1] = pq_w; pp[2] = pq_c; pp[3] = pq_f;
+        }
+    }
+
+    tc_fence_before();
+    cluster_sync();
+    if (warp == ALLOC_WARP) tmem_dealloc<CG>(tmem_base, 512);
+}
+
+// =====================================================================================
 // Host side
 // =====================================================================================
 bool sym_supported(int P) { return P >= 64 && P <= kMaxP && P % 64 == 0; }
 
-template <int MT>
+template <int MT, int PARTS>
+static tina_status launch_symt(DevCtx* ctx, const Plan* plan, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
+                               const CUtensorMap& tmap_x, const CUtensorMap& tmap_w, const SymParams& prm, int grid, cudaStream_t st)
+{
+    auto kern = pfb_symt_kernel<MT, PARTS>;
+    tina_status as = ensure_smem(ctx, reinterpret_cast<const void*>(kern), (int)ST_SMEM_BYTES, "cudaFuncSetAttribute(pfb_symt_kernel)");
+    if (as != TINA_OK) return as;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(UMMA_THREADS);
+    cfg.dynamicSmemBytes = ST_SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = UMMA_CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    SymParams prm2 = prm;
+#ifdef TINA_DEV
+    const bool prof = options().prof;
+    if (prof) {
+        cudaError_t pe = cudaMalloc(&prm2.prof, (size_t)grid * 16 * 8);
+        if (pe == cudaSuccess) pe = cudaMemsetAsync(prm2.prof, 0, (size_t)grid * 16 * 8, st);
+        if (pe != cudaSuccess) { if (prm2.prof) cudaFree(prm2.prof); return check_cuda(pe, "TINA_PROF counter buffer"); }
+    }
+#endif
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, plan->tmap32, tmap_out, tmap_out2, tmap_x, tmap_w, prm2);
+#ifdef TINA_DEV
+    if (prof) {
+        std::vector<unsigned long long> h((size_t)grid * 16);
+        cudaError_t pe = cudaStreamSynchronize(st);
+        if (pe == cudaSuccess) pe = cudaMemcpy(h.data(), prm2.prof, h.size() * 8, cudaMemcpyDeviceToHost);
+        cudaFree(prm2.prof);
+        if (pe != cudaSuccess) return check_cuda(pe, "TINA_PROF counter read-back");
+        double acc[16] = {0};
+        for (int b = 0; b < grid; b += UMMA_CG) for (int i = 0; i < 16; ++i) acc[i] += (double)h[(size_t)b * 16 + i] / (grid / UMMA_CG);
+        fprintf(stderr, "[tina prof symt] leader mean cycles: mma0 tot %.0f a_full %.0f b_full %.0f t_empty %.0f | mma1 tot %.0f a %.0f b %.0f t %.0f | epi tot %.0f t_full %.0f drain %.0f | prod tot %.0f waits %.0f lds+mac+sts %.0f fence %.0f\n",
+                acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], acc[7], acc[8], acc[9], acc[10], acc[12], acc[13], acc[14], acc[15]);
+    }
+#endif
+    count_launch();
+    g_last_path = kPathUmma;
+    note_kernel("pfb_symt_kernel", 0.5);
+    if (e != cudaSuccess) return check_cuda(e, "pfb_symt_kernel launch");
+    return check_cuda(cudaGetLastError(), "pfb_symt_kernel launch");
+}
+
+template <int MT, int PARTS>
 static tina_status launch_sym(DevCtx* ctx, const CUtensorMap& tmap, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
                               const SymParams& prm, int grid, cudaStream_t st)
 {
-    auto kern = pfb_sym_kernel<MT>;
+    auto kern = pfb_sym_kernel<MT, PARTS>;
     tina_status as = ensure_smem(ctx, reinterpret_cast<const void*>(kern), (int)SY_SMEM_BYTES, "cudaFuncSetAttribute(pfb_sym_kernel)");
     if (as != TINA_OK) return as;
     cudaLaunchConfig_t cfg = {};
@@ -463,7 +874,29 @@ static tina_status launch_sym(DevCtx* ctx, const CUtensorMap& tmap, const CUtens
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tmap, tmap_out, tmap_out2, prm);
+    SymParams prm2 = prm;
+#ifdef TINA_DEV
+    const bool prof = options().prof;
+    if (prof) {
+        cudaError_t pe = cudaMalloc(&prm2.prof, (size_t)grid * 16 * 8);
+        if (pe == cudaSuccess) pe = cudaMemsetAsync(prm2.prof, 0, (size_t)grid * 16 * 8, st);
+        if (pe != cudaSuccess) { if (prm2.prof) cudaFree(prm2.prof); return check_cuda(pe, "TINA_PROF counter buffer"); }
+    }
+#endif
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tmap, tmap_out, tmap_out2, prm2);
+#ifdef TINA_DEV
+    if (prof) {
+        std::vector<unsigned long long> h((size_t)grid * 16);
+        cudaError_t pe = cudaStreamSynchronize(st);
+        if (pe == cudaSuccess) pe = cudaMemcpy(h.data(), prm2.prof, h.size() * 8, cudaMemcpyDeviceToHost);
+        cudaFree(prm2.prof);
+        if (pe != cudaSuccess) return check_cuda(pe, "TINA_PROF counter read-back");
+        double acc[16] = {0};
+        for (int b = 0; b < grid; b += UMMA_CG) for (int i = 0; i < 16; ++i) acc[i] += (double)h[(size_t)b * 16 + i] / (grid / UMMA_CG);
+        fprintf(stderr, "[tina prof sym] leader mean cycles: mma0 tot %.0f a_full %.0f b_full %.0f t_empty %.0f | mma1 tot %.0f a %.0f b %.0f t %.0f | epi tot %.0f t_full %.0f drain %.0f | prod tot %.0f a_empty %.0f work+loads %.0f fence %.0f\n",
+                acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], acc[7], acc[8], acc[9], acc[10], acc[12], acc[13], acc[14], acc[15]);
+    }
+#endif
     count_launch();
     g_last_path = kPathUmma;
     note_kernel("pfb_sym_kernel", 0.5);
@@ -502,8 +935,10 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
     prm.total_work = (int)total;
     prm.parts = parts;
     prm.fp16 = fp16 ? 1 : 0;
+    const bool staged = !options().sym_v1;                        // TMA-staged input window (default) or register-window producers
+    const int kc_len = staged ? ST_KC : KC;                       // contraction elements per pipeline chunk
     prm.k_splits = (P + KSPLIT_MAX - 1) / KSPLIT_MAX;             // accumulation chains of <= 1024
-    prm.kc_per_split = ((P / KC) + prm.k_splits - 1) / prm.k_splits;
+    prm.kc_per_split = ((P / kc_len) + prm.k_splits - 1) / prm.k_splits;
     prm.debug = options().debug_skip;                             // 0 unless -DTINA_DEV
     const int n_cl = ctx->n_sm / UMMA_CG;
     const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
@@ -530,10 +965,45 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(out) failed (%d)", (int)r);
     }
-    if (!window) return launch_sym<0>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
-    if (M <= 4) return launch_sym<4>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
-    if (M <= 8) return launch_sym<8>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
-    return launch_sym<16>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st);
+    if (staged) {
+        // input as [S][NB][2P] floats, boxes of 64 floats (32 complex columns) x (128 + MT - 1) rows; the window as
+        // [M][P] floats, boxes of 32 x MT (rows >= M read as zeros)
+        const int MT = !window ? 0 : (M <= 4 ? 4 : (M <= 8 ? 8 : 16));
+        CUtensorMap tmap_x, tmap_w;
+        memset(&tmap_x, 0, sizeof(tmap_x));
+        memset(&tmap_w, 0, sizeof(tmap_w));
+        const cuuint32_t estr[3] = {1, 1, 1};
+        const cuuint64_t xdims[3] = {(cuuint64_t)2 * P, (cuuint64_t)NBLK, (cuuint64_t)S};
+        const cuuint64_t xstrides[2] = {(cuuint64_t)2 * P * sizeof(float),
+                                        S > 1 ? (cuuint64_t)2 * n_samples * sizeof(float) : (cuuint64_t)NBLK * 2 * P * sizeof(float)};
+        const cuuint32_t xbox[3] = {64, (cuuint32_t)(BM + (MT > 0 ? MT : 1) - 1), 1};
+        CUresult r = enc(&tmap_x, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(x), xdims, xstrides, xbox, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r == CUDA_SUCCESS && MT > 0) {
+            const cuuint64_t wdims[2] = {(cuuint64_t)P, (cuuint64_t)M};
+            const cuuint64_t wstrides[1] = {(cuuint64_t)P * sizeof(float)};
+            const cuuint32_t wbox[2] = {32, (cuuint32_t)MT};
+            r = enc(&tmap_w, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(window), wdims, wstrides, wbox, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        }
+        if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(input) failed (%d)", (int)r);
+#define TINA_SYMT(MT_) (parts == 2 ? launch_symt<MT_, 2>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st) \
+                                   : launch_symt<MT_, 1>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st))
+        if (MT == 0) return TINA_SYMT(0);
+        if (MT == 4) return TINA_SYMT(4);
+        if (MT == 8) return TINA_SYMT(8);
+        return TINA_SYMT(16);
+#undef TINA_SYMT
+    }
+#define TINA_SYM(MT_) (parts == 2 ? launch_sym<MT_, 2>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st) \
+                                  : launch_sym<MT_, 1>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st))
+    if (!window) return TINA_SYM(0);
+    if (M <= 4) return TINA_SYM(4);
+    if (M <= 8) return TINA_SYM(8);
+    return TINA_SYM(16);
+#undef TINA_SYM
 }
 
 }  // namespace tina

@@ -166,6 +166,13 @@ tina_status get_plan(int P, bool real, bool inverse, int parts, bool fp16, cudaS
     CUresult r = enc(&pl.tmap, fp16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, pl.tt, dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    memset(&pl.tmap32, 0, sizeof(pl.tmap32));
+    if (r == CUDA_SUCCESS && sym) {
+        const cuuint32_t box32[2] = {32, box[1]};
+        r = enc(&pl.tmap32, fp16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, pl.tt, dims, strides, box32, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
     if (r != CUDA_SUCCESS) { cudaFree(pl.tt); return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r); }
     auto ins = g_plans.emplace(key, pl);
     *out = &ins.first->second;

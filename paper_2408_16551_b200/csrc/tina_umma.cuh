@@ -52,6 +52,7 @@ EncodeTiledFn encode_fn();      // cuTensorMapEncodeTiled through the runtime's 
 struct Plan {
     __nv_bfloat16* tt = nullptr;
     CUtensorMap tmap;
+    CUtensorMap tmap32;     // sym plans only: boxes of 32 contraction elements (64-byte rows, SWIZZLE_64B)
 };
 tina_status get_plan(int P, bool real, bool inverse, int parts, bool fp16, cudaStream_t st, const Plan** out, bool sym = false);
 
