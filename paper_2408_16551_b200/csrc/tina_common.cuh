@@ -97,7 +97,8 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
 void umma_clear_plans();
 // complex kind with every distinct column pair (k, P-k) of the Fourier matrix contracted once (tina_sym.cu)
 bool sym_supported(int P);
-tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool inverse,
+bool sym_real_supported(int P);     // real kind: even / odd samples against the columns of the bins [0, P/4)
+tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool real, bool inverse,
                     tina_precision prec, void* out, cudaStream_t st);
 // PFB with the factorised (two-stage, 32 x 32) Fourier stage: complex kind, P = 1024, M <= 16 (tina_ct.cu)
 tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st);

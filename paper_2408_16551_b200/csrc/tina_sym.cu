@@ -49,6 +49,7 @@ struct SymParams {
     int parts;                 // 2: bf16x3, 1: single pass
     int fp16;
     int k_splits, kc_per_split;
+    int real;                  // 1: real kind (pfb_symt_kernel<.., REAL = true>): x is float32, out rows are P + 2 floats
     int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 16 no mirrored-tile stores, 32 no forward-tile stores
     unsigned long long* prof;  // -DTINA_DEV only (TINA_PROF): [grid][16] cycle counters
 };
@@ -62,6 +63,19 @@ struct SymParams {
 #define SY_NOW() 0LL
 #define SY_PROF 0
 #endif
+
+__device__ __forceinline__ float2 lds_f2(uint32_t addr)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds_f1(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
 
 __device__ __forceinline__ void sts16(uint32_t addr, uint32_t v)
 {
@@ -492,16 +506,120 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
     if (warp == ALLOC_WARP) tmem_dealloc<CG>(tmem_base, 512);
 }
 
+// Epilogue of the REAL kind (pfb_symt_kernel<.., REAL = true>).  The real frame y[p] is contracted as its even
+// samples (the "yr" tiles) and its odd samples (the "yi" tiles) against the cos / sin columns of the bins
+// k in [0, P/4):  U = sum_q y[2q] c, Z = sum_q y[2q] s  (D1),  W = sum_q y[2q+1] c', V = sum_q y[2q+1] s'  (D2),
+// with c, s at angle 2 pi (2q) k / P and c', s' at 2 pi (2q+1) k / P.  Columns k and P/2 - k of the Fourier
+// matrix agree on the even samples and differ in sign on the odd ones, so
+//     X[k] = (U + W) - i (Z + V),        X[P/2 - k] = (U - W) + i (Z - V).
+// Bin 0 has s = s' = 0: its sine columns carry (-1)^q instead and deliver the unpaired bin P/4
+// (X[P/4] = D1[1] - i D2[1]); the mirror of bin 0 is the Nyquist bin.  Output rows are P + 2 floats, i.e. only
+// 8-byte aligned, so the tiles leave through a swizzled shared-memory transpose and 8-byte stores (two rows x
+// 128 contiguous bytes per instruction); later accumulation chains add with red.global.add.v2.f32.
+__device__ __forceinline__ void sym_epilogue_real(const SymParams& prm, const EpiCtx& e, const int q, const int lane)
+{
+    constexpr int CG = UMMA_CG;
+    const int P = prm.P, quarter = P >> 2, npg = prm.n_passes;
+    const uint32_t sb = e.stage + (uint32_t)q * SY_STAGE;
+    const uint32_t taddr = e.tmem_base + ((uint32_t)(q * 32) << 16);
+    const uint32_t rowoff = (uint32_t)lane * 128u, sw = (uint32_t)lane & 7u;
+    // transposed read-out: lane -> (row lane >> 4 (+ 2 i), bin lane & 15)
+    const uint32_t rd_c = (uint32_t)lane & 15u, rd_r0 = (uint32_t)lane >> 4;
+    uint32_t tf_phase = 0;
+    long long pe_w = 0, pe_d = 0, pe_x, pe_tot = SY_NOW();
+    for (int w = e.cl; w < prm.total_work; w += e.n_cl) {
+        const int tile = w / npg;
+        const int k0 = (w % npg) * SY_BINS;
+        const int ncol = 2 * min(SY_BINS, quarter - k0);
+        const int s = tile / prm.tiles_per_stream;
+        const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + e.rank * BM + q * 32;
+        const int rows_valid = (int)min(32LL, prm.F - row0);
+        float* const otile = prm.out + ((long long)s * prm.F + row0) * (long long)(P + 2);
+        for (int ks = 0; ks < prm.k_splits; ++ks) {
+            pe_x = SY_NOW();
+            mbar_wait<256>(e.t_full0, tf_phase);
+            mbar_wait<256>(e.t_full1, tf_phase);
+            pe_w += SY_NOW() - pe_x; pe_x = SY_NOW();
+            tf_phase ^= 1u;
+            tc_fence_after();
+            uint32_t r1[32], r2[32];
+            tmem_ld32(taddr, r1);
+            tmem_ld32(taddr + 256u, r2);
+            // store a staged 32 x 16-bin tile whose first bin is `bin0`: lanes 0-15 / 16-31 take rows 2 i / 2 i + 1
+            auto flush = [&](uint32_t tile_s, int bin0) {
+#pragma unroll 4
+                for (int i = 0; i < 16; ++i) {
+                    const uint32_t r = rd_r0 + 2u * (uint32_t)i;
+                    const float2 v = lds_f2(tile_s + r * 128u + ((((rd_c >> 1) ^ (r & 7u))) << 4) + (rd_c & 1u) * 8u);
+                    if ((int)r < rows_valid) {
+                        float2* g = reinterpret_cast<float2*>(otile + (long long)r * (P + 2) + 2 * (bin0 + (int)rd_c));
+                        if (ks > 0) atomicAdd(g, v); else *g = v;
+                    }
+                }
+            };
+            for (int cb = 0; cb < ncol; cb += 32) {
+                const int kb = k0 + (cb >> 1);
+                const bool last = cb + 32 >= ncol;
+                tmem_ld_wait();
+                if (last) {
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {
+                        arrive_leader<CG>(e.t_empty0, e.rank, 0);
+                        arrive_leader<CG>(e.t_empty1, e.rank, 0);
+                    }
+                    pe_d += SY_NOW() - pe_x;
+                }
+#define SY_F(v) __uint_as_float(v)
+                if (kb == 0) {
+                    // the sine slots of bin 0 carry (-1)^q: X[P/4] = D1[1] - i D2[1] (unpaired)
+                    if (lane < rows_valid) {
+                        float2* g = reinterpret_cast<float2*>(otile + (long long)lane * (P + 2) + 2 * quarter);
+                        const float2 v = make_float2(SY_F(r1[1]), -SY_F(r2[1]));
+                        if (ks > 0) atomicAdd(g, v); else *g = v;
+                    }
+                    r1[1] = 0u; r2[1] = 0u;                      // Z = V = 0 for bin 0
+                }
+                __syncwarp();                                     // the previous step's read-out of both tiles is done
+#pragma unroll
+                for (int g = 0; g < 8; ++g) {
+                    const float U0 = SY_F(r1[4 * g]), Z0 = SY_F(r1[4 * g + 1]), U1 = SY_F(r1[4 * g + 2]), Z1 = SY_F(r1[4 * g + 3]);
+                    const float W0 = SY_F(r2[4 * g]), V0 = SY_F(r2[4 * g + 1]), W1 = SY_F(r2[4 * g + 2]), V1 = SY_F(r2[4 * g + 3]);
+                    // forward: bins kb + 2g, kb + 2g + 1 -> 16-byte chunk g; the imaginary part of bin 0 is +0
+                    const float i0 = (kb == 0 && g == 0) ? 0.f : -(Z0 + V0);
+                    sts128(sb + rowoff + (((uint32_t)g ^ sw) << 4), __float_as_uint(U0 + W0), __float_as_uint(i0),
+                           __float_as_uint(U1 + W1), __float_as_uint(-(Z1 + V1)));
+                    // mirrored: bin P/2 - kb - j at position 15 - j: j = 2g + 1 -> position 14 - 2g, j = 2g -> 15 - 2g: chunk 7 - g
+                    sts128(sb + 4096u + rowoff + (((uint32_t)(7 - g) ^ sw) << 4), __float_as_uint(U1 - W1), __float_as_uint(Z1 - V1),
+                           __float_as_uint(U0 - W0), __float_as_uint(Z0 - V0));
+                }
+#undef SY_F
+                if (!last) { tmem_ld32(taddr + cb + 32, r1); tmem_ld32(taddr + 256u + cb + 32, r2); }
+                __syncwarp();
+                flush(sb, kb);
+                flush(sb + 4096u, (P >> 1) - kb - 15);
+            }
+        }
+    }
+    if (SY_PROF && prm.prof && q == 0 && lane == 0) {
+        unsigned long long* pp = prm.prof + blockIdx.x * 16 + 8;
+        pp[0] = SY_NOW() - pe_tot; pp[1] = pe_w; pp[2] = pe_d;
+    }
+}
+
 // =====================================================================================
 // pfb_symt_kernel: the same contraction with the INPUT WINDOW AND THE TAPS STAGED BY TMA (the north_star
 // sketch): per chunk of 32 complex columns the (128 + MT - 1) x 32 block of input
 // rows and the MT x 32 block of prototype-filter taps are bulk-copied into a two-slot shared-memory ring; the
 // FIR producers read their sliding window from shared memory (no long-latency global loads in the FIR warps,
 // every input row fetched from L2 once per CTA and chunk instead of once per 16-frame warp slab, taps once per
-// CTA instead of once per warp).  To make room the operand tiles are 32 contraction elements wide (64-byte
+// CTA instead of once per warp).  REAL = true: the real kind, contracted as even / odd samples against the
+// cos / sin columns of the bins [0, P/4) -- see sym_epilogue_real; the producers are the same (an adjacent pair of
+// real samples takes the place of (re, im)), each MMA warp has its own twiddle entries (even-sample and
+// odd-sample matrices), and K = P/2.  To make room the operand tiles are 32 contraction elements wide (64-byte
 // rows, SWIZZLE_64B): A slot = 4 x 8 KB, B entry = 8 KB per CTA, two K = 16 MMAs per tile and product.
 //   shared memory: A ring 64 KB (2 slots; 4 for the single pass) | B ring 48 KB (6 entries = 3 chunks) |
-//                  input ring 2 x 38 KB | epilogue staging 32 KB
+//                  input ring 2 x 40 KB | epilogue staging 32 KB
 //   warps: 0-7 FIR producers, 8-11 epilogue, 12 TMA (twiddles), 13 / 15 MMA issuers, 14 TMEM allocation + TMA (input)
 // =====================================================================================
 constexpr int ST_KC = 32;                                  // contraction elements (complex columns) per chunk
@@ -511,7 +629,7 @@ constexpr int ST_B_ENTRY = (NSUB / UMMA_CG) * ST_KC * 2;   // 8 KB per CTA
 constexpr int ST_B_ENTRIES = 6;
 constexpr int ST_IN_ROWS_MAX = BM + 15;                    // 143 input rows of 256 B
 constexpr int ST_IN_TAPS = ST_IN_ROWS_MAX * 256;           // byte offset of the taps block in an input slot
-constexpr int ST_IN_SLOT = 38 * 1024;                      // 36 608 B of rows + 2 KB of taps, 1024-byte multiple
+constexpr int ST_IN_SLOT = 40 * 1024;                      // 36 608 B of rows + up to 4 KB of taps (real kind: 64 per row)
 constexpr int ST_IN_SLOTS = 2;
 
 struct SmemCtlT {
@@ -524,20 +642,7 @@ struct SmemCtlT {
 constexpr size_t ST_SMEM_BYTES = ST_A_RING + ST_B_ENTRIES * ST_B_ENTRY + ST_IN_SLOTS * ST_IN_SLOT + 4 * SY_STAGE + sizeof(SmemCtlT);
 static_assert(ST_SMEM_BYTES <= 232448, "exceeds the 227 KB shared memory opt-in limit");
 
-__device__ __forceinline__ float2 lds_f2(uint32_t addr)
-{
-    float2 v;
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ float lds_f1(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-    return v;
-}
-
-template <int MT, int PARTS>
+template <int MT, int PARTS, bool REAL>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_out,
                 const __grid_constant__ CUtensorMap tmap_out2, const __grid_constant__ CUtensorMap tmap_x,
@@ -559,20 +664,24 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
     constexpr uint32_t n_a = (uint32_t)ST_A_RING / a_slot_bytes;       // 2 (bf16x3) or 4 (single pass)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int P = prm.P, M = prm.M;
-    const int n_kc = P / ST_KC;
-    const int half = P >> 1;
+    const int kdim = REAL ? (P >> 1) : P;                              // contraction length (sample pairs / complex samples)
+    const int n_kc = kdim / ST_KC;
+    const int half = REAL ? (P >> 2) : (P >> 1);                       // bins contracted: [0, P/4) real, [0, P/2) complex
+    constexpr int EO = REAL ? 2 : 1;                                   // twiddle matrices: even / odd samples, or one
+    constexpr uint32_t EPC = (uint32_t)parts * EO;                     // B ring entries per chunk
     const uint32_t rank = cluster_ctarank();
     constexpr uint32_t leader = 0;
     constexpr uint16_t pair_mask = 3;
     const int cl = blockIdx.x / CG, n_cl = gridDim.x / CG;
     const int npg = prm.n_passes;
-    const uint32_t b_box_bytes = (uint32_t)(P < NSUB ? P : NSUB) / CG * ST_KC * 2;
+    const int b_rows = 2 * half;                                       // matrix rows per part (and per even / odd half)
+    const uint32_t b_box_bytes = (uint32_t)(b_rows < NSUB ? b_rows : NSUB) / CG * ST_KC * 2;
 
     if (warp == TMA_WARP && lane == 0) {
         prefetch_tmap(&tmap_b); prefetch_tmap(&tmap_out); prefetch_tmap(&tmap_out2); prefetch_tmap(&tmap_x);
         if (MT > 0) prefetch_tmap(&tmap_w);
         for (int i = 0; i < 4; ++i) { mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0)); mbar_init(smem_u32(&ctl->a_empty[i]), 2); }
-        for (int i = 0; i < ST_B_ENTRIES; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), 2); }
+        for (int i = 0; i < ST_B_ENTRIES; ++i) { mbar_init(smem_u32(&ctl->b_full[i]), 1); mbar_init(smem_u32(&ctl->b_empty[i]), REAL ? 1 : 2); }
         for (int i = 0; i < ST_IN_SLOTS; ++i) { mbar_init(smem_u32(&ctl->in_full[i]), 1); mbar_init(smem_u32(&ctl->in_empty[i]), N_PROD_WARPS); }
         for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
         fence_mbar_init();
@@ -599,9 +708,9 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     mbar_wait<64>(smem_u32(&ctl->in_empty[in.idx]), in.phase ^ 1);
                     const uint32_t bar = smem_u32(&ctl->in_full[in.idx]);
                     const uint32_t dst = smem_u32(in_ring + in.idx * ST_IN_SLOT);
-                    mbar_expect_tx(bar, (uint32_t)IN_ROWS * 256u + (MT > 0 ? (uint32_t)MT * 128u : 0u));
+                    mbar_expect_tx(bar, (uint32_t)IN_ROWS * 256u + (MT > 0 ? (uint32_t)MT * (REAL ? 256u : 128u) : 0u));
                     tma_load_3d(dst, &tmap_x, bar, kc * 2 * ST_KC, r0, s);       // rows outside [0, NB) arrive as zeros
-                    if (MT > 0) tma_load_2d(dst + ST_IN_TAPS, &tmap_w, bar, kc * ST_KC, 0);   // rows >= M arrive as zeros
+                    if (MT > 0) tma_load_2d(dst + ST_IN_TAPS, &tmap_w, bar, kc * ST_KC * (REAL ? 2 : 1), 0);   // rows >= M arrive as zeros
                     in.advance(ST_IN_SLOTS);
                 }
             }
@@ -614,11 +723,11 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 const int k0 = (w % npg) * SY_BINS;
                 const int nw = 2 * min(SY_BINS, half - k0);
                 for (int kc = 0; kc < n_kc; ++kc)
-                    for (int part = 0; part < parts; ++part) {
+                    for (int pe = 0; pe < (int)EPC; ++pe) {             // (part, even / odd) in ring order
                         mbar_wait<64>(smem_u32(&ctl->b_empty[b.idx]), b.phase ^ 1);
                         const uint32_t bar = smem_u32(&ctl->b_full[b.idx]);
                         const uint32_t dst = smem_u32(b_ring + b.idx * ST_B_ENTRY);
-                        const int row = part * P + 2 * k0 + (int)rank * (nw / CG);
+                        const int row = pe * b_rows + 2 * k0 + (int)rank * (nw / CG);
                         if (rank == 0) mbar_expect_tx(bar, 2 * b_box_bytes);
                         tma_load_2d_cg2(dst, &tmap_b, mapa_u32(bar, leader), kc * ST_KC, row);
                         b.advance(ST_B_ENTRIES);
@@ -639,7 +748,8 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 }
         }
         if (rank == 0) {
-            RingPos a, b;
+            RingPos a;
+            uint32_t be = 0;                                       // B ring entries issued before this chunk
             uint32_t te_phase = 0;
             const uint32_t d = tmem_base + (uint32_t)h * 256u;
             long long pm_a = 0, pm_b = 0, pm_t = 0, pm_x, pm_tot = SY_NOW();
@@ -659,10 +769,14 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             te_phase ^= 1u;
                             tc_fence_after();
                         }
-                        pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
+                        // ring order per chunk: (hi, even) [(hi, odd)] (lo, even) [(lo, odd)]; the real kind gives each
+                        // MMA warp its own matrix (h = 0: even samples, h = 1: odd samples), the complex kind shares one
+                        uint32_t e_i = be + (REAL ? (uint32_t)h : 0u);
+                        uint32_t bi = e_i % ST_B_ENTRIES, bp = (e_i / ST_B_ENTRIES) & 1u;
+                        pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); pm_b += SY_NOW() - pm_x;
                         tc_fence_after();
                         if (lane == 0) {
-                            const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + b.idx * ST_B_ENTRY));
+                            const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + bi * ST_B_ENTRY));
                             uint32_t acc = kc > kc_begin;
                             if (parts > 1) {
                                 const uint64_t ad = smem_desc_sw64(a_lo);
@@ -672,23 +786,23 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             const uint64_t ad = smem_desc_sw64(a_hi);
 #pragma unroll
                             for (int k = 0; k < ST_KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
-                            commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]), pair_mask);
+                            commit_cg<CG>(smem_u32(&ctl->b_empty[bi]), pair_mask);
                         }
                         __syncwarp();
-                        b.advance(ST_B_ENTRIES);
                         if (parts > 1) {
-                            pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
+                            e_i += EO; bi = e_i % ST_B_ENTRIES; bp = (e_i / ST_B_ENTRIES) & 1u;
+                            pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); pm_b += SY_NOW() - pm_x;
                             tc_fence_after();
                             if (lane == 0) {
-                                const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + b.idx * ST_B_ENTRY));
+                                const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + bi * ST_B_ENTRY));
                                 const uint64_t ad = smem_desc_sw64(a_hi);
 #pragma unroll
                                 for (int k = 0; k < ST_KC / 16; ++k) umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
-                                commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]), pair_mask);
+                                commit_cg<CG>(smem_u32(&ctl->b_empty[bi]), pair_mask);
                             }
                             __syncwarp();
-                            b.advance(ST_B_ENTRIES);
                         }
+                        be += EPC;
                         if (lane == 0) {
                             commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
                             if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[h]), pair_mask);
@@ -708,7 +822,8 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         ec.t_full0 = smem_u32(&ctl->t_full[0]); ec.t_full1 = smem_u32(&ctl->t_full[1]);
         ec.t_empty0 = smem_u32(&ctl->t_empty[0]); ec.t_empty1 = smem_u32(&ctl->t_empty[1]);
         ec.stage = smem_u32(stage); ec.tmem_base = tmem_base; ec.rank = rank; ec.cl = cl; ec.n_cl = n_cl;
-        sym_epilogue(prm, &tmap_out, &tmap_out2, ec, warp - EPI_WARP0, lane);
+        if (REAL) sym_epilogue_real(prm, ec, warp - EPI_WARP0, lane);
+        else      sym_epilogue(prm, &tmap_out, &tmap_out2, ec, warp - EPI_WARP0, lane);
     } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ FIR producers =========================================
         // Warp pw owns frames 16 pw .. 16 pw + 15 of the CTA's tile, lane = complex column of the chunk.  Per
@@ -723,7 +838,7 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             cell0[j] = a_ring_s + (uint32_t)(pw * FPW) * 64u + ((((uint32_t)lane >> 3) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 7u) * 2u;
         constexpr uint32_t im_off = (uint32_t)parts * ST_TILE;
         const uint32_t in_lane = in_ring_s + (uint32_t)(pw * FPW) * 256u + (uint32_t)lane * 8u;
-        const uint32_t tap_lane = in_ring_s + ST_IN_TAPS + (uint32_t)lane * 4u;
+        const uint32_t tap_lane = in_ring_s + ST_IN_TAPS + (uint32_t)lane * (REAL ? 8u : 4u);
         long long pq_w = 0, pq_c = 0, pq_f = 0, pq_x, pq_tot = SY_NOW();
         RingPos in, a;
         for (int w = cl; w < prm.total_work; w += n_cl)
@@ -736,7 +851,10 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     const uint32_t src = in_lane + in.idx * ST_IN_SLOT, tsrc = tap_lane + in.idx * ST_IN_SLOT;
                     if (MT > 0) {
 #pragma unroll
-                        for (int m = 0; m < WA; ++m) { const float hh = lds_f1(tsrc + (uint32_t)m * 128u); rg.tap[m] = make_float2(hh, hh); }
+                        for (int m = 0; m < WA; ++m) {
+                            if (REAL) rg.tap[m] = lds_f2(tsrc + (uint32_t)m * 256u);        // one tap per real sample of the pair
+                            else { const float hh = lds_f1(tsrc + (uint32_t)m * 128u); rg.tap[m] = make_float2(hh, hh); }
+                        }
                     }
 #pragma unroll
                     for (int j = 0; j < WA - 1 + FPW; ++j) rg.row[j] = lds_f2(src + (uint32_t)j * 256u);
@@ -806,11 +924,11 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
 // =====================================================================================
 bool sym_supported(int P) { return P >= 64 && P <= kMaxP && P % 64 == 0; }
 
-template <int MT, int PARTS>
+template <int MT, int PARTS, bool REAL>
 static tina_status launch_symt(DevCtx* ctx, const Plan* plan, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
                                const CUtensorMap& tmap_x, const CUtensorMap& tmap_w, const SymParams& prm, int grid, cudaStream_t st)
 {
-    auto kern = pfb_symt_kernel<MT, PARTS>;
+    auto kern = pfb_symt_kernel<MT, PARTS, REAL>;
     tina_status as = ensure_smem(ctx, reinterpret_cast<const void*>(kern), (int)ST_SMEM_BYTES, "cudaFuncSetAttribute(pfb_symt_kernel)");
     if (as != TINA_OK) return as;
     cudaLaunchConfig_t cfg = {};
@@ -850,7 +968,7 @@ static tina_status launch_symt(DevCtx* ctx, const Plan* plan, const CUtensorMap&
 #endif
     count_launch();
     g_last_path = kPathUmma;
-    note_kernel("pfb_symt_kernel", 0.5);
+    note_kernel(REAL ? "pfb_symt_kernel<real>" : "pfb_symt_kernel", 0.5);
     if (e != cudaSuccess) return check_cuda(e, "pfb_symt_kernel launch");
     return check_cuda(cudaGetLastError(), "pfb_symt_kernel launch");
 }
@@ -904,8 +1022,11 @@ static tina_status launch_sym(DevCtx* ctx, const CUtensorMap& tmap, const CUtens
     return check_cuda(cudaGetLastError(), "pfb_sym_kernel launch");
 }
 
-// complex kind, P % 64 == 0, window == nullptr (DFT batch) or M <= 16
-tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool inverse,
+bool sym_real_supported(int P) { return P >= 128 && P <= kMaxP && P % 64 == 0 && !options().sym_v1; }
+
+// complex kind with P % 64 == 0, or real kind with P % 64 == 0 and P >= 128 (TMA-staged kernel only);
+// window == nullptr (DFT batch, complex) or M <= 16
+tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool real, bool inverse,
                     tina_precision prec, void* out, cudaStream_t st)
 {
     const long long NBLK = n_samples / P;
@@ -913,45 +1034,48 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
     const int parts = prec == TINA_PREC_FP32 ? 2 : 1;
     const bool fp16 = prec == TINA_PREC_FP16;
     const Plan* plan = nullptr;
-    tina_status ps = get_plan(P, false, inverse, parts, fp16, st, &plan, true);
+    tina_status ps = get_plan(P, real, inverse, parts, fp16, st, &plan, true);
     if (ps != TINA_OK) return ps;
     DevCtx* ctx = nullptr;
     if ((ps = dev_ctx(&ctx)) != TINA_OK) return ps;
+    const bool staged = real || !options().sym_v1;                // TMA-staged input window (default) or register-window producers
+    const int kdim = real ? P / 2 : P;                            // contraction length
+    const int bins = real ? P / 4 : P / 2;                        // bins contracted (the rest are their mirrors)
 
     SymParams prm;
     memset(&prm, 0, sizeof(prm));
     prm.x = static_cast<const float*>(x);
     prm.window = window;
     prm.out = static_cast<float*>(out);
-    prm.stream_stride = 2 * n_samples;
+    prm.stream_stride = real ? n_samples : 2 * n_samples;
     prm.F = F;
     prm.NBLK = NBLK;
     prm.P = P;
     prm.M = M;
+    prm.real = real ? 1 : 0;
     prm.tiles_per_stream = (int)((F + BM * UMMA_CG - 1) / (BM * UMMA_CG));
-    prm.n_passes = (P / 2 + SY_BINS - 1) / SY_BINS;
+    prm.n_passes = (bins + SY_BINS - 1) / SY_BINS;
     const long long total = (long long)S * prm.tiles_per_stream * prm.n_passes;
     if (total > 0x7fffffffLL) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: too many tiles");
     prm.total_work = (int)total;
     prm.parts = parts;
     prm.fp16 = fp16 ? 1 : 0;
-    const bool staged = !options().sym_v1;                        // TMA-staged input window (default) or register-window producers
     const int kc_len = staged ? ST_KC : KC;                       // contraction elements per pipeline chunk
-    prm.k_splits = (P + KSPLIT_MAX - 1) / KSPLIT_MAX;             // accumulation chains of <= 1024
-    prm.kc_per_split = ((P / kc_len) + prm.k_splits - 1) / prm.k_splits;
+    prm.k_splits = (kdim + KSPLIT_MAX - 1) / KSPLIT_MAX;          // accumulation chains of <= 1024
+    prm.kc_per_split = ((kdim / kc_len) + prm.k_splits - 1) / prm.k_splits;
     prm.debug = options().debug_skip;                             // 0 unless -DTINA_DEV
     const int n_cl = ctx->n_sm / UMMA_CG;
     const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
 
-    // Output maps over [S][F][2P] floats: 32 x 32 swizzled boxes, and 28-float-wide dense boxes for the mirrored
-    // tile of a pass's last step (see the epilogue).
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    const cuuint32_t estr[3] = {1, 1, 1};
+    // Output maps (complex kind) over [S][F][2P] floats: 32 x 32 swizzled boxes, and 28-float-wide dense boxes for
+    // the mirrored tile of a pass's last step (see the epilogue).  The real kind stores from registers.
     CUtensorMap tmap_out, tmap_out2;
     memset(&tmap_out, 0, sizeof(tmap_out));
     memset(&tmap_out2, 0, sizeof(tmap_out2));
-    EncodeTiledFn enc = encode_fn();
-    if (!enc) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
-    {
-        const cuuint32_t estr[3] = {1, 1, 1};
+    if (!real) {
         const cuuint64_t dims[3] = {(cuuint64_t)2 * P, (cuuint64_t)F, (cuuint64_t)S};
         const cuuint64_t strides[2] = {(cuuint64_t)2 * P * sizeof(float), (cuuint64_t)F * 2 * P * sizeof(float)};
         const cuuint32_t box[3] = {32, 32, 1};
@@ -966,16 +1090,16 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
         if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(out) failed (%d)", (int)r);
     }
     if (staged) {
-        // input as [S][NB][2P] floats, boxes of 64 floats (32 complex columns) x (128 + MT - 1) rows; the window as
-        // [M][P] floats, boxes of 32 x MT (rows >= M read as zeros)
+        // input as [S][NB][row] floats (row = 2P complex, P real), boxes of 64 floats (32 complex columns / 32 pairs of
+        // real samples) x (128 + MT - 1) rows; the window as [M][P] floats, boxes of (32 | 64) x MT (rows >= M read as zeros)
         const int MT = !window ? 0 : (M <= 4 ? 4 : (M <= 8 ? 8 : 16));
+        const long long row_f = real ? P : 2LL * P;
         CUtensorMap tmap_x, tmap_w;
         memset(&tmap_x, 0, sizeof(tmap_x));
         memset(&tmap_w, 0, sizeof(tmap_w));
-        const cuuint32_t estr[3] = {1, 1, 1};
-        const cuuint64_t xdims[3] = {(cuuint64_t)2 * P, (cuuint64_t)NBLK, (cuuint64_t)S};
-        const cuuint64_t xstrides[2] = {(cuuint64_t)2 * P * sizeof(float),
-                                        S > 1 ? (cuuint64_t)2 * n_samples * sizeof(float) : (cuuint64_t)NBLK * 2 * P * sizeof(float)};
+        const cuuint64_t xdims[3] = {(cuuint64_t)row_f, (cuuint64_t)NBLK, (cuuint64_t)S};
+        const cuuint64_t xstrides[2] = {(cuuint64_t)row_f * sizeof(float),
+                                        S > 1 ? (cuuint64_t)prm.stream_stride * sizeof(float) : (cuuint64_t)NBLK * row_f * sizeof(float)};
         const cuuint32_t xbox[3] = {64, (cuuint32_t)(BM + (MT > 0 ? MT : 1) - 1), 1};
         CUresult r = enc(&tmap_x, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(x), xdims, xstrides, xbox, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -983,19 +1107,21 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
         if (r == CUDA_SUCCESS && MT > 0) {
             const cuuint64_t wdims[2] = {(cuuint64_t)P, (cuuint64_t)M};
             const cuuint64_t wstrides[1] = {(cuuint64_t)P * sizeof(float)};
-            const cuuint32_t wbox[2] = {32, (cuuint32_t)MT};
+            const cuuint32_t wbox[2] = {real ? 64u : 32u, (cuuint32_t)MT};
             r = enc(&tmap_w, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(window), wdims, wstrides, wbox, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         }
         if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(input) failed (%d)", (int)r);
-#define TINA_SYMT(MT_) (parts == 2 ? launch_symt<MT_, 2>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st) \
-                                   : launch_symt<MT_, 1>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st))
-        if (MT == 0) return TINA_SYMT(0);
+#define TINA_SYMT2(MT_, R_) (parts == 2 ? launch_symt<MT_, 2, R_>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st) \
+                                        : launch_symt<MT_, 1, R_>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st))
+#define TINA_SYMT(MT_) (real ? TINA_SYMT2(MT_, true) : TINA_SYMT2(MT_, false))
+        if (MT == 0) return real ? fail(TINA_ERR_UNSUPPORTED, "real kind needs a window") : TINA_SYMT2(0, false);
         if (MT == 4) return TINA_SYMT(4);
         if (MT == 8) return TINA_SYMT(8);
         return TINA_SYMT(16);
 #undef TINA_SYMT
+#undef TINA_SYMT2
     }
 #define TINA_SYM(MT_) (parts == 2 ? launch_sym<MT_, 2>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st) \
                                   : launch_sym<MT_, 1>(ctx, plan->tmap, tmap_out, tmap_out2, prm, grid, st))

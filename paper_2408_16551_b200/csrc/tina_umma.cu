@@ -74,13 +74,27 @@ struct UmmaParams {
 __global__ void twiddle_kernel(__nv_bfloat16* __restrict__ tt, int P, int real, int inverse, int parts, int fp16, int sym)
 {
     const int N = (real || sym) ? P : 2 * P;
-    const long long total = (long long)N * N;
+    const int Kd = (real && sym) ? P / 2 : N;          // contraction length (row length); real + sym: sample PAIRS
+    const long long total = (long long)N * Kd;
     const double scale = inverse ? 1.0 / (double)P : 1.0;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
          e += (long long)gridDim.x * blockDim.x) {
-        const int n = (int)(e / N), c = (int)(e % N);
+        const int n = (int)(e / Kd), c = (int)(e % Kd);
         double v;
-        if (sym) {
+        if (sym && real) {
+            // real kind, column-paired (tina_sym.cu): rows [eo][2k + j], eo = 0 the even samples p = 2q, eo = 1 the odd
+            // samples p = 2q + 1, k in [0, P/4): j = 0 cos(2 pi p k / P), j = 1 sin(2 pi p k / P); the sine rows of
+            // bin 0 (identically zero) carry (-1)^q, which gives the unpaired bin P/4
+            const int eo = n / (P / 2), nn = n % (P / 2);
+            if (nn == 1) v = (c & 1) ? -1.0 : 1.0;
+            else {
+                const int k = nn >> 1;
+                const long long r = ((long long)(2 * c + eo) * k) % P;
+                double sn, cs;
+                sincospi(2.0 * (double)r / (double)P, &sn, &cs);
+                v = (nn & 1) ? sn : cs;
+            }
+        } else if (sym) {
             if (n == 1) v = (c & 1) ? -1.0 : 1.0;
             else {
                 const int k = n >> 1;
@@ -147,8 +161,9 @@ tina_status get_plan(int P, bool real, bool inverse, int parts, bool fp16, cudaS
     if (it != g_plans.end()) { *out = &it->second; return TINA_OK; }
 
     const int N = (real || sym) ? P : 2 * P;
+    const int Kd = (real && sym) ? P / 2 : N;           // row length (contraction elements)
     Plan pl;
-    const size_t bytes = (size_t)parts * N * N * sizeof(__nv_bfloat16);
+    const size_t bytes = (size_t)parts * N * Kd * sizeof(__nv_bfloat16);
     e = cudaMalloc(&pl.tt, bytes);
     if (e != cudaSuccess) return check_cuda(e, "cudaMalloc(twiddles)");
     twiddle_kernel<<<592, 256, 0, st>>>(pl.tt, P, real ? 1 : 0, inverse ? 1 : 0, parts, fp16 ? 1 : 0, sym ? 1 : 0);
@@ -159,9 +174,10 @@ tina_status get_plan(int P, bool real, bool inverse, int parts, bool fp16, cudaS
 
     EncodeTiledFn enc = encode_fn();
     if (!enc) { cudaFree(pl.tt); return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found"); }
-    const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)parts * N};       // innermost (K) first
-    const cuuint64_t strides[1] = {(cuuint64_t)N * sizeof(__nv_bfloat16)};
-    const cuuint32_t box[2] = {(cuuint32_t)KC, (cuuint32_t)((N < NSUB ? N : NSUB) / UMMA_CG)};
+    const cuuint64_t dims[2] = {(cuuint64_t)Kd, (cuuint64_t)parts * N};      // innermost (K) first
+    const cuuint64_t strides[1] = {(cuuint64_t)Kd * sizeof(__nv_bfloat16)};
+    const int nb_rows = (real && sym) ? N / 2 : N;       // rows of one matrix (real + sym: even- and odd-sample halves)
+    const cuuint32_t box[2] = {(cuuint32_t)KC, (cuuint32_t)((nb_rows < NSUB ? nb_rows : NSUB) / UMMA_CG)};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(&pl.tmap, fp16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, pl.tt, dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -819,8 +835,8 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     }
 
     // complex kind: the column-paired contraction (half the tensor work) wherever its tiling applies
-    if (!real && sym_supported(P) && !options().no_sym)
-        return sym_pfb(x, S, n_samples, P, M, window, inverse, prec, out, st);
+    if (!options().no_sym && (real ? (window && sym_real_supported(P)) : sym_supported(P)))
+        return sym_pfb(x, S, n_samples, P, M, window, real, inverse, prec, out, st);
 
     const Plan* plan = nullptr;
     tina_status ps = get_plan(P, real, inverse, parts, fp16, st, &plan);
