@@ -411,7 +411,7 @@ def run_ours(args, w):
 
     # ---- e2e: host buffers through the C ABI (H2D + kernel + D2H inside the timed region) --
     e2e = None
-    if w["call"] == "pfb":
+    if w["call"] == "pfb" and not args.profile:
         xp, wp = x_host.pin_memory(), w_host.pin_memory()
         outp = torch.empty((w["S"], w["F"], NK), dtype=torch.complex64, pin_memory=True)
         n_e2e = max(2, min(args.steps, 5))
@@ -470,8 +470,8 @@ def run_ours(args, w):
     roof["kernel_ms_min"] = kern_min
     roof["kernel"] = variant
 
-    cpu_val, cores, sample, _ = cpu_oracle_rate(w) if world == 1 else (None, None, None, None)
-    cpu_np = cpu_numpy_rate(w) if world == 1 else None
+    cpu_val, cores, sample, _ = cpu_oracle_rate(w) if (world == 1 and not args.profile) else (None, None, None, None)
+    cpu_np = cpu_numpy_rate(w) if (world == 1 and not args.profile) else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": n_warm,
         "ms_per_step": ms_per_step, "ms_mean": kern_ms, "ms_min": kern_min,
@@ -486,6 +486,8 @@ def run_ours(args, w):
                    "parallelism": f"frame-sharded replicas x{world}, no collective"},
         "roofline": roof, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "tina_env": env,
     }
+    if args.profile:
+        line["profile_run"] = True
     if hot is not None:
         line["hot"] = hot
     if cpu_val is not None:
@@ -505,6 +507,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4")
+    ap.add_argument("--profile", action="store_true",
+                    help="profiling run (under ncu): skip the CPU baselines and the e2e leg; the line is not a bench value")
     args = ap.parse_args()
     w = workload_spec(args.workload)
     if w["call"] == "peaks":

@@ -107,7 +107,10 @@ tina_status tina_dft(const void* x, void* out, long long B, int N, int inverse,
  *           spectrum k in [0,P/2]) (device), F = tina_pfb_num_frames(n_samples, P, M)
  * Supported: 2 <= P <= 8192 (even for REAL), 1 <= M <= 64, F >= 1.  COMPLEX with
  * P % 32 == 0 and REAL with P % 64 == 0 run on the tensor-core path; other P on the
- * generic CUDA-core path (fp32 regardless of `prec`).
+ * generic CUDA-core path (fp32 regardless of `prec`).  Where P % 64 == 0 (REAL: and P >= 128)
+ * the tensor-core path contracts every distinct column pair of the Fourier matrix once
+ * (bins k and P-k, REAL: k and P/2-k, share their cosine / sine sums; half the tensor
+ * flops, same result and contract) with the input window and taps staged by TMA.
  * tina_pfb_batched: S independent streams in one launch, x [S][n_samples],
  * out [S][F][...]; n_samples must then keep every stream 16-byte aligned
  * (n_samples even for COMPLEX, % 4 == 0 for REAL) else ALIGNMENT.                          */
