@@ -862,39 +862,65 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
                 mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
                 pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
-                // polyphase MAC + split + de-interleaved store (as fir_compute_store_sym, 64-byte rows)
+                // polyphase MAC + split + de-interleaved store (as fir_compute_store_sym, 64-byte rows).  The 32 stores of
+                // the first eight frames are interleaved with the packed FMAs of the last eight, so that the
+                // shared-memory store queue drains under arithmetic instead of stalling the warp.
                 const uint32_t so = a.idx * a_slot_bytes;
-#pragma unroll
-                for (int i0 = 0; i0 < FPW; i0 += 8) {
-                    float2 yv[8];
-                    if (MT > 0) {
-#pragma unroll
-                        for (int g = 0; g < 8; ++g) yv[g] = fmul2(rg.tap[0], rg.row[i0 + g + WA - 1]);
-#pragma unroll
-                        for (int m = 1; m < WA; ++m)
-#pragma unroll
-                            for (int g = 0; g < 8; ++g) yv[g] = ffma2(rg.tap[m], rg.row[i0 + g + WA - 1 - m], yv[g]);
-                    } else {
-#pragma unroll
-                        for (int g = 0; g < 8; ++g) yv[g] = rg.row[i0 + g];
-                    }
+                auto convert = [&](const float2 (&yv)[8], uint32_t (&hb)[8], uint32_t (&lb)[8]) {
 #pragma unroll
                     for (int g = 0; g < 8; ++g) {
-                        const int i = i0 + g;
-                        uint32_t hb;
-                        if (parts == 1 && prm.fp16) { const __half2 hh = __floats2half2_rn(yv[g].x, yv[g].y); hb = *reinterpret_cast<const uint32_t*>(&hh); }
-                        else { const __nv_bfloat162 hi = __floats2bfloat162_rn(yv[g].x, yv[g].y); hb = *reinterpret_cast<const uint32_t*>(&hi); }
-                        const uint32_t addr = cell0[(i >> 1) & 3] + so + (uint32_t)i * 64u;
-                        sts16(addr, hb);
-                        sts16(addr + im_off, hb >> 16);
+                        if (parts == 1 && prm.fp16) { const __half2 hh = __floats2half2_rn(yv[g].x, yv[g].y); hb[g] = *reinterpret_cast<const uint32_t*>(&hh); }
+                        else { const __nv_bfloat162 hi = __floats2bfloat162_rn(yv[g].x, yv[g].y); hb[g] = *reinterpret_cast<const uint32_t*>(&hi); }
                         if (parts > 1) {
-                            const float lx = yv[g].x - __uint_as_float(hb << 16);
-                            const float ly = yv[g].y - __uint_as_float(hb & 0xffff0000u);
+                            const float lx = yv[g].x - __uint_as_float(hb[g] << 16);
+                            const float ly = yv[g].y - __uint_as_float(hb[g] & 0xffff0000u);
                             const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
-                            const uint32_t lb = *reinterpret_cast<const uint32_t*>(&lo);
-                            sts16(addr + ST_TILE, lb);
-                            sts16(addr + im_off + ST_TILE, lb >> 16);
+                            lb[g] = *reinterpret_cast<const uint32_t*>(&lo);
+                        } else lb[g] = 0u;
+                    }
+                };
+                auto store_frame = [&](int i, uint32_t hb, uint32_t lb) {
+                    const uint32_t addr = cell0[(i >> 1) & 3] + so + (uint32_t)i * 64u;
+                    sts16(addr, hb);
+                    sts16(addr + im_off, hb >> 16);
+                    if (parts > 1) {
+                        sts16(addr + ST_TILE, lb);
+                        sts16(addr + im_off + ST_TILE, lb >> 16);
+                    }
+                };
+                float2 yv[8];
+                uint32_t hb0[8], lb0[8];
+                if (MT > 1) {
+                    constexpr int FGN = 4, NG = FPW / FGN;                // frames per group, groups
+#pragma unroll
+                    for (int k = 0; k < NG; ++k) {
+                        // MAC of group k; the stores of group k - 1 (converted below) leave underneath it
+#pragma unroll
+                        for (int g = 0; g < FGN; ++g) yv[g] = fmul2(rg.tap[0], rg.row[k * FGN + g + WA - 1]);
+#pragma unroll
+                        for (int m = 1; m < WA; ++m) {
+#pragma unroll
+                            for (int g = 0; g < FGN; ++g) yv[g] = ffma2(rg.tap[m], rg.row[k * FGN + g + WA - 1 - m], yv[g]);
+                            if (k > 0) {
+#pragma unroll
+                                for (int f = 0; f < FGN; ++f)
+                                    if (f * (WA - 1) / FGN == m - 1) store_frame((k - 1) * FGN + f, hb0[f], lb0[f]);
+                            }
                         }
+#pragma unroll
+                        for (int g = FGN; g < 8; ++g) yv[g] = make_float2(0.f, 0.f);
+                        convert(yv, hb0, lb0);
+                    }
+#pragma unroll
+                    for (int g = 0; g < FGN; ++g) store_frame((NG - 1) * FGN + g, hb0[g], lb0[g]);
+                } else {
+#pragma unroll
+                    for (int i0 = 0; i0 < FPW; i0 += 8) {
+#pragma unroll
+                        for (int g = 0; g < 8; ++g) yv[g] = MT == 1 ? fmul2(rg.tap[0], rg.row[i0 + g]) : rg.row[i0 + g];
+                        convert(yv, hb0, lb0);
+#pragma unroll
+                        for (int g = 0; g < 8; ++g) store_frame(i0 + g, hb0[g], lb0[g]);
                     }
                 }
                 // the window has been consumed: hand the input slot back to the TMA warp
