@@ -266,6 +266,38 @@ def test_pfb_many_taps_two_launch_route(tina, oracle, P, M, F, real, S):
         assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
 
 
+@pytest.mark.parametrize("P,M,F,real,S", [(320, 5, 300, False, 1), (192, 3, 257, False, 2), (8192, 1, 40, False, 1),
+                                           (320, 4, 200, True, 1), (256, 16, 100, True, 2), (128, 1, 513, True, 1),
+                                           (1024, 16, 700, False, 3), (4096, 8, 300, True, 1), (64, 16, 1000, False, 1)])
+def test_pfb_column_paired_kernel_shapes(tina, oracle, P, M, F, real, S):
+    """Shapes that exercise the column-paired kernel's tiling (tina_sym.cu): a last pass narrower than 128 bins
+    (P = 320, 192), one 32-element chunk per pass (P = 64), the longest contraction (P = 8192: eight accumulation
+    chains with add-reduce epilogues), M below / at the unrolled tap counts, several streams, ragged frame tiles;
+    both variants (TMA-staged input, and register-window producers where they exist) give the oracle's result."""
+    rng = np.random.default_rng(640 + P + M)
+    case = ti.pfb_case(P, M, F, real=real, streams=S, seed=641 + P + F, window=ti.random_taps(rng, P * M))
+    got = _run_pfb(tina, case)
+    assert tina.last_kernel().startswith("pfb_symt_kernel")
+    for s in range(S):
+        ref = oracle.pfb(case.x[s], P, M, case.window)
+        assert rel_l2_rows(got[s], ref) <= TOL_FP32
+        if real:
+            assert np.all(got[s][:, 0].imag == 0) and np.all(got[s][:, P // 2].imag == 0)
+
+
+def test_pfb_column_paired_variants_agree(tina, oracle, tina_env):
+    """TINA_SYM_V1 (register-window producers) and TINA_NO_SYM (round-1 block-form kernel) stay correct."""
+    case = ti.pfb_case(1024, 16, 300, streams=2, seed=655)
+    ref = [oracle.pfb(case.x[s], 1024, 16, case.window) for s in range(2)]
+    for env, name in (({"TINA_SYM_V1": 1}, "pfb_sym_kernel"), ({"TINA_NO_SYM": 1}, "pfb_umma_kernel")):
+        tina_env(**env)
+        got = _run_pfb(tina, case)
+        assert tina.last_kernel() == name
+        for s in range(2):
+            assert rel_l2_rows(got[s], ref[s]) <= TOL_FP32
+        tina_env(**{k: 0 for k in env})
+
+
 def test_pfb_complex_multichain_batched(tina, oracle):
     """Complex kind, K = 4096: four accumulation chains (TMA add-reduce epilogue), 8 column passes,
     ragged last tile, 2 streams."""
