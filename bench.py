@@ -248,7 +248,7 @@ def run_peaks(args):
     import torch
     import paper_2408_16551_b200 as tina
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
-    names = {0: "ffma_fp32", 1: "ffma2_fp32", 2: "tcgen05_tf32", 3: "tcgen05_bf16"}
+    names = {0: "ffma_fp32", 1: "ffma2_fp32", 2: "tcgen05_tf32", 3: "tcgen05_bf16", 4: "tcgen05_bf16_n128", 5: "tcgen05_bf16_n64"}
     out = {}
     for which, name in names.items():
         base = 4096 if which < 2 else 2048

@@ -18,7 +18,7 @@
  * several host threads and on several devices of one process (state is kept per CUDA device; the
  * current device at call time is the one used).  The `_host` entry point serialises per device.
  * Environment: TINA_* variant switches (TINA_SHARE, TINA_NT256, TINA_NO_OUT_TMA, TINA_FIR_SIMT,
- * TINA_CT_NO_WS, TINA_CTR_WS, TINA_NO_SYM, TINA_SYM_V1) select between kernels that compute the same result under the
+ * TINA_FIR_V1, TINA_CT_NO_WS, TINA_CTR_WS, TINA_NO_SYM, TINA_SYM_V1) select between kernels that compute the same result under the
  * same contract; they are read once (tina_reload_options() re-reads them).  Knobs that skip work or
  * change the accuracy contract exist only in development builds (-DTINA_DEV, tina_build_is_dev()).
  *
@@ -181,7 +181,7 @@ int         tina_build_is_dev(void);             /* 1: built with -DTINA_DEV (de
 /* Measured arithmetic ceilings of the device (bare loops, no memory traffic; the denominators of the
  * rooflines bench.py reports -- SURVEY.md section 8(d)).  which: 0 = fp32 fma.rn.f32 on the CUDA cores,
  * 1 = packed fma.rn.f32x2, 2 = tcgen05.mma kind::tf32, 3 = tcgen05.mma kind::f16 with bf16 operands
- * (M = 128, N = 256 per instruction, operands in shared memory).  Runs `iters` loop iterations per thread
+ * (M = 128, N = 256 per instruction, operands in shared memory), 4 / 5 = the bf16 loop with N = 128 / 64.  Runs `iters` loop iterations per thread
  * (FMA) or MMA groups per SM (tensor) after a short warm-up, SYNCHRONISES, and returns TFLOP/s in *tflops
  * and the elapsed milliseconds in *ms (host pointers; ms may be NULL).                                  */
 tina_status tina_probe_peak(int which, int iters, double* tflops, double* ms, void* stream);

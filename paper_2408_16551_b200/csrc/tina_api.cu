@@ -49,6 +49,7 @@ static void load_options_locked()
     o.share = on("TINA_SHARE") && !on("TINA_NO_SHARE");
     o.no_out_tma = on("TINA_NO_OUT_TMA");
     o.fir_simt = on("TINA_FIR_SIMT");
+    o.fir_v1 = on("TINA_FIR_V1");
     o.ct_no_ws = on("TINA_CT_NO_WS");
     o.ctr_ws = on("TINA_CTR_WS");
     o.no_sym = on("TINA_NO_SYM");
@@ -183,6 +184,7 @@ tina_status tina_fir(const float* x, const float* taps, float* y, int C, long lo
     if ((const void*)x == (const void*)y) return fail(TINA_ERR_BAD_SHAPE, "tina_fir: in-place not supported");
     if (!aligned16(x) || !aligned16(y)) return fail(TINA_ERR_ALIGNMENT, "tina_fir: x, y must be 16-byte aligned");
     tina_status fs = TINA_OK;
+    if (firt_fir(x, taps, y, C, L, M, false, (cudaStream_t)stream, &fs)) return fs;
     if (umma_fir(x, taps, y, C, L, M, (cudaStream_t)stream, &fs)) return fs;
     return simt_fir(x, taps, y, C, L, M, (cudaStream_t)stream);
 }
@@ -194,6 +196,8 @@ tina_status tina_fir_multi(const float* x, const float* taps, float* y, int C, l
     if (M > kMaxTapsFir) return fail(TINA_ERR_UNSUPPORTED, "tina_fir_multi: M > %d", kMaxTapsFir);
     if ((const void*)x == (const void*)y) return fail(TINA_ERR_BAD_SHAPE, "tina_fir_multi: in-place not supported");
     if (!aligned16(x) || !aligned16(y)) return fail(TINA_ERR_ALIGNMENT, "tina_fir_multi: x, y must be 16-byte aligned");
+    tina_status fs = TINA_OK;
+    if (firt_fir(x, taps, y, C, L, M, true, (cudaStream_t)stream, &fs)) return fs;
     return simt_fir(x, taps, y, C, L, M, (cudaStream_t)stream, true);
 }
 
@@ -427,7 +431,7 @@ int tina_build_is_dev(void)
 tina_status tina_probe_peak(int which, int iters, double* tflops, double* ms, void* stream)
 {
     if (!tflops) return fail(TINA_ERR_NULL_POINTER, "tina_probe_peak: null pointer");
-    if (which < 0 || which > 3 || iters < 1) return fail(TINA_ERR_BAD_SHAPE, "tina_probe_peak: which in 0..3, iters >= 1");
+    if (which < 0 || which > 5 || iters < 1) return fail(TINA_ERR_BAD_SHAPE, "tina_probe_peak: which in 0..5, iters >= 1");
     return probe_peak(which, iters, tflops, ms, (cudaStream_t)stream);
 }
 

@@ -36,6 +36,7 @@ struct Options {
     bool share = false;        // TINA_SHARE: clusters of four share the subfilter stage (dense kernel)
     bool no_out_tma = false;   // TINA_NO_OUT_TMA: real-kind epilogue through registers instead of TMA stores
     bool fir_simt = false;     // TINA_FIR_SIMT: tina_fir on the CUDA-core kernel even where the Toeplitz path applies
+    bool fir_v1 = false;       // TINA_FIR_V1: Toeplitz FIR through the round-1 route (pfb_umma_kernel) instead of fir_umma_kernel
     bool ct_no_ws = false;     // TINA_CT_NO_WS: factorised complex kernel without warp specialisation
     bool ctr_ws = false;       // TINA_CTR_WS: warp-specialised factorised real kernel
     bool no_sym = false;       // TINA_NO_SYM: complex dense contraction without the k <-> P-k column pairing
@@ -106,6 +107,10 @@ tina_status arith_ew(const float* a, const float* b, float* o, long long n, bool
 tina_status arith_sum(const float* x, long long rows, long long n, float* out, cudaStream_t st);
 tina_status arith_matmul(const float* x, const float* y, float* z, long long M, long long L, long long N, cudaStream_t st);
 tina_status ctr_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st);
+// standalone FIR as a Toeplitz contraction with a resident matrix and TMA-staged signal (tina_firt.cu);
+// false = shape not covered (L % 128 != 0 or M > 193): fall back to umma_fir / simt_fir
+bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, int M, bool per_channel, cudaStream_t st,
+              tina_status* status);
 // standalone FIR as a Toeplitz contraction on the tensor cores; false = shape not covered (use simt_fir)
 bool umma_fir(const float* x, const float* taps, float* y, int C, long long L, int M, cudaStream_t st,
               tina_status* status);

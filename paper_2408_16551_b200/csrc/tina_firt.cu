@@ -1,0 +1,385 @@
+// tina_firt.cu -- standalone FIR (Eq. (15)) as a banded-Toeplitz contraction on the tensor cores,
+// round-2 kernel: the paper's unfolding view (Eq. (17)-(19)).
+//
+// A channel is cut into blocks of T = 128 outputs; block b needs the T + M - 1 inputs x[bT .. bT + T + M - 2]:
+//     y[bT + n] = sum_c x[bT + c] * Tz[c][n],      Tz[c][n] = a[n + M-1 - c]   (0 outside the band 0 <= . < M)
+// i.e. a GEMM whose A rows are overlapping windows of the signal (row pitch T) and whose B is the fixed Toeplitz
+// matrix of the taps, K = T + M - 1 padded to a multiple of 32.  fp32 accuracy as everywhere in libtina: A and B
+// split into bf16 hi + lo, three products (lo*hi, hi*hi, hi*lo), fp32 accumulation in TMEM.
+//
+// What differs from the round-1 route through pfb_umma_kernel (measured there: the issuing thread needed ~207
+// cycles per M256 x N128 x K16 instruction against ~90 for the bare loop, producers busy 70 % on exposed global
+// load latency, 0.46 of the HBM roofline):
+//   * the Toeplitz matrix is built ONCE per CTA from the taps, straight into shared memory, and stays resident
+//     (no per-call toeplitz_kernel, no tensor map, no B ring, no L2 traffic for B);
+//   * the signal is staged by TMA: a 3-D map {128, L / 128, C} over x, boxes of 32 floats x 128 rows; chunk kc of
+//     a tile is the box at column 32 (kc % 4) of row (tile row + kc / 4) -- the overlap of the A rows costs
+//     nothing but L2 bandwidth, and rows past the end of a channel arrive as zeros;
+//   * the producers only convert: ld.shared.v2 -> bf16x2 hi, exact remainder, bf16x2 lo -> two conflict-free
+//     32-bit st.shared into the 64-byte-swizzled A tiles;
+//   * four TMEM accumulator stages of 128 columns, so the epilogue of a tile overlaps the MMAs of the next three.
+// CTA pair, tcgen05.mma.cta_group::2, M = 256 (each CTA 128 rows), N = 128 (each CTA holds 64 rows of B).
+// Needs L % 128 == 0 (the 3-D view) and M <= 193; other shapes keep the round-1 route or the CUDA-core kernel.
+#include "tina_umma.cuh"
+
+#include <cstring>
+
+namespace tina {
+
+using namespace ptx;
+
+constexpr int FT_T = 128;                         // outputs per block (GEMM N) and A row pitch
+constexpr int FT_KC = 32;                         // contraction elements per chunk (64-byte rows, SWIZZLE_64B)
+constexpr int FT_A_TILE = BM * FT_KC * 2;         // 8 KB
+constexpr int FT_A_SLOT = 2 * FT_A_TILE;          // hi | lo
+constexpr int FT_B_TILE = (FT_T / UMMA_CG) * FT_KC * 2;   // 4 KB: this CTA's 64 rows of one chunk and part
+constexpr int FT_IN_SLOT = BM * FT_KC * 4;        // 16 KB fp32
+constexpr int FT_PITCH = 132;                     // staged row pitch (floats) of the epilogue
+constexpr int FT_STAGE = 32 * FT_PITCH * 4;       // per epilogue warp
+constexpr int FT_ACC = 4;                         // TMEM accumulator stages of 128 columns
+
+struct FirtCtl {
+    uint64_t a_full[4], a_empty[4];
+    uint64_t in_full[4], in_empty[4];
+    uint64_t t_full[FT_ACC], t_empty[FT_ACC];
+    uint64_t b_free, b_ready;          // per-channel taps: "all MMAs that read the old matrix are done" / "new matrix written"
+    uint32_t tmem_base;
+};
+
+struct FirtParams {
+    const float* taps;         // [M] (taps_stride == 0) or [C][M]
+    float* y;                  // [C][Lo]
+    long long Lo;              // outputs per channel
+    int M, n_kc;               // taps, chunks (Kp / 32)
+    int taps_stride;           // 0: one tap vector; M: one per channel
+    int tiles_per_chan, total_work;
+    int a_slots, in_slots;     // ring depths
+};
+
+__device__ __forceinline__ float2 firt_lds_f2(uint32_t addr)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void firt_sts16(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared.b16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+
+__global__ void __launch_bounds__(UMMA_THREADS, 1)
+fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    if ((smem_u32(smem) & 1023u) != 0) __trap();
+    constexpr int CG = UMMA_CG;
+    const int n_kc = prm.n_kc;
+    uint8_t* b_res = smem;                                               // [n_kc][hi | lo] x 4 KB
+    uint8_t* a_ring = b_res + (size_t)n_kc * 2 * FT_B_TILE;               // multiples of 8 KB: 1024-aligned
+    uint8_t* in_ring = a_ring + (size_t)prm.a_slots * FT_A_SLOT;
+    uint8_t* stage = in_ring + (size_t)prm.in_slots * FT_IN_SLOT;
+    FirtCtl* ctl = reinterpret_cast<FirtCtl*>(stage + 4 * FT_STAGE);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    constexpr uint32_t leader = 0;
+    constexpr uint16_t pair_mask = 3;
+    const int cl = blockIdx.x / CG, n_cl = gridDim.x / CG;
+    const uint32_t n_a = (uint32_t)prm.a_slots, n_in = (uint32_t)prm.in_slots;
+    // contiguous ranges of tiles per pair: a pair stays inside a channel as long as possible (per-channel taps
+    // rebuild the Toeplitz matrix only when the channel changes)
+    const int per = (prm.total_work + n_cl - 1) / n_cl;
+    const int w_begin = min(cl * per, prm.total_work), w_end = min(w_begin + per, prm.total_work);
+
+    if (warp == TMA_WARP && lane == 0) {
+        prefetch_tmap(&tmap_x);
+        for (int i = 0; i < 4; ++i) {
+            mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0));
+            mbar_init(smem_u32(&ctl->a_empty[i]), 1);
+            mbar_init(smem_u32(&ctl->in_full[i]), 1);
+            mbar_init(smem_u32(&ctl->in_empty[i]), N_PROD_WARPS);
+        }
+        for (int i = 0; i < FT_ACC; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
+        mbar_init(smem_u32(&ctl->b_free), 1);
+        mbar_init(smem_u32(&ctl->b_ready), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0));
+        fence_mbar_init();
+    }
+    if (warp == ALLOC_WARP) {
+        tmem_alloc<CG>(smem_u32(&ctl->tmem_base), 512);
+        tmem_relinquish<CG>();
+    }
+    // Toeplitz matrix of channel `chan` (this CTA's 64 output columns n = 64 rank + nl), bf16 hi | lo, K-major,
+    // 64-byte-swizzled: element (nl, c) of chunk c / 32 at row nl, 16-byte chunk ((c % 32) >> 3) ^ ((nl >> 1) & 3)
+    auto build_b = [&](int chan, int tid, int nthreads) {
+        const float* taps = prm.taps + (long long)chan * prm.taps_stride;
+        const int Kp = n_kc * FT_KC, M = prm.M;
+        const uint32_t b_s = smem_u32(b_res);
+        for (int idx = tid; idx < (FT_T / CG) * Kp; idx += nthreads) {
+            const int nl = idx / Kp, c = idx - nl * Kp;
+            const int k = (int)rank * (FT_T / CG) + nl + M - 1 - c;
+            const float v = (k >= 0 && k < M) ? __ldg(taps + k) : 0.f;
+            const __nv_bfloat16 hi = __float2bfloat16(v);
+            const __nv_bfloat16 lo = __float2bfloat16(v - __bfloat162float(hi));
+            const int cc = c & (FT_KC - 1);
+            const uint32_t off = (uint32_t)(c / FT_KC) * 2u * FT_B_TILE + (uint32_t)nl * 64u +
+                                 ((((uint32_t)cc >> 3) ^ (((uint32_t)nl >> 1) & 3u)) << 4) + ((uint32_t)cc & 7u) * 2u;
+            firt_sts16(b_s + off, (uint32_t)__bfloat16_as_ushort(hi));
+            firt_sts16(b_s + off + FT_B_TILE, (uint32_t)__bfloat16_as_ushort(lo));
+        }
+    };
+    if (prm.taps_stride == 0 || w_begin < w_end) build_b(prm.taps_stride ? w_begin / prm.tiles_per_chan : 0, threadIdx.x, UMMA_THREADS);
+    fence_proxy_async();
+    tc_fence_before();
+    cluster_sync();
+    tc_fence_after();
+    const uint32_t tmem_base = ctl->tmem_base;
+    // per-channel taps: tile w starts a new channel (the pair's first tile was built above)
+    auto new_channel = [&](int w) { return prm.taps_stride != 0 && w > w_begin && (w % prm.tiles_per_chan) == 0; };
+
+    if (warp == TMA_WARP) {
+        // ============================ TMA producer: signal rows ================================
+        if (lane == 0) {
+            RingPos in;
+            for (int w = w_begin; w < w_end; ++w) {
+                const int chan = w / prm.tiles_per_chan;
+                const int row0 = (w % prm.tiles_per_chan) * (BM * CG) + (int)rank * BM;
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    mbar_wait<64>(smem_u32(&ctl->in_empty[in.idx]), in.phase ^ 1);
+                    const uint32_t bar = smem_u32(&ctl->in_full[in.idx]);
+                    mbar_expect_tx(bar, FT_IN_SLOT);
+                    tma_load_3d(smem_u32(in_ring + in.idx * FT_IN_SLOT), &tmap_x, bar, FT_KC * (kc & 3), row0 + (kc >> 2), chan);
+                    in.advance(n_in);
+                }
+            }
+        }
+    } else if (warp == MMA_WARP) {
+        // ============================ MMA issuer =============================================
+        if (rank != 0) {
+            RingPos a;                                    // forward "my A tile is ready" to the leader
+            uint32_t br_phase = 0;
+            for (int w = w_begin; w < w_end; ++w) {
+                if (new_channel(w)) {                     // ... and "my half of the new Toeplitz matrix is written"
+                    mbar_wait(smem_u32(&ctl->b_ready), br_phase);
+                    br_phase ^= 1u;
+                    if (lane == 0) mbar_arrive_cluster(smem_u32(&ctl->b_ready), leader);
+                    __syncwarp();
+                }
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                    if (lane == 0) mbar_arrive_cluster(smem_u32(&ctl->a_full[a.idx]), leader);
+                    __syncwarp();
+                    a.advance(n_a);
+                }
+            }
+        } else {
+            RingPos a, t;
+            uint32_t br_phase = 0;
+            const uint32_t idesc = idesc_bf16(BM * CG, FT_T, false);
+            const uint32_t b_s = smem_u32(b_res);
+            for (int w = w_begin; w < w_end; ++w) {
+                if (new_channel(w)) {
+                    // every MMA issued so far has read the old matrix: release it once they are done, then wait
+                    // until both CTAs have written the new one
+                    if (lane == 0) commit_cg<CG>(smem_u32(&ctl->b_free), pair_mask);
+                    __syncwarp();
+                    mbar_wait(smem_u32(&ctl->b_ready), br_phase);
+                    br_phase ^= 1u;
+                    tc_fence_after();
+                }
+                mbar_wait(smem_u32(&ctl->t_empty[t.idx]), t.phase ^ 1);      // the epilogue has drained this stage
+                tc_fence_after();
+                const uint32_t d = tmem_base + t.idx * (uint32_t)FT_T;
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                    tc_fence_after();
+                    if (lane == 0) {
+                        const uint64_t a_hi = smem_desc_sw64(smem_u32(a_ring + a.idx * FT_A_SLOT));
+                        const uint64_t a_lo = smem_desc_sw64(smem_u32(a_ring + a.idx * FT_A_SLOT + FT_A_TILE));
+                        const uint64_t b_hi = smem_desc_sw64(b_s + (uint32_t)kc * 2u * FT_B_TILE);
+                        const uint64_t b_lo = smem_desc_sw64(b_s + (uint32_t)kc * 2u * FT_B_TILE + FT_B_TILE);
+                        uint32_t acc = kc > 0;
+#pragma unroll
+                        for (int k = 0; k < FT_KC / 16; ++k) { umma_bf16<CG>(d, a_lo + 2 * k, b_hi + 2 * k, idesc, acc); acc = 1; }
+#pragma unroll
+                        for (int k = 0; k < FT_KC / 16; ++k) umma_bf16<CG>(d, a_hi + 2 * k, b_hi + 2 * k, idesc, 1);
+#pragma unroll
+                        for (int k = 0; k < FT_KC / 16; ++k) umma_bf16<CG>(d, a_hi + 2 * k, b_lo + 2 * k, idesc, 1);
+                        commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
+                        if (kc == n_kc - 1) commit_cg<CG>(smem_u32(&ctl->t_full[t.idx]), pair_mask);
+                    }
+                    __syncwarp();
+                    a.advance(n_a);
+                }
+                t.advance(FT_ACC);
+            }
+        }
+    } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
+        // ============================ epilogue ==============================================
+        // The warp's 32 rows x 128 columns are ONE contiguous run of 4096 floats of y[chan] that is only 4-byte
+        // aligned (Lo is odd for even L and M): stage it (row pitch 132 floats), hand the accumulator back, and
+        // write the run as 16-byte-aligned float4 with a scalar head and tail.
+        const int q = warp - EPI_WARP0;
+        float* stg = reinterpret_cast<float*>(stage + q * FT_STAGE);
+        RingPos t;
+        for (int w = w_begin; w < w_end; ++w) {
+            const int chan = w / prm.tiles_per_chan;
+            const long long row0 = (long long)(w % prm.tiles_per_chan) * (BM * CG) + rank * BM + q * 32;
+            mbar_wait<128>(smem_u32(&ctl->t_full[t.idx]), t.phase);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + t.idx * (uint32_t)FT_T + ((uint32_t)(q * 32) << 16);
+            uint32_t r[32];
+            tmem_ld32(taddr, r);
+#pragma unroll
+            for (int cb = 0; cb < FT_T; cb += 32) {
+                tmem_ld_wait();
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    *reinterpret_cast<float4*>(stg + lane * FT_PITCH + cb + 4 * j) =
+                        make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
+                                    __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
+                if (cb + 32 < FT_T) tmem_ld32(taddr + cb + 32, r);
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[t.idx]), rank, leader);
+            const long long e0 = row0 * FT_T;                              // first element of the run in the channel
+            long long n_run = prm.Lo - e0;
+            if (n_run > 32LL * FT_T) n_run = 32LL * FT_T;
+            if (n_run > 0) {
+                float* g = prm.y + (long long)chan * prm.Lo + e0;
+                const int run = (int)n_run;
+                const int head = min(run, (int)(((16u - ((uint32_t)(uintptr_t)g & 15u)) & 15u) >> 2));
+                const int nv4 = (run - head) >> 2;
+                auto at = [&](int l) { return stg[(l >> 7) * FT_PITCH + (l & 127)]; };
+                if (lane < head) g[lane] = at(lane);
+                for (int v = lane; v < nv4; v += 32) {
+                    const int l = head + 4 * v;
+                    *reinterpret_cast<float4*>(g + l) = make_float4(at(l), at(l + 1), at(l + 2), at(l + 3));
+                }
+                const int tail0 = head + 4 * nv4;
+                if (tail0 + lane < run) g[tail0 + lane] = at(tail0 + lane);
+            }
+            __syncwarp();
+            t.advance(FT_ACC);
+        }
+    } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
+        // ============================ producers: fp32 -> bf16 hi / lo =========================
+        // warp pw converts rows 16 pw .. +15 of the staged 128 x 32 block; lanes 0-15 take an even row, lanes
+        // 16-31 the next one, each lane two adjacent contraction elements (one 32-bit operand word per part).
+        const int pw = warp - PROD_WARP0;
+        const uint32_t hl = (uint32_t)lane >> 4, wl = (uint32_t)lane & 15u;
+        const uint32_t in_lane = smem_u32(in_ring) + ((uint32_t)(pw * FPW) + hl) * 128u + wl * 8u;
+        const uint32_t a_lane = smem_u32(a_ring) + ((uint32_t)(pw * FPW) + hl) * 64u + (wl & 3u) * 4u;
+        const uint32_t wc = wl >> 2;                                       // 16-byte chunk of the operand word
+        RingPos in, a;
+        uint32_t bf_phase = 0;
+        for (int w = w_begin; w < w_end; ++w) {
+            if (new_channel(w)) {
+                mbar_wait(smem_u32(&ctl->b_free), bf_phase);
+                bf_phase ^= 1u;
+                build_b(w / prm.tiles_per_chan, pw * 32 + lane, N_PROD_WARPS * 32);
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));
+            }
+            for (int kc = 0; kc < n_kc; ++kc) {
+                mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase);
+                float2 v[FPW / 2];
+#pragma unroll
+                for (int i = 0; i < FPW / 2; ++i) v[i] = firt_lds_f2(in_lane + in.idx * FT_IN_SLOT + (uint32_t)i * 256u);
+                mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
+#pragma unroll
+                for (int i = 0; i < FPW / 2; ++i) {
+                    const __nv_bfloat162 hi = __floats2bfloat162_rn(v[i].x, v[i].y);
+                    const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
+                    const __nv_bfloat162 lo = __floats2bfloat162_rn(v[i].x - __uint_as_float(hb << 16),
+                                                                     v[i].y - __uint_as_float(hb & 0xffff0000u));
+                    // row r = 16 pw + 2 i + hl: swizzle phase (r >> 1) & 3 = i & 3
+                    const uint32_t addr = a_lane + a.idx * FT_A_SLOT + (uint32_t)i * 128u + ((wc ^ ((uint32_t)i & 3u)) << 4);
+                    sts32(addr, hb);
+                    sts32(addr + FT_A_TILE, *reinterpret_cast<const uint32_t*>(&lo));
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
+                in.advance(n_in);
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[a.idx]));
+                a.advance(n_a);
+            }
+        }
+    }
+
+    tc_fence_before();
+    cluster_sync();
+    if (warp == ALLOC_WARP) tmem_dealloc<CG>(tmem_base, 512);
+}
+
+// true if this kernel handled the call (shared taps: taps [M]; per_channel: taps [C][M])
+bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, int M, bool per_channel, cudaStream_t st,
+              tina_status* status)
+{
+    if (M > 193 || L % FT_T != 0 || L / FT_T > 0x7fffffffLL || options().fir_simt || options().fir_v1) return false;
+    const long long Lo = L - M + 1;
+    const int Kp = (FT_T + M - 1 + FT_KC - 1) / FT_KC * FT_KC;
+    const int n_kc = Kp / FT_KC;
+    const long long R = (Lo + FT_T - 1) / FT_T;                      // output blocks (A rows) per channel
+    const long long tps = (R + BM * UMMA_CG - 1) / (BM * UMMA_CG);
+    if (tps * C > 0x7fffffffLL) return false;
+    DevCtx* ctx = nullptr;
+    if ((*status = dev_ctx(&ctx)) != TINA_OK) return true;
+
+    FirtParams prm;
+    memset(&prm, 0, sizeof(prm));
+    prm.taps = taps; prm.y = y; prm.Lo = Lo; prm.M = M; prm.n_kc = n_kc;
+    prm.taps_stride = per_channel ? M : 0;
+    prm.tiles_per_chan = (int)tps;
+    prm.total_work = (int)(tps * C);
+    const size_t fixed = (size_t)n_kc * 2 * FT_B_TILE + 4 * FT_STAGE + sizeof(FirtCtl);
+    prm.a_slots = 4; prm.in_slots = 4;
+    while (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) {
+        if (prm.in_slots > 2 && prm.in_slots >= prm.a_slots) --prm.in_slots;
+        else if (prm.a_slots > 2) --prm.a_slots;
+        else return false;
+    }
+    const size_t smem = fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT;
+
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) { *status = fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found"); return true; }
+    CUtensorMap tmap_x;
+    memset(&tmap_x, 0, sizeof(tmap_x));
+    {
+        const cuuint32_t estr[3] = {1, 1, 1};
+        const cuuint64_t dims[3] = {(cuuint64_t)FT_T, (cuuint64_t)(L / FT_T), (cuuint64_t)C};
+        const cuuint64_t strides[2] = {(cuuint64_t)FT_T * sizeof(float), (cuuint64_t)L * sizeof(float)};
+        const cuuint32_t box[3] = {FT_KC, BM, 1};
+        CUresult r = enc(&tmap_x, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(x), dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { *status = fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(fir input) failed (%d)", (int)r); return true; }
+    }
+    if ((*status = ensure_smem(ctx, reinterpret_cast<const void*>(fir_umma_kernel), 232448, "cudaFuncSetAttribute(fir_umma_kernel)")) != TINA_OK)
+        return true;
+    const int n_cl = ctx->n_sm / UMMA_CG;
+    const int grid = UMMA_CG * (prm.total_work < n_cl ? prm.total_work : n_cl);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(UMMA_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = UMMA_CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, fir_umma_kernel, tmap_x, prm);
+    count_launch();
+    g_last_path = kPathUmma;
+    note_kernel(per_channel ? "fir_umma_kernel<per-channel taps>" : "fir_umma_kernel");
+    *status = e != cudaSuccess ? check_cuda(e, "fir_umma_kernel launch") : check_cuda(cudaGetLastError(), "fir_umma_kernel launch");
+    return true;
+}
+
+}  // namespace tina

@@ -6,6 +6,8 @@
 //   TINA_PEAK_TF32   tcgen05.mma kind::tf32   (M = 128, N = 256, K = 8 per instruction, operands in smem)
 //   TINA_PEAK_BF16   tcgen05.mma kind::f16    (bf16, M = 128, N = 256, K = 16) -- cross-check of the
 //                                              driver's cuBLAS figure in MEASURED_PEAKS.json
+//   4 / 5            the same bf16 loop with N = 128 / N = 64 columns per instruction (how the tensor rate
+//                    falls with narrow tiles: the Toeplitz FIR uses N = 128)
 // Operands are pseudo-random (not zeros): the tensor-pipe power draw, and with it the clock the part
 // sustains, depends on the data toggling.
 #include "tina_common.cuh"
@@ -53,7 +55,7 @@ __device__ __forceinline__ void umma_tf32_cg1(uint32_t d_tmem, uint64_t adesc, u
 
 template <bool TF32>
 __global__ void __launch_bounds__(128, 1)
-peak_umma_kernel(int iters)
+peak_umma_kernel(int iters, int n_cols)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* a_tile = smem;                         // 16 KB
@@ -79,7 +81,7 @@ peak_umma_kernel(int iters)
         const uint64_t ad = smem_desc_sw128(smem_u32(a_tile)), bd = smem_desc_sw128(smem_u32(b_tile));
         // kind::tf32: a/b format 2; kind::f16 with bf16: format 1; fp32 accumulate; M = 128, N = 256
         const uint32_t fmt = TF32 ? 2u : 1u;
-        const uint32_t idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((256u >> 3) << 17) | ((128u >> 4) << 24);
+        const uint32_t idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | (((uint32_t)n_cols >> 3) << 17) | ((128u >> 4) << 24);
         uint32_t phase = 0;
         for (int it = 0; it < iters; ++it) {
             const uint32_t d = tmem + (uint32_t)(it & 1) * 256u;
@@ -119,9 +121,10 @@ tina_status probe_peak(int which, int iters, double* tflops, double* ms_out, cud
             flops = (double)blocks * 512 * (double)n * 16 * 2;
         } else {
             const int smem = 49152 + 128;
-            if (which == 2) peak_umma_kernel<true><<<ctx->n_sm, 128, smem, st>>>(n);
-            else            peak_umma_kernel<false><<<ctx->n_sm, 128, smem, st>>>(n);
-            flops = (double)ctx->n_sm * (double)n * 4 * 2.0 * 128 * 256 * (which == 2 ? 8 : 16);
+            const int ncols = which == 4 ? 128 : (which == 5 ? 64 : 256);
+            if (which == 2) peak_umma_kernel<true><<<ctx->n_sm, 128, smem, st>>>(n, ncols);
+            else            peak_umma_kernel<false><<<ctx->n_sm, 128, smem, st>>>(n, ncols);
+            flops = (double)ctx->n_sm * (double)n * 4 * 2.0 * 128 * ncols * (which == 2 ? 8 : 16);
         }
         count_launch();
         return cudaGetLastError();

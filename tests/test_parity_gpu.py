@@ -94,6 +94,39 @@ def test_fir_toeplitz_tensor_path(tina, oracle, C, L, K):
     assert np.allclose(yi.cpu().numpy()[0, :K], a, rtol=2e-5, atol=1e-6 * np.abs(a).max())
 
 
+@pytest.mark.parametrize("C,L,K", [(1, 128, 64), (3, 4096, 1), (2, 128 * 70, 64), (5, 128 * 300, 193), (2, 128 * 257, 33),
+                                   (3, 128 * 1025, 64), (70, 128 * 40, 17)])
+@pytest.mark.parametrize("per_channel", [False, True])
+def test_fir_resident_toeplitz_kernel(tina, oracle, C, L, K, per_channel):
+    """L % 128 == 0 and K <= 193: fir_umma_kernel (Toeplitz matrix resident in shared memory, signal staged by TMA,
+    four accumulator stages).  Single block, one tap, the largest K, ragged last tile, more channels than CTA pairs
+    (per-channel taps rebuild the matrix at every channel change); asymmetric random taps."""
+    import torch
+    rng = np.random.default_rng(190 + C + K)
+    x = ti.noise_real(rng, C * L).reshape(C, L)
+    if per_channel:
+        a = rng.standard_normal((C, K)).astype(np.float32)
+        y = tina.fir_multi(_cuda(x), _cuda(a)); ref = oracle.fir_multi(x, a)
+    else:
+        a = ti.random_taps(rng, K)
+        y = tina.fir(_cuda(x), _cuda(a)); ref = oracle.fir(x, a)
+    torch.cuda.synchronize()
+    assert tina.last_kernel().startswith("fir_umma_kernel")
+    assert y.shape == ref.shape
+    assert rel_l2_rows(y.cpu().numpy(), ref) <= TOL_FP32
+
+
+def test_fir_round1_toeplitz_route_still_correct(tina, oracle, tina_env):
+    import torch
+    tina_env(TINA_FIR_V1=1)
+    rng = np.random.default_rng(199)
+    x = ti.noise_real(rng, 3 * 128 * 40).reshape(3, 128 * 40)
+    a = ti.random_taps(rng, 64)
+    y = tina.fir(_cuda(x), _cuda(a)); torch.cuda.synchronize()
+    assert tina.last_kernel() == "pfb_umma_kernel"
+    assert rel_l2_rows(y.cpu().numpy(), oracle.fir(x, a)) <= TOL_FP32
+
+
 def test_unfold_matches_oracle_and_paper_example(tina, oracle):
     """Eq. (17); bit-exact (a gather).  Includes the paper's worked example."""
     import torch
