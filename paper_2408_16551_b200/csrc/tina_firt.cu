@@ -23,6 +23,7 @@
 #include "tina_umma.cuh"
 
 #include <cstring>
+#include <vector>
 
 namespace tina {
 
@@ -54,7 +55,19 @@ struct FirtParams {
     int taps_stride;           // 0: one tap vector; M: one per channel
     int tiles_per_chan, total_work;
     int a_slots, in_slots;     // ring depths
+    unsigned long long* prof;  // -DTINA_DEV only (TINA_PROF): [grid][16] cycle counters
+    int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 64 element-wise epilogue write-out, 128 no global stores, 256 no TMA loads
 };
+#ifdef TINA_DEV
+#define FT_DBG(b) (prm.debug & (b))
+#else
+#define FT_DBG(b) 0
+#endif
+#ifdef TINA_DEV
+#define FT_NOW() (prm.prof ? clock64() : 0LL)
+#else
+#define FT_NOW() 0LL
+#endif
 
 __device__ __forceinline__ float2 firt_lds_f2(uint32_t addr)
 {
@@ -140,17 +153,22 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
         // ============================ TMA producer: signal rows ================================
         if (lane == 0) {
             RingPos in;
+            long long pt_w = 0, pt_x, pt_tot = FT_NOW();
             for (int w = w_begin; w < w_end; ++w) {
                 const int chan = w / prm.tiles_per_chan;
                 const int row0 = (w % prm.tiles_per_chan) * (BM * CG) + (int)rank * BM;
                 for (int kc = 0; kc < n_kc; ++kc) {
-                    mbar_wait<64>(smem_u32(&ctl->in_empty[in.idx]), in.phase ^ 1);
+                    pt_x = FT_NOW(); mbar_wait<64>(smem_u32(&ctl->in_empty[in.idx]), in.phase ^ 1); pt_w += FT_NOW() - pt_x;
                     const uint32_t bar = smem_u32(&ctl->in_full[in.idx]);
-                    mbar_expect_tx(bar, FT_IN_SLOT);
-                    tma_load_3d(smem_u32(in_ring + in.idx * FT_IN_SLOT), &tmap_x, bar, FT_KC * (kc & 3), row0 + (kc >> 2), chan);
+                    if (FT_DBG(256)) mbar_arrive(bar);
+                    else {
+                        mbar_expect_tx(bar, FT_IN_SLOT);
+                        tma_load_3d(smem_u32(in_ring + in.idx * FT_IN_SLOT), &tmap_x, bar, FT_KC * (kc & 3), row0 + (kc >> 2), chan);
+                    }
                     in.advance(n_in);
                 }
             }
+            if (prm.prof) { unsigned long long* pp = prm.prof + blockIdx.x * 16; pp[0] = FT_NOW() - pt_tot; pp[1] = pt_w; }
         }
     } else if (warp == MMA_WARP) {
         // ============================ MMA issuer =============================================
@@ -174,6 +192,7 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
         } else {
             RingPos a, t;
             uint32_t br_phase = 0;
+            long long pm_a = 0, pm_t = 0, pm_x, pm_tot = FT_NOW();
             const uint32_t idesc = idesc_bf16(BM * CG, FT_T, false);
             const uint32_t b_s = smem_u32(b_res);
             for (int w = w_begin; w < w_end; ++w) {
@@ -186,11 +205,11 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                     br_phase ^= 1u;
                     tc_fence_after();
                 }
-                mbar_wait(smem_u32(&ctl->t_empty[t.idx]), t.phase ^ 1);      // the epilogue has drained this stage
+                pm_x = FT_NOW(); mbar_wait(smem_u32(&ctl->t_empty[t.idx]), t.phase ^ 1); pm_t += FT_NOW() - pm_x;      // the epilogue has drained this stage
                 tc_fence_after();
                 const uint32_t d = tmem_base + t.idx * (uint32_t)FT_T;
                 for (int kc = 0; kc < n_kc; ++kc) {
-                    mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase);
+                    pm_x = FT_NOW(); mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase); pm_a += FT_NOW() - pm_x;
                     tc_fence_after();
                     if (lane == 0) {
                         const uint64_t a_hi = smem_desc_sw64(smem_u32(a_ring + a.idx * FT_A_SLOT));
@@ -212,6 +231,7 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                 }
                 t.advance(FT_ACC);
             }
+            if (prm.prof && lane == 0) { unsigned long long* pp = prm.prof + blockIdx.x * 16; pp[2] = FT_NOW() - pm_tot; pp[3] = pm_a; pp[4] = pm_t; }
         }
     } else if (warp >= EPI_WARP0 && warp < EPI_WARP0 + 4) {
         // ============================ epilogue ==============================================
@@ -221,10 +241,11 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
         const int q = warp - EPI_WARP0;
         float* stg = reinterpret_cast<float*>(stage + q * FT_STAGE);
         RingPos t;
+        long long pe_w = 0, pe_s = 0, pe_x, pe_tot = FT_NOW();
         for (int w = w_begin; w < w_end; ++w) {
             const int chan = w / prm.tiles_per_chan;
             const long long row0 = (long long)(w % prm.tiles_per_chan) * (BM * CG) + rank * BM + q * 32;
-            mbar_wait<128>(smem_u32(&ctl->t_full[t.idx]), t.phase);
+            pe_x = FT_NOW(); mbar_wait<128>(smem_u32(&ctl->t_full[t.idx]), t.phase); pe_w += FT_NOW() - pe_x; pe_x = FT_NOW();
             tc_fence_after();
             const uint32_t taddr = tmem_base + t.idx * (uint32_t)FT_T + ((uint32_t)(q * 32) << 16);
             uint32_t r[32];
@@ -242,16 +263,19 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
             tc_fence_before();
             __syncwarp();
             if (lane == 0) arrive_leader<CG>(smem_u32(&ctl->t_empty[t.idx]), rank, leader);
+            pe_s += FT_NOW() - pe_x;
             const long long e0 = row0 * FT_T;                              // first element of the run in the channel
             long long n_run = prm.Lo - e0;
             if (n_run > 32LL * FT_T) n_run = 32LL * FT_T;
-            if (n_run > 0) {
+            if (n_run > 0 && !FT_DBG(128)) {
                 float* g = prm.y + (long long)chan * prm.Lo + e0;
                 const int run = (int)n_run;
                 const int head = min(run, (int)(((16u - ((uint32_t)(uintptr_t)g & 15u)) & 15u) >> 2));
                 const int nv4 = (run - head) >> 2;
                 auto at = [&](int l) { return stg[(l >> 7) * FT_PITCH + (l & 127)]; };
                 if (lane < head) g[lane] = at(lane);
+                // (an aligned-float4 variant -- two ld.shared.v4 of the staged row and a funnel shift by `head` instead of
+                // four scalar loads -- was measured slower: 0.177 against 0.137 ms; the scalar form stays)
                 for (int v = lane; v < nv4; v += 32) {
                     const int l = head + 4 * v;
                     *reinterpret_cast<float4*>(g + l) = make_float4(at(l), at(l + 1), at(l + 2), at(l + 3));
@@ -262,17 +286,30 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
             __syncwarp();
             t.advance(FT_ACC);
         }
+        if (prm.prof && q == 0 && lane == 0) { unsigned long long* pp = prm.prof + blockIdx.x * 16; pp[5] = FT_NOW() - pe_tot; pp[6] = pe_w; pp[7] = pe_s; }
     } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ producers: fp32 -> bf16 hi / lo =========================
         // warp pw converts rows 16 pw .. +15 of the staged 128 x 32 block; lanes 0-15 take an even row, lanes
         // 16-31 the next one, each lane two adjacent contraction elements (one 32-bit operand word per part).
+        // (Two groups of four warps on alternate chunks were tried: with an odd ring depth a slot is then shared by
+        // both groups and a group can test the parity of a barrier that is a whole phase behind -- a rare deadlock;
+        // with even depths the input ring shrinks to two slots and the kernel slows from 0.141 to 0.173 ms.)
         const int pw = warp - PROD_WARP0;
+        constexpr int RPW = FPW;                                           // rows per warp and chunk
         const uint32_t hl = (uint32_t)lane >> 4, wl = (uint32_t)lane & 15u;
-        const uint32_t in_lane = smem_u32(in_ring) + ((uint32_t)(pw * FPW) + hl) * 128u + wl * 8u;
-        const uint32_t a_lane = smem_u32(a_ring) + ((uint32_t)(pw * FPW) + hl) * 64u + (wl & 3u) * 4u;
+        const uint32_t in_lane = smem_u32(in_ring) + ((uint32_t)(pw * RPW) + hl) * 128u + wl * 8u;
+        const uint32_t a_lane = smem_u32(a_ring) + ((uint32_t)(pw * RPW) + hl) * 64u + (wl & 3u) * 4u;
         const uint32_t wc = wl >> 2;                                       // 16-byte chunk of the operand word
         RingPos in, a;
         uint32_t bf_phase = 0;
+        long long pp_i = 0, pp_a = 0, pp_x, pp_tot = FT_NOW();
+        float2 v[RPW / 2];
+        auto load_rows = [&]() {                                           // wait for the current input slot and read this warp's rows
+            pp_x = FT_NOW(); mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase); pp_i += FT_NOW() - pp_x;
+#pragma unroll
+            for (int i = 0; i < RPW / 2; ++i) v[i] = firt_lds_f2(in_lane + in.idx * FT_IN_SLOT + (uint32_t)i * 256u);
+        };
+        if (w_begin < w_end) load_rows();
         for (int w = w_begin; w < w_end; ++w) {
             if (new_channel(w)) {
                 mbar_wait(smem_u32(&ctl->b_free), bf_phase);
@@ -280,34 +317,40 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                 build_b(w / prm.tiles_per_chan, pw * 32 + lane, N_PROD_WARPS * 32);
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));
+                if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));          // all eight warps rebuild
             }
             for (int kc = 0; kc < n_kc; ++kc) {
-                mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase);
-                float2 v[FPW / 2];
+                // v holds this chunk's rows (loaded at the end of the previous iteration): convert, hand the input slot
+                // back, start the NEXT chunk's loads, then store / fence / publish -- the load latency and the wait for
+                // the next bulk copy overlap the store phase
+                uint32_t hb[RPW / 2], lb[RPW / 2];
 #pragma unroll
-                for (int i = 0; i < FPW / 2; ++i) v[i] = firt_lds_f2(in_lane + in.idx * FT_IN_SLOT + (uint32_t)i * 256u);
-                mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
-#pragma unroll
-                for (int i = 0; i < FPW / 2; ++i) {
+                for (int i = 0; i < RPW / 2; ++i) {
                     const __nv_bfloat162 hi = __floats2bfloat162_rn(v[i].x, v[i].y);
-                    const uint32_t hb = *reinterpret_cast<const uint32_t*>(&hi);
-                    const __nv_bfloat162 lo = __floats2bfloat162_rn(v[i].x - __uint_as_float(hb << 16),
-                                                                     v[i].y - __uint_as_float(hb & 0xffff0000u));
-                    // row r = 16 pw + 2 i + hl: swizzle phase (r >> 1) & 3 = i & 3
-                    const uint32_t addr = a_lane + a.idx * FT_A_SLOT + (uint32_t)i * 128u + ((wc ^ ((uint32_t)i & 3u)) << 4);
-                    sts32(addr, hb);
-                    sts32(addr + FT_A_TILE, *reinterpret_cast<const uint32_t*>(&lo));
+                    hb[i] = *reinterpret_cast<const uint32_t*>(&hi);
+                    const __nv_bfloat162 lo = __floats2bfloat162_rn(v[i].x - __uint_as_float(hb[i] << 16),
+                                                                     v[i].y - __uint_as_float(hb[i] & 0xffff0000u));
+                    lb[i] = *reinterpret_cast<const uint32_t*>(&lo);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
                 in.advance(n_in);
+                if (!(w == w_end - 1 && kc == n_kc - 1)) load_rows();
+                pp_x = FT_NOW(); mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1); pp_a += FT_NOW() - pp_x;
+#pragma unroll
+                for (int i = 0; i < RPW / 2; ++i) {
+                    // row r = 16 pw + 2 i + hl: swizzle phase (r >> 1) & 3 = i & 3
+                    const uint32_t addr = a_lane + a.idx * FT_A_SLOT + (uint32_t)i * 128u + ((wc ^ ((uint32_t)i & 3u)) << 4);
+                    sts32(addr, hb[i]);
+                    sts32(addr + FT_A_TILE, lb[i]);
+                }
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[a.idx]));
                 a.advance(n_a);
             }
         }
+        if (prm.prof && pw == 0 && lane == 0) { unsigned long long* pp = prm.prof + blockIdx.x * 16; pp[8] = FT_NOW() - pp_tot; pp[9] = pp_i; pp[10] = pp_a; }
     }
 
     tc_fence_before();
@@ -336,12 +379,19 @@ bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, i
     prm.tiles_per_chan = (int)tps;
     prm.total_work = (int)(tps * C);
     const size_t fixed = (size_t)n_kc * 2 * FT_B_TILE + 4 * FT_STAGE + sizeof(FirtCtl);
-    prm.a_slots = 4; prm.in_slots = 4;
+    // ring depths: the input ring is what keeps HBM busy (bytes in flight), the A ring only decouples the producers
+    // from the MMA warp
+    prm.a_slots = 3; prm.in_slots = 4;
     while (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) {
-        if (prm.in_slots > 2 && prm.in_slots >= prm.a_slots) --prm.in_slots;
-        else if (prm.a_slots > 2) --prm.a_slots;
+        if (prm.a_slots > 2) --prm.a_slots;
+        else if (prm.in_slots > 2) --prm.in_slots;
         else return false;
     }
+#ifdef TINA_DEV
+    if (options().a_slots) prm.a_slots = options().a_slots;
+    if (options().b_entries) prm.in_slots = options().b_entries;
+    prm.debug = options().debug_skip;
+#endif
     const size_t smem = fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT;
 
     EncodeTiledFn enc = encode_fn();
@@ -374,7 +424,28 @@ bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, i
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+#ifdef TINA_DEV
+    const bool prof = options().prof;
+    if (prof) {
+        cudaError_t pe = cudaMalloc(&prm.prof, (size_t)grid * 16 * 8);
+        if (pe == cudaSuccess) pe = cudaMemsetAsync(prm.prof, 0, (size_t)grid * 16 * 8, st);
+        if (pe != cudaSuccess) { if (prm.prof) cudaFree(prm.prof); *status = check_cuda(pe, "TINA_PROF counter buffer"); return true; }
+    }
+#endif
     cudaError_t e = cudaLaunchKernelEx(&cfg, fir_umma_kernel, tmap_x, prm);
+#ifdef TINA_DEV
+    if (prof) {
+        std::vector<unsigned long long> h((size_t)grid * 16);
+        cudaError_t pe = cudaStreamSynchronize(st);
+        if (pe == cudaSuccess) pe = cudaMemcpy(h.data(), prm.prof, h.size() * 8, cudaMemcpyDeviceToHost);
+        cudaFree(prm.prof);
+        if (pe != cudaSuccess) { *status = check_cuda(pe, "TINA_PROF counter read-back"); return true; }
+        double acc[16] = {0};
+        for (int b = 0; b < grid; b += UMMA_CG) for (int i = 0; i < 16; ++i) acc[i] += (double)h[(size_t)b * 16 + i] / (grid / UMMA_CG);
+        fprintf(stderr, "[tina prof fir] leader mean cycles: tma tot %.0f in_empty %.0f | mma tot %.0f a_full %.0f t_empty %.0f | epi tot %.0f t_full %.0f tmem->smem %.0f | prod tot %.0f in_full %.0f a_empty %.0f\n",
+                acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], acc[7], acc[8], acc[9], acc[10]);
+    }
+#endif
     count_launch();
     g_last_path = kPathUmma;
     note_kernel(per_channel ? "fir_umma_kernel<per-channel taps>" : "fir_umma_kernel");
