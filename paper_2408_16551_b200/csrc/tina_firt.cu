@@ -54,9 +54,10 @@ struct FirtParams {
     int M, n_kc;               // taps, chunks (Kp / 32)
     int taps_stride;           // 0: one tap vector; M: one per channel
     int tiles_per_chan, total_work;
-    int a_slots, in_slots;     // ring depths
+    int a_slots, in_slots;     // ring depths (even: see the producers)
+    int b_part_bytes;          // bytes of one part (hi or lo) of the resident band matrix, multiple of 1024
     unsigned long long* prof;  // -DTINA_DEV only (TINA_PROF): [grid][16] cycle counters
-    int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 64 element-wise epilogue write-out, 128 no global stores, 256 no TMA loads
+    int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 128 no global stores, 256 no TMA loads, 512 no MMAs, 1024 no operand stores, 2048 no TMEM read-out
 };
 #ifdef TINA_DEV
 #define FT_DBG(b) (prm.debug & (b))
@@ -87,8 +88,12 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
     if ((smem_u32(smem) & 1023u) != 0) __trap();
     constexpr int CG = UMMA_CG;
     const int n_kc = prm.n_kc;
-    uint8_t* b_res = smem;                                               // [n_kc][hi | lo] x 4 KB
-    uint8_t* a_ring = b_res + (size_t)n_kc * 2 * FT_B_TILE;               // multiples of 8 KB: 1024-aligned
+    // Every 32-row chunk of the Toeplitz matrix is a window of ONE band matrix G[n'][c'] = a[n' + M-1 - c'],
+    // c' in [0, 32): chunk kc needs the rows n' = n - 32 kc, so this CTA keeps the 64 + 32 (n_kc - 1) rows
+    // n' in [64 rank - 32 (n_kc - 1), 64 rank + 64) once (hi | lo) and chunk kc's B tile starts 32 (n_kc - 1 - kc) rows in.
+    uint8_t* b_res = smem;
+    const uint32_t b_part = (uint32_t)prm.b_part_bytes;                   // bytes of one part, multiple of 1024
+    uint8_t* a_ring = b_res + 2 * (size_t)b_part;
     uint8_t* in_ring = a_ring + (size_t)prm.a_slots * FT_A_SLOT;
     uint8_t* stage = in_ring + (size_t)prm.in_slots * FT_IN_SLOT;
     FirtCtl* ctl = reinterpret_cast<FirtCtl*>(stage + 4 * FT_STAGE);
@@ -107,10 +112,10 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
     if (warp == TMA_WARP && lane == 0) {
         prefetch_tmap(&tmap_x);
         for (int i = 0; i < 4; ++i) {
-            mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS + (rank == 0 ? CG - 1 : 0));
+            mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS / 2 + (rank == 0 ? CG - 1 : 0));   // one producer group per chunk
             mbar_init(smem_u32(&ctl->a_empty[i]), 1);
             mbar_init(smem_u32(&ctl->in_full[i]), 1);
-            mbar_init(smem_u32(&ctl->in_empty[i]), N_PROD_WARPS);
+            mbar_init(smem_u32(&ctl->in_empty[i]), N_PROD_WARPS / 2);
         }
         for (int i = 0; i < FT_ACC; ++i) { mbar_init(smem_u32(&ctl->t_full[i]), 1); mbar_init(smem_u32(&ctl->t_empty[i]), 4 * CG); }
         mbar_init(smem_u32(&ctl->b_free), 1);
@@ -121,23 +126,22 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
         tmem_alloc<CG>(smem_u32(&ctl->tmem_base), 512);
         tmem_relinquish<CG>();
     }
-    // Toeplitz matrix of channel `chan` (this CTA's 64 output columns n = 64 rank + nl), bf16 hi | lo, K-major,
-    // 64-byte-swizzled: element (nl, c) of chunk c / 32 at row nl, 16-byte chunk ((c % 32) >> 3) ^ ((nl >> 1) & 3)
+    // band matrix of channel `chan`, bf16 hi | lo, K-major, 64-byte-swizzled: element (j, c') at row j, 16-byte chunk
+    // (c' >> 3) ^ ((j >> 1) & 3)
     auto build_b = [&](int chan, int tid, int nthreads) {
         const float* taps = prm.taps + (long long)chan * prm.taps_stride;
-        const int Kp = n_kc * FT_KC, M = prm.M;
+        const int M = prm.M, rows = FT_T / CG + FT_KC * (n_kc - 1);
+        const int n0 = (int)rank * (FT_T / CG) - FT_KC * (n_kc - 1);      // n' of row 0
         const uint32_t b_s = smem_u32(b_res);
-        for (int idx = tid; idx < (FT_T / CG) * Kp; idx += nthreads) {
-            const int nl = idx / Kp, c = idx - nl * Kp;
-            const int k = (int)rank * (FT_T / CG) + nl + M - 1 - c;
+        for (int idx = tid; idx < rows * FT_KC; idx += nthreads) {
+            const int j = idx / FT_KC, cc = idx - j * FT_KC;
+            const int k = n0 + j + M - 1 - cc;
             const float v = (k >= 0 && k < M) ? __ldg(taps + k) : 0.f;
             const __nv_bfloat16 hi = __float2bfloat16(v);
             const __nv_bfloat16 lo = __float2bfloat16(v - __bfloat162float(hi));
-            const int cc = c & (FT_KC - 1);
-            const uint32_t off = (uint32_t)(c / FT_KC) * 2u * FT_B_TILE + (uint32_t)nl * 64u +
-                                 ((((uint32_t)cc >> 3) ^ (((uint32_t)nl >> 1) & 3u)) << 4) + ((uint32_t)cc & 7u) * 2u;
+            const uint32_t off = (uint32_t)j * 64u + ((((uint32_t)cc >> 3) ^ (((uint32_t)j >> 1) & 3u)) << 4) + ((uint32_t)cc & 7u) * 2u;
             firt_sts16(b_s + off, (uint32_t)__bfloat16_as_ushort(hi));
-            firt_sts16(b_s + off + FT_B_TILE, (uint32_t)__bfloat16_as_ushort(lo));
+            firt_sts16(b_s + off + b_part, (uint32_t)__bfloat16_as_ushort(lo));
         }
     };
     if (prm.taps_stride == 0 || w_begin < w_end) build_b(prm.taps_stride ? w_begin / prm.tiles_per_chan : 0, threadIdx.x, UMMA_THREADS);
@@ -214,15 +218,18 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                     if (lane == 0) {
                         const uint64_t a_hi = smem_desc_sw64(smem_u32(a_ring + a.idx * FT_A_SLOT));
                         const uint64_t a_lo = smem_desc_sw64(smem_u32(a_ring + a.idx * FT_A_SLOT + FT_A_TILE));
-                        const uint64_t b_hi = smem_desc_sw64(b_s + (uint32_t)kc * 2u * FT_B_TILE);
-                        const uint64_t b_lo = smem_desc_sw64(b_s + (uint32_t)kc * 2u * FT_B_TILE + FT_B_TILE);
+                        const uint32_t b_off = (uint32_t)(n_kc - 1 - kc) * (FT_KC * 64u);     // 32 rows of 64 B per chunk step
+                        const uint64_t b_hi = smem_desc_sw64(b_s + b_off);
+                        const uint64_t b_lo = smem_desc_sw64(b_s + b_off + b_part);
                         uint32_t acc = kc > 0;
+                        if (!FT_DBG(512)) {
 #pragma unroll
                         for (int k = 0; k < FT_KC / 16; ++k) { umma_bf16<CG>(d, a_lo + 2 * k, b_hi + 2 * k, idesc, acc); acc = 1; }
 #pragma unroll
                         for (int k = 0; k < FT_KC / 16; ++k) umma_bf16<CG>(d, a_hi + 2 * k, b_hi + 2 * k, idesc, 1);
 #pragma unroll
                         for (int k = 0; k < FT_KC / 16; ++k) umma_bf16<CG>(d, a_hi + 2 * k, b_lo + 2 * k, idesc, 1);
+                        }
                         commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
                         if (kc == n_kc - 1) commit_cg<CG>(smem_u32(&ctl->t_full[t.idx]), pair_mask);
                     }
@@ -249,6 +256,7 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
             tc_fence_after();
             const uint32_t taddr = tmem_base + t.idx * (uint32_t)FT_T + ((uint32_t)(q * 32) << 16);
             uint32_t r[32];
+            if (!FT_DBG(2048)) {
             tmem_ld32(taddr, r);
 #pragma unroll
             for (int cb = 0; cb < FT_T; cb += 32) {
@@ -259,6 +267,7 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                         make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
                                     __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
                 if (cb + 32 < FT_T) tmem_ld32(taddr + cb + 32, r);
+            }
             }
             tc_fence_before();
             __syncwarp();
@@ -289,27 +298,21 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
         if (prm.prof && q == 0 && lane == 0) { unsigned long long* pp = prm.prof + blockIdx.x * 16; pp[5] = FT_NOW() - pe_tot; pp[6] = pe_w; pp[7] = pe_s; }
     } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ producers: fp32 -> bf16 hi / lo =========================
-        // warp pw converts rows 16 pw .. +15 of the staged 128 x 32 block; lanes 0-15 take an even row, lanes
-        // 16-31 the next one, each lane two adjacent contraction elements (one 32-bit operand word per part).
-        // (Two groups of four warps on alternate chunks were tried: with an odd ring depth a slot is then shared by
-        // both groups and a group can test the parity of a barrier that is a whole phase behind -- a rare deadlock;
-        // with even depths the input ring shrinks to two slots and the kernel slows from 0.141 to 0.173 ms.)
+        // Two groups of four warps take alternate chunks (a chunk's fence / barrier round trip overlaps the other
+        // group's conversion; ring depths are even, so a slot always belongs to one group); within a group warp pwl
+        // converts rows 32 pwl .. +31 of the staged 128 x 32 block; lanes 0-15 take an even row, lanes 16-31 the next
+        // one, each lane two adjacent contraction elements (one 32-bit operand word per part).
         const int pw = warp - PROD_WARP0;
-        constexpr int RPW = FPW;                                           // rows per warp and chunk
+        const uint32_t grp = (uint32_t)pw >> 2, pwl = (uint32_t)pw & 3u;
+        constexpr int RPW = 2 * FPW;                                       // rows per warp and chunk
         const uint32_t hl = (uint32_t)lane >> 4, wl = (uint32_t)lane & 15u;
-        const uint32_t in_lane = smem_u32(in_ring) + ((uint32_t)(pw * RPW) + hl) * 128u + wl * 8u;
-        const uint32_t a_lane = smem_u32(a_ring) + ((uint32_t)(pw * RPW) + hl) * 64u + (wl & 3u) * 4u;
+        const uint32_t in_lane = smem_u32(in_ring) + (pwl * RPW + hl) * 128u + wl * 8u;
+        const uint32_t a_lane = smem_u32(a_ring) + (pwl * RPW + hl) * 64u + (wl & 3u) * 4u;
         const uint32_t wc = wl >> 2;                                       // 16-byte chunk of the operand word
         RingPos in, a;
         uint32_t bf_phase = 0;
         long long pp_i = 0, pp_a = 0, pp_x, pp_tot = FT_NOW();
-        float2 v[RPW / 2];
-        auto load_rows = [&]() {                                           // wait for the current input slot and read this warp's rows
-            pp_x = FT_NOW(); mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase); pp_i += FT_NOW() - pp_x;
-#pragma unroll
-            for (int i = 0; i < RPW / 2; ++i) v[i] = firt_lds_f2(in_lane + in.idx * FT_IN_SLOT + (uint32_t)i * 256u);
-        };
-        if (w_begin < w_end) load_rows();
+        uint32_t n_chunk = 0;
         for (int w = w_begin; w < w_end; ++w) {
             if (new_channel(w)) {
                 mbar_wait(smem_u32(&ctl->b_free), bf_phase);
@@ -319,10 +322,12 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));          // all eight warps rebuild
             }
-            for (int kc = 0; kc < n_kc; ++kc) {
-                // v holds this chunk's rows (loaded at the end of the previous iteration): convert, hand the input slot
-                // back, start the NEXT chunk's loads, then store / fence / publish -- the load latency and the wait for
-                // the next bulk copy overlap the store phase
+            for (int kc = 0; kc < n_kc; ++kc, ++n_chunk) {
+                if ((n_chunk & 1u) != grp) { in.advance(n_in); a.advance(n_a); continue; }
+                pp_x = FT_NOW(); mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase); pp_i += FT_NOW() - pp_x;
+                float2 v[RPW / 2];
+#pragma unroll
+                for (int i = 0; i < RPW / 2; ++i) v[i] = firt_lds_f2(in_lane + in.idx * FT_IN_SLOT + (uint32_t)i * 256u);
                 uint32_t hb[RPW / 2], lb[RPW / 2];
 #pragma unroll
                 for (int i = 0; i < RPW / 2; ++i) {
@@ -335,11 +340,11 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
                 in.advance(n_in);
-                if (!(w == w_end - 1 && kc == n_kc - 1)) load_rows();
                 pp_x = FT_NOW(); mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1); pp_a += FT_NOW() - pp_x;
+                if (!FT_DBG(1024))
 #pragma unroll
                 for (int i = 0; i < RPW / 2; ++i) {
-                    // row r = 16 pw + 2 i + hl: swizzle phase (r >> 1) & 3 = i & 3
+                    // row r = 32 pwl + 2 i + hl: swizzle phase (r >> 1) & 3 = i & 3
                     const uint32_t addr = a_lane + a.idx * FT_A_SLOT + (uint32_t)i * 128u + ((wc ^ ((uint32_t)i & 3u)) << 4);
                     sts32(addr, hb[i]);
                     sts32(addr + FT_A_TILE, lb[i]);
@@ -378,15 +383,14 @@ bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, i
     prm.taps_stride = per_channel ? M : 0;
     prm.tiles_per_chan = (int)tps;
     prm.total_work = (int)(tps * C);
-    const size_t fixed = (size_t)n_kc * 2 * FT_B_TILE + 4 * FT_STAGE + sizeof(FirtCtl);
-    // ring depths: the input ring is what keeps HBM busy (bytes in flight), the A ring only decouples the producers
-    // from the MMA warp
-    prm.a_slots = 3; prm.in_slots = 4;
-    while (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) {
-        if (prm.a_slots > 2) --prm.a_slots;
-        else if (prm.in_slots > 2) --prm.in_slots;
-        else return false;
-    }
+    prm.b_part_bytes = ((FT_T / UMMA_CG + FT_KC * (n_kc - 1)) * 64 + 1023) / 1024 * 1024;
+    const size_t fixed = 2 * (size_t)prm.b_part_bytes + 4 * FT_STAGE + sizeof(FirtCtl);
+    // Ring depths are EVEN: the two producer groups take alternate chunks, and a slot shared by both groups would let a
+    // group test the parity of a barrier that is a whole phase behind (measured: a rare deadlock with a 3-slot ring).
+    prm.a_slots = 4; prm.in_slots = 4;
+    if (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) prm.a_slots = 2;
+    if (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) prm.in_slots = 2;
+    if (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) return false;
 #ifdef TINA_DEV
     if (options().a_slots) prm.a_slots = options().a_slots;
     if (options().b_entries) prm.in_slots = options().b_entries;
