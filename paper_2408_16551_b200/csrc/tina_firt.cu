@@ -35,7 +35,7 @@ constexpr int FT_A_TILE = BM * FT_KC * 2;         // 8 KB
 constexpr int FT_A_SLOT = 2 * FT_A_TILE;          // hi | lo
 constexpr int FT_B_TILE = (FT_T / UMMA_CG) * FT_KC * 2;   // 4 KB: this CTA's 64 rows of one chunk and part
 constexpr int FT_IN_SLOT = BM * FT_KC * 4;        // 16 KB fp32
-constexpr int FT_PITCH = 132;                     // staged row pitch (floats) of the epilogue
+constexpr int FT_PITCH = 129;                     // staged row pitch (floats) of the epilogue: odd, see below
 constexpr int FT_STAGE = 32 * FT_PITCH * 4;       // per epilogue warp
 constexpr int FT_ACC = 4;                         // TMEM accumulator stages of 128 columns
 
@@ -261,11 +261,13 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
 #pragma unroll
             for (int cb = 0; cb < FT_T; cb += 32) {
                 tmem_ld_wait();
+                // staged layout: element e of a row at word (e >> 2) + 32 (e & 3) of the row (pitch 129 words): the
+                // writes (lane = row, odd pitch) and the read-out below (lanes 4 elements apart) are both conflict-free
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
-                    *reinterpret_cast<float4*>(stg + lane * FT_PITCH + cb + 4 * j) =
-                        make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]),
-                                    __uint_as_float(r[4 * j + 2]), __uint_as_float(r[4 * j + 3]));
+#pragma unroll
+                    for (int k = 0; k < 4; ++k)
+                        stg[lane * FT_PITCH + (cb >> 2) + j + 32 * k] = __uint_as_float(r[4 * j + k]);
                 if (cb + 32 < FT_T) tmem_ld32(taddr + cb + 32, r);
             }
             }
@@ -281,7 +283,7 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                 const int run = (int)n_run;
                 const int head = min(run, (int)(((16u - ((uint32_t)(uintptr_t)g & 15u)) & 15u) >> 2));
                 const int nv4 = (run - head) >> 2;
-                auto at = [&](int l) { return stg[(l >> 7) * FT_PITCH + (l & 127)]; };
+                auto at = [&](int l) { return stg[(l >> 7) * FT_PITCH + ((l & 127) >> 2) + 32 * (l & 3)]; };
                 if (lane < head) g[lane] = at(lane);
                 // (an aligned-float4 variant -- two ld.shared.v4 of the staged row and a funnel shift by `head` instead of
                 // four scalar loads -- was measured slower: 0.177 against 0.137 ms; the scalar form stays)
