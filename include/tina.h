@@ -63,8 +63,9 @@ typedef enum {
  *   y    [C][L-M+1]   float32, row-major (device), must not overlap x
  * Supported: C >= 1, 1 <= M <= 4096, L >= M.  Even L with M <= 193 runs as a banded-Toeplitz
  * contraction on the tensor cores (blocks of 128 outputs, bf16x3 error-compensated, rel. L2 per
- * channel <= 1e-5, the unfolding view of Eq. (17)-(19)); any other shape on the
- * CUDA-core register-window kernel (fp32 FMA).  Errors: NULL_POINTER, BAD_SHAPE, UNSUPPORTED
+ * channel <= 1e-5, the unfolding view of Eq. (17)-(19)) -- with L % 128 == 0 on
+ * the kernel that keeps the Toeplitz band matrix resident in shared memory and stages the signal by
+ * TMA; any other shape on the CUDA-core register-window kernel (fp32 FMA).  Errors: NULL_POINTER, BAD_SHAPE, UNSUPPORTED
  * (M > 4096), ALIGNMENT (x, y not 16-byte aligned), CUDA.                                          */
 tina_status tina_fir(const float* x, const float* taps, float* y,
                      int C, long long L, int M, void* stream);
@@ -75,7 +76,9 @@ tina_status tina_fir(const float* x, const float* taps, float* y,
  *     y[c][j] = sum_{k=0}^{M-1} taps[c][k] * x[c][j + M-1 - k],   j in [0, L-M+1)
  *   x    [C][L]       float32 (device)      taps [C][M] float32, row c = channel c's taps (device)
  *   y    [C][L-M+1]   float32 (device), must not overlap x
- * Supported: C >= 1, 1 <= M <= 4096, L >= M; runs on the CUDA-core register-window kernel (fp32 FMA).
+ * Supported: C >= 1, 1 <= M <= 4096, L >= M.  L % 128 == 0 with M <= 193 runs on the tensor-core
+ * Toeplitz kernel (the band matrix is rebuilt in shared memory whenever the channel changes; same
+ * 1e-5 contract), any other shape on the CUDA-core register-window kernel (fp32 FMA).
  * Errors as tina_fir.                                                                              */
 tina_status tina_fir_multi(const float* x, const float* taps, float* y,
                            int C, long long L, int M, void* stream);
