@@ -406,6 +406,17 @@ def run_ours(args, w):
         h_total, h_per, _, _ = timed(args.steps, lambda i: steps_of[0])
         hot = {"ms_per_step": h_total / args.steps, "ms_mean": float(np.mean(h_per)), "ms_min": float(np.min(h_per)),
                "value": world * samples / (h_total / args.steps * 1e-3) / 1e9}
+    # launch-latency-bound workloads (c1: a 1 MB problem): microseconds per call of a back-to-back burst of calls on the
+    # same buffers, host clock around the burst including the final synchronise (no per-step events in between)
+    call_us = None
+    if set_bytes < 16e6:
+        n_b2b = 2000
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_b2b):
+            steps_of[0]()
+        torch.cuda.synchronize()
+        call_us = (time.perf_counter() - t0) / n_b2b * 1e6
     issued_ratio = tina.last_issued_ratio() if hasattr(tina, "last_issued_ratio") else None
     variant = tina.last_kernel() if hasattr(tina, "last_kernel") else None
 
@@ -490,6 +501,8 @@ def run_ours(args, w):
         line["profile_run"] = True
     if hot is not None:
         line["hot"] = hot
+    if call_us is not None:
+        line["hot"]["back_to_back_us_per_call"] = call_us
     if cpu_val is not None:
         line["cpu_baseline"] = {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                 "note": "float64 direct sums (the parity oracle): not a performance baseline"}

@@ -117,6 +117,22 @@ tina_status ensure_smem(DevCtx* ctx, const void* func, int bytes, const char* wh
     return TINA_OK;
 }
 
+bool tmap_cache_get(DevCtx* ctx, const TmapKey& key, TmapSet* out)
+{
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    for (const auto& e : ctx->tmaps)
+        if (e.first == key) { *out = e.second; return true; }
+    return false;
+}
+
+void tmap_cache_put(DevCtx* ctx, const TmapKey& key, const TmapSet& set)
+{
+    constexpr size_t kMax = 16;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    if (ctx->tmaps.size() < kMax) ctx->tmaps.emplace_back(key, set);
+    else ctx->tmaps[ctx->tmap_next++ % kMax] = std::make_pair(key, set);
+}
+
 void dev_ctx_release_all()
 {
     std::lock_guard<std::mutex> lk(g_ctx_mu);
@@ -129,6 +145,7 @@ void dev_ctx_release_all()
         cudaSetDevice(c->dev);
         for (int i = 0; i < 3; ++i) { if (c->stage_p[i]) cudaFree(c->stage_p[i]); c->stage_p[i] = nullptr; c->stage_n[i] = 0; }
         if (c->tz_ring) { cudaFree(c->tz_ring); c->tz_ring = nullptr; }
+        c->tmaps.clear();
     }
     cudaSetDevice(cur);
 }

@@ -5,8 +5,10 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <cstring>
 #include <map>
 #include <mutex>
+#include <vector>
 
 #include "../../include/tina.h"
 
@@ -48,6 +50,16 @@ struct Options {
 const Options& options();
 void reload_options();
 
+// ---- cache of encoded TMA tensor maps (per device): a map is a pure function of base pointer, shape and box, so
+// a call that repeats the pointers and sizes of an earlier one skips its cuTensorMapEncodeTiled calls
+struct TmapKey {
+    const void* p[3];          // base pointers (input, window / taps, output)
+    long long n[2];            // n_samples / L, ...
+    int i[6];                  // S / C, P, M, kind, tap-count template, caller tag
+    bool operator==(const TmapKey& o) const { return memcmp(this, &o, sizeof(TmapKey)) == 0; }
+};
+struct TmapSet { alignas(64) unsigned char m[4][128]; };   // up to four CUtensorMap (128 bytes each)
+
 // ---- per-device state: SM count, kernels whose >48 KB dynamic shared memory opt-in has been set ---
 struct DevCtx {
     int dev = -1;
@@ -63,7 +75,11 @@ struct DevCtx {
     cudaStream_t s_in = nullptr, s_cmp = nullptr, s_out = nullptr;
     cudaEvent_t ev_start = nullptr, ev_in[64] = {}, ev_cmp[64] = {};
     std::mutex host_mu;                     // serialises tina_pfb_batched_host on this device
+    std::vector<std::pair<TmapKey, TmapSet>> tmaps;   // small round-robin cache (guarded by mu)
+    unsigned tmap_next = 0;
 };
+bool tmap_cache_get(DevCtx* ctx, const TmapKey& key, TmapSet* out);
+void tmap_cache_put(DevCtx* ctx, const TmapKey& key, const TmapSet& set);
 // context of the CURRENT device (cudaGetDevice), created on first use; the registry is mutex-guarded
 tina_status dev_ctx(DevCtx** out);
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (device, kernel)
