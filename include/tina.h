@@ -171,6 +171,21 @@ tina_status tina_add(const float* a, const float* b, float* out, long long n, vo
 tina_status tina_sum(const float* x, long long rows, long long n, float* out, void* stream);
 tina_status tina_matmul(const float* x, const float* y, float* z, long long M, long long L, long long N, void* stream);
 
+/* tina_sum for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): Eq. (11) exactly as tina_sum computes it -- same blocks per
+ * row, same float32 chains, same double-precision combination, so the results are bit-identical -- but the
+ * per-block partial sums go to a file-scope `static __device__` array of 2 * TINA_SUM_STATIC_MAX_ROWS doubles
+ * (64 KB) instead of a cudaMallocAsync temporary.  Every GPU that loads the library holds that array until the
+ * process exits.  The call makes no cudaMalloc / cudaFree / allocating library call (its first use on a device
+ * looks the array's address up with cudaGetSymbolAddress).  x, out: device pointers as in tina_sum.
+ * Limit: rows <= TINA_SUM_STATIC_MAX_ROWS, else UNSUPPORTED (tina_last_error names the limit); n is unlimited.
+ * ALL calls on a device share the one array: calls that overlap on the GPU (different streams, or graphs replayed
+ * concurrently) race on it and give wrong sums -- order them on one stream or with events.  The array keeps the
+ * previous call's partials; nothing needs clearing, because every entry a call reads it has written first.
+ * Errors: BAD_SHAPE (negative size), UNSUPPORTED (rows over the limit), NULL_POINTER, CUDA.                   */
+#define TINA_SUM_STATIC_MAX_ROWS 4096
+tina_status tina_sum_static(const float* x, long long rows, long long n, float* out, void* stream);
+
 /* F = floor(n_samples / P) - M + 1; <= 0 means the input is too short.                     */
 long long   tina_pfb_num_frames(long long n_samples, int P, int M);
 

@@ -19,7 +19,7 @@ _lib = None
 EXPORTS = ["tina_fir", "tina_fir_multi", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
            "tina_pfb_batched_host", "tina_pfb_num_frames", "tina_status_string", "tina_last_error",
            "tina_clear_plan_cache", "tina_version", "tina_launch_count", "tina_last_path", "tina_reload_options", "tina_build_is_dev", "tina_probe_peak", "tina_last_kernel", "tina_last_issued_ratio",
-           "tina_mul", "tina_add", "tina_sum", "tina_matmul"]
+           "tina_mul", "tina_add", "tina_sum", "tina_sum_static", "tina_matmul"]
 
 
 class TinaError(RuntimeError):
@@ -50,8 +50,9 @@ def lib() -> ctypes.CDLL:
     L.tina_mul.argtypes = [vp, vp, vp, ll, vp]
     L.tina_add.argtypes = [vp, vp, vp, ll, vp]
     L.tina_sum.argtypes = [vp, ll, ll, vp, vp]
+    L.tina_sum_static.argtypes = [vp, ll, ll, vp, vp]
     L.tina_matmul.argtypes = [vp, vp, vp, ll, ll, ll, vp]
-    for f in ("tina_mul", "tina_add", "tina_sum", "tina_matmul"):
+    for f in ("tina_mul", "tina_add", "tina_sum", "tina_sum_static", "tina_matmul"):
         getattr(L, f).restype = ci
     for f in ("tina_fir", "tina_unfold", "tina_dft", "tina_pfb", "tina_pfb_batched", "tina_pfb_fir_batched", "tina_pfb_fft_batched",
               "tina_pfb_batched_host", "tina_clear_plan_cache", "tina_version", "tina_last_path", "tina_reload_options",
@@ -235,6 +236,23 @@ def summation(x, out=None, stream=None):
     out = _out(out, (rows,), torch.float32, x.device)
     _check(lib().tina_sum(x.data_ptr(), rows, n, out.data_ptr(), _stream_ptr(stream)))
     return out[0] if one_d else out
+
+
+def summation_static(x, out, stream=None):
+    """tina_sum_static: tina_sum with its partial sums in a static device array (no device allocation inside the
+    call, so `out` [rows] (or 0-d for 1-D x) must be supplied); rows <= 4096; calls that overlap on the GPU race."""
+    import torch
+    x = _dev(x, torch.float32, "x")
+    if x.dim() == 1:
+        x = x[None, :]
+    if x.dim() != 2:
+        raise ValueError("x must be 1-D or 2-D")
+    rows, n = x.shape
+    if out is None or out.numel() != rows:
+        raise ValueError("summation_static needs a preallocated out of rows elements")
+    out = _dev(out, torch.float32, "out")
+    _check(lib().tina_sum_static(x.data_ptr(), rows, n, out.data_ptr(), _stream_ptr(stream)))
+    return out
 
 
 def matmul(x, y, out=None, stream=None):

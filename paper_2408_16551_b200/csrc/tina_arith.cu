@@ -196,3 +196,65 @@ tina_status arith_matmul(const float* x, const float* y, float* z, long long M, 
 }
 
 }  // namespace tina
+
+// ---- tina_sum_static: Eq. (11) with the per-block partial sums in a file-scope device array instead of a
+// cudaMallocAsync temporary, for callers that may not allocate (CUDA graph capture, tight serving loops).
+// The array is part of this module's image on every GPU that loads libtina.so and is held until the process exits.
+// In host code `g_sum_static_scratch` is a host-side stand-in, not a device address, so it is never passed to a
+// kernel: the device address is looked up once per device with cudaGetSymbolAddress, with that device current.
+namespace {
+
+constexpr long long kSumStaticRows = TINA_SUM_STATIC_MAX_ROWS;            // documented limit (include/tina.h)
+constexpr long long kSumStaticScratch = 2 * TINA_SUM_STATIC_MAX_ROWS;     // doubles: 8192 x 8 bytes = 64 KB
+static __device__ __align__(256) double g_sum_static_scratch[kSumStaticScratch];
+
+constexpr int kSumStaticMaxDev = 64;
+std::mutex g_sum_static_mu;
+double* g_sum_static_ptr[kSumStaticMaxDev] = {};                          // per device, filled on first use
+
+tina_status sum_static_scratch(double** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return tina::check_cuda(e, "cudaGetDevice");
+    if (dev < 0 || dev >= kSumStaticMaxDev) return tina::fail(TINA_ERR_UNSUPPORTED, "tina_sum_static: device ordinal %d >= %d", dev, kSumStaticMaxDev);
+    std::lock_guard<std::mutex> lk(g_sum_static_mu);
+    if (!g_sum_static_ptr[dev]) {
+        double* p = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_sum_static_scratch);
+        if (e != cudaSuccess || !p) return tina::check_cuda(e != cudaSuccess ? e : cudaErrorInvalidSymbol, "cudaGetSymbolAddress(sum scratch)");
+        g_sum_static_ptr[dev] = p;
+    }
+    *out = g_sum_static_ptr[dev];
+    return TINA_OK;
+}
+
+}  // namespace
+
+extern "C" tina_status tina_sum_static(const float* x, long long rows, long long n, float* out, void* stream)
+{
+    using namespace tina;
+    if (rows < 0 || n < 0) return fail(TINA_ERR_BAD_SHAPE, "tina_sum_static: negative size");
+    if (rows > kSumStaticRows)
+        return fail(TINA_ERR_UNSUPPORTED, "tina_sum_static: rows = %lld exceeds the static scratch limit of %lld rows (use tina_sum)",
+                    rows, kSumStaticRows);
+    if (rows > 0 && (!out || (n > 0 && !x))) return fail(TINA_ERR_NULL_POINTER, "tina_sum_static: null pointer");
+    if (rows == 0) return TINA_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the decomposition of arith_sum (same blocks per row and chunk, hence the same rounding order), except that a
+    // single block per row also goes through the scratch: one code path, every partial written before it is read
+    long long gx = ((long long)sm_count() * 8 + rows - 1) / rows;
+    const long long need = (n + 4095) / 4096;
+    if (gx > need) gx = need;
+    if (gx < 1) gx = 1;
+    if (rows * gx > kSumStaticScratch) gx = kSumStaticScratch / rows;     // >= 2 since rows <= kSumStaticScratch / 2
+    const long long chunk = ((n + gx - 1) / gx + 255) / 256 * 256;
+    double* partial = nullptr;
+    tina_status s = sum_static_scratch(&partial);
+    if (s != TINA_OK) return s;
+    g_last_path = kPathSimt; note_kernel("sum_kernel<static scratch>");
+    sum_kernel<<<dim3((unsigned)gx, (unsigned)rows), 256, 0, st>>>(x, n, chunk > 0 ? chunk : 256, partial, nullptr);
+    sum_final_kernel<<<(unsigned)((rows + 7) / 8), 256, 0, st>>>(partial, (int)gx, out, rows);
+    count_launch(2);
+    return check_cuda(cudaGetLastError(), "sum_kernel launch (static scratch)");
+}
