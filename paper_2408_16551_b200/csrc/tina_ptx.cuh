@@ -298,6 +298,20 @@ __device__ __forceinline__ uint64_t smem_desc_sw64(uint32_t saddr)
     d |= (uint64_t)4 << 61;                           // SWIZZLE_64B
     return d;
 }
+// MN-major operand (consecutive bf16 elements run along M / N, not along K) in the canonical 128-byte-swizzled
+// layout: rows of 128 B = 64 consecutive M elements for one k, atoms of 8 k-rows (1024 B, 16-byte units XOR-ed with
+// the row index); `lbo` = byte distance between blocks of 64 M elements, `sbo` = between groups of 8 k.
+__device__ __forceinline__ uint64_t smem_desc_mn_sw128(uint32_t saddr, uint32_t lbo, uint32_t sbo)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+    d |= (uint64_t)(lbo >> 4) << 16;
+    d |= (uint64_t)(sbo >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;                           // SWIZZLE_128B
+    return d;
+}
+constexpr uint32_t IDESC_A_MN_MAJOR = 1u << 15;      // instruction descriptor: A operand is MN-major
 // Instruction descriptor for kind::f16 with bf16 A/B (both K-major), fp32 D.
 // (a_format / b_format: 1 = bf16, 0 = fp16)
 __host__ __device__ constexpr uint32_t idesc_bf16(int M, int N, bool fp16 = false)

@@ -632,14 +632,22 @@ __device__ __forceinline__ void sym_epilogue_real(const SymParams& prm, const Ep
 // CTA instead of once per warp).  REAL = true: the real kind, contracted as even / odd samples against the
 // cos / sin columns of the bins [0, P/4) -- see sym_epilogue_real; the producers are the same (an adjacent pair of
 // real samples takes the place of (re, im)), each MMA warp has its own twiddle entries (even-sample and
-// odd-sample matrices), and K = P/2.  To make room the operand tiles are 32 contraction elements wide (64-byte
-// rows, SWIZZLE_64B): A slot = 4 x 8 KB, B entry = 8 KB per CTA, two K = 16 MMAs per tile and product.
+// odd-sample matrices), and K = P/2.  To make room the operand tiles are 32 contraction elements wide: A slot =
+// 4 x 8 KB, B entry = 8 KB per CTA (64-byte rows, SWIZZLE_64B), two K = 16 MMAs per tile and product.
+// The A tiles are MN-MAJOR (frames contiguous, SWIZZLE_128B: [2 blocks of 64 frames][4 groups of 8 columns][8 columns]
+// [128 B = 8 units of 8 frames]): a producer lane owns one column, so 8 consecutive frames of one part are ONE 16-byte
+// store (conflict-free per quarter warp) instead of eight 2-byte stores -- the K-major layout cost 64 st.shared.b16
+// per warp and chunk at two wavefronts each (two lanes share a 32-bit word), 1024 of the ~3000 shared-memory
+// wavefronts per chunk that bound the kernel (ncu: 37.9 M store bank conflicts per c4 launch).
 //   shared memory: A ring 64 KB (2 slots; 4 for the single pass) | B ring 48 KB (6 entries = 3 chunks) |
 //                  input ring 2 x 40 KB | epilogue staging 32 KB
 //   warps: 0-7 FIR producers, 8-11 epilogue, 12 TMA (twiddles), 13 / 15 MMA issuers, 14 TMEM allocation + TMA (input)
 // =====================================================================================
 constexpr int ST_KC = 32;                                  // contraction elements (complex columns) per chunk
-constexpr int ST_TILE = BM * ST_KC * 2;                    // 8 KB: 128 rows x 64 B
+constexpr int ST_TILE = BM * ST_KC * 2;                    // 8 KB: 128 frames x 32 columns of bf16
+constexpr uint32_t ST_A_LBO = 4096;                        // MN-major A tile: bytes between the two blocks of 64 frames
+constexpr uint32_t ST_A_SBO = 1024;                        //                  bytes between groups of 8 columns
+constexpr uint32_t ST_A_KSTEP = (2 * ST_A_SBO) >> 4;       // descriptor advance per K = 16 MMA (two column groups)
 constexpr int ST_A_RING = 64 * 1024;
 constexpr int ST_B_ENTRY = (NSUB / UMMA_CG) * ST_KC * 2;   // 8 KB per CTA
 constexpr int ST_B_ENTRIES = 6;
@@ -772,7 +780,7 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
             for (int w = cl; w < prm.total_work; w += n_cl) {
                 const int k0 = (w % npg) * SY_BINS;
                 const int nw = 2 * min(SY_BINS, half - k0);
-                const uint32_t idesc = idesc_bf16(BM * CG, nw, prm.fp16 != 0);
+                const uint32_t idesc = idesc_bf16(BM * CG, nw, prm.fp16 != 0) | IDESC_A_MN_MAJOR;
                 for (int ks = 0; ks < prm.k_splits; ++ks) {
                     const int kc_begin = ks * prm.kc_per_split, kc_end = min(n_kc, kc_begin + prm.kc_per_split);
                     for (int kc = kc_begin; kc < kc_end; ++kc) {
@@ -795,13 +803,13 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + bi * ST_B_ENTRY));
                             uint32_t acc = kc > kc_begin;
                             if (parts > 1) {
-                                const uint64_t ad = smem_desc_sw64(a_lo);
+                                const uint64_t ad = smem_desc_mn_sw128(a_lo, ST_A_LBO, ST_A_SBO);
 #pragma unroll
-                                for (int k = 0; k < ST_KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                                for (int k = 0; k < ST_KC / 16; ++k) { umma_bf16<CG>(d, ad + ST_A_KSTEP * k, bd + 2 * k, idesc, acc); acc = 1; }
                             }
-                            const uint64_t ad = smem_desc_sw64(a_hi);
+                            const uint64_t ad = smem_desc_mn_sw128(a_hi, ST_A_LBO, ST_A_SBO);
 #pragma unroll
-                            for (int k = 0; k < ST_KC / 16; ++k) { umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, acc); acc = 1; }
+                            for (int k = 0; k < ST_KC / 16; ++k) { umma_bf16<CG>(d, ad + ST_A_KSTEP * k, bd + 2 * k, idesc, acc); acc = 1; }
                             commit_cg<CG>(smem_u32(&ctl->b_empty[bi]), pair_mask);
                         }
                         __syncwarp();
@@ -811,9 +819,9 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             tc_fence_after();
                             if (lane == 0) {
                                 const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + bi * ST_B_ENTRY));
-                                const uint64_t ad = smem_desc_sw64(a_hi);
+                                const uint64_t ad = smem_desc_mn_sw128(a_hi, ST_A_LBO, ST_A_SBO);
 #pragma unroll
-                                for (int k = 0; k < ST_KC / 16; ++k) umma_bf16<CG>(d, ad + 2 * k, bd + 2 * k, idesc, 1);
+                                for (int k = 0; k < ST_KC / 16; ++k) umma_bf16<CG>(d, ad + ST_A_KSTEP * k, bd + 2 * k, idesc, 1);
                                 commit_cg<CG>(smem_u32(&ctl->b_empty[bi]), pair_mask);
                             }
                             __syncwarp();
@@ -845,13 +853,15 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         // Warp pw owns frames 16 pw .. 16 pw + 15 of the CTA's tile, lane = complex column of the chunk.  Per
         // chunk: wait for the staged rows, read the 16 + MT - 1 rows of the sliding window and the MT taps from
         // shared memory, polyphase MAC in registers (Eq. (20)), split into bf16 hi / lo, de-interleave into the
-        // 64-byte-swizzled yr / yi tiles: row r, 16-byte chunk (lane >> 3) stored at chunk ^ ((r >> 1) & 3).
+        // MN-major yr / yi tiles: column c = lane sits in column group c >> 3, row c & 7 of the atom; the warp's frames
+        // 16 pw .. 16 pw + 15 are the 16-byte units 2 (pw & 3), + 1 of the 64-frame block pw >> 2, stored at unit ^ (c & 7).
         const int pw = warp - PROD_WARP0;
         const uint32_t a_ring_s = smem_u32(a_ring), in_ring_s = smem_u32(in_ring);
-        uint32_t cell0[4];
+        uint32_t cell0[FPW / 8];
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-            cell0[j] = a_ring_s + (uint32_t)(pw * FPW) * 64u + ((((uint32_t)lane >> 3) ^ (uint32_t)j) << 4) + ((uint32_t)lane & 7u) * 2u;
+        for (int j = 0; j < FPW / 8; ++j)
+            cell0[j] = a_ring_s + (uint32_t)(pw >> 2) * ST_A_LBO + ((uint32_t)lane >> 3) * ST_A_SBO + ((uint32_t)lane & 7u) * 128u +
+                       (((2u * ((uint32_t)pw & 3u) + (uint32_t)j) ^ ((uint32_t)lane & 7u)) << 4);
         constexpr uint32_t im_off = (uint32_t)parts * ST_TILE;
         const uint32_t in_lane = in_ring_s + (uint32_t)(pw * FPW) * 256u + (uint32_t)lane * 8u;
         const uint32_t tap_lane = in_ring_s + ST_IN_TAPS + (uint32_t)lane * (REAL ? 8u : 4u);
@@ -878,66 +888,47 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
                 mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
                 pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
-                // polyphase MAC + split + de-interleaved store (as fir_compute_store_sym, 64-byte rows).  The 32 stores of
-                // the first eight frames are interleaved with the packed FMAs of the last eight, so that the
-                // shared-memory store queue drains under arithmetic instead of stalling the warp.
+                // polyphase MAC + split + de-interleaved store, eight frames at a time: eight independent FMA chains, then
+                // the (hi, lo) x (re, im) parts of the eight frames as four 16-byte stores.
                 const uint32_t so = a.idx * a_slot_bytes;
-                auto convert = [&](const float2 (&yv)[8], uint32_t (&hb)[8], uint32_t (&lb)[8]) {
-#pragma unroll
-                    for (int g = 0; g < 8; ++g) {
-                        if (parts == 1 && prm.fp16) { const __half2 hh = __floats2half2_rn(yv[g].x, yv[g].y); hb[g] = *reinterpret_cast<const uint32_t*>(&hh); }
-                        else { const __nv_bfloat162 hi = __floats2bfloat162_rn(yv[g].x, yv[g].y); hb[g] = *reinterpret_cast<const uint32_t*>(&hi); }
-                        if (parts > 1) {
-                            const float lx = yv[g].x - __uint_as_float(hb[g] << 16);
-                            const float ly = yv[g].y - __uint_as_float(hb[g] & 0xffff0000u);
-                            const __nv_bfloat162 lo = __floats2bfloat162_rn(lx, ly);
-                            lb[g] = *reinterpret_cast<const uint32_t*>(&lo);
-                        } else lb[g] = 0u;
-                    }
+                auto pack2 = [&](float a0, float a1) -> uint32_t {        // (a0 -> low half, a1 -> high half)
+                    if (parts == 1 && prm.fp16) { const __half2 hh = __floats2half2_rn(a0, a1); return *reinterpret_cast<const uint32_t*>(&hh); }
+                    const __nv_bfloat162 hb = __floats2bfloat162_rn(a0, a1);
+                    return *reinterpret_cast<const uint32_t*>(&hb);
                 };
-                auto store_frame = [&](int i, uint32_t hb, uint32_t lb) {
-                    const uint32_t addr = cell0[(i >> 1) & 3] + so + (uint32_t)i * 64u;
-                    sts16(addr, hb);
-                    sts16(addr + im_off, hb >> 16);
+                auto store8 = [&](int j, const float2 (&yv)[8]) {
+                    uint32_t hr[4], hi[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) { hr[q] = pack2(yv[2 * q].x, yv[2 * q + 1].x); hi[q] = pack2(yv[2 * q].y, yv[2 * q + 1].y); }
+                    const uint32_t addr = cell0[j] + so;
+                    sts128(addr, hr[0], hr[1], hr[2], hr[3]);
+                    sts128(addr + im_off, hi[0], hi[1], hi[2], hi[3]);
                     if (parts > 1) {
-                        sts16(addr + ST_TILE, lb);
-                        sts16(addr + im_off + ST_TILE, lb >> 16);
+                        uint32_t lr[4], li[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            lr[q] = pack2(yv[2 * q].x - __uint_as_float(hr[q] << 16), yv[2 * q + 1].x - __uint_as_float(hr[q] & 0xffff0000u));
+                            li[q] = pack2(yv[2 * q].y - __uint_as_float(hi[q] << 16), yv[2 * q + 1].y - __uint_as_float(hi[q] & 0xffff0000u));
+                        }
+                        sts128(addr + ST_TILE, lr[0], lr[1], lr[2], lr[3]);
+                        sts128(addr + im_off + ST_TILE, li[0], li[1], li[2], li[3]);
                     }
                 };
-                float2 yv[8];
-                uint32_t hb0[8], lb0[8];
-                if (MT > 1) {
-                    constexpr int FGN = 4, NG = FPW / FGN;                // frames per group, groups
 #pragma unroll
-                    for (int k = 0; k < NG; ++k) {
-                        // MAC of group k; the stores of group k - 1 (converted below) leave underneath it
+                for (int j = 0; j < FPW / 8; ++j) {
+                    float2 yv[8];
+                    if (MT > 1) {
 #pragma unroll
-                        for (int g = 0; g < FGN; ++g) yv[g] = fmul2(rg.tap[0], rg.row[k * FGN + g + WA - 1]);
+                        for (int g = 0; g < 8; ++g) yv[g] = fmul2(rg.tap[0], rg.row[8 * j + g + WA - 1]);
 #pragma unroll
-                        for (int m = 1; m < WA; ++m) {
+                        for (int m = 1; m < WA; ++m)
 #pragma unroll
-                            for (int g = 0; g < FGN; ++g) yv[g] = ffma2(rg.tap[m], rg.row[k * FGN + g + WA - 1 - m], yv[g]);
-                            if (k > 0) {
+                            for (int g = 0; g < 8; ++g) yv[g] = ffma2(rg.tap[m], rg.row[8 * j + g + WA - 1 - m], yv[g]);
+                    } else {
 #pragma unroll
-                                for (int f = 0; f < FGN; ++f)
-                                    if (f * (WA - 1) / FGN == m - 1) store_frame((k - 1) * FGN + f, hb0[f], lb0[f]);
-                            }
-                        }
-#pragma unroll
-                        for (int g = FGN; g < 8; ++g) yv[g] = make_float2(0.f, 0.f);
-                        convert(yv, hb0, lb0);
+                        for (int g = 0; g < 8; ++g) yv[g] = MT == 1 ? fmul2(rg.tap[0], rg.row[8 * j + g]) : rg.row[8 * j + g];
                     }
-#pragma unroll
-                    for (int g = 0; g < FGN; ++g) store_frame((NG - 1) * FGN + g, hb0[g], lb0[g]);
-                } else {
-#pragma unroll
-                    for (int i0 = 0; i0 < FPW; i0 += 8) {
-#pragma unroll
-                        for (int g = 0; g < 8; ++g) yv[g] = MT == 1 ? fmul2(rg.tap[0], rg.row[i0 + g]) : rg.row[i0 + g];
-                        convert(yv, hb0, lb0);
-#pragma unroll
-                        for (int g = 0; g < 8; ++g) store_frame(i0 + g, hb0[g], lb0[g]);
-                    }
+                    store8(j, yv);
                 }
                 // the window has been consumed: hand the input slot back to the TMA warp
                 __syncwarp();
