@@ -97,9 +97,10 @@ tina_status tina_dft(const void* x, void* out, long long B, int N, int inverse,
 
 /* ---------------------------------------------------------------------------------------
  * Polyphase filter bank: subfilter stage Eq. (20) followed by a P-point DFT
- * across the branches, fused in one kernel for M <= 16 (the subfiltered signals
- * never touch HBM; for 16 < M <= 64 the subfilter stage runs as its own kernel into a stream-ordered
- * temporary of S*F*P samples, followed by the contraction -- two launches):
+ * across the branches, fused in one kernel for every M <= 64 when P is a multiple of 64 (the
+ * subfiltered signals never touch HBM; 16 < M <= 64 taps are processed in groups of 16 inside the kernel).  Only for
+ * 16 < M <= 64 with a P the tensor-core kernel does not tile (not a multiple of 64) the subfilter stage runs as its
+ * own kernel into a stream-ordered temporary of S*F*P samples, followed by the contraction -- two launches:
  *     y[f][p] = sum_{m=0}^{M-1} window[m P + p] * x[(f + M-1 - m) P + p]
  *     out[f][k] = sum_{p=0}^{P-1} y[f][p] * exp(-2 pi i p k / P)
  * with x_p(n') = x[n' P + p], h_p(m) = window[m P + p], frame f <-> n' = f + M-1.

@@ -666,7 +666,12 @@ struct SmemCtlT {
 constexpr size_t ST_SMEM_BYTES = ST_A_RING + ST_B_ENTRIES * ST_B_ENTRY + ST_IN_SLOTS * ST_IN_SLOT + 4 * SY_STAGE + sizeof(SmemCtlT);
 static_assert(ST_SMEM_BYTES <= 232448, "exceeds the 227 KB shared memory opt-in limit");
 
-template <int MT, int PARTS, bool REAL>
+// GROUPED = true (MT = 16 only): 16 < M <= 64 taps.  The taps are processed in groups of 16: per chunk and group g the
+// TMA warp stages the 143 rows starting 16 g rows EARLIER and the tap rows 16 g .. 16 g + 15 (rows >= M read as
+// zeros), the producers accumulate y += sum_{m' < 16} w[16 g + m'] x[f + M-1 - 16 g - m'] over the groups in
+// registers (two sets of 8 frames so that the sums stay live) and only then split and store the operand tile: the
+// subfiltered signal never leaves the SM for any M the library accepts.
+template <int MT, int PARTS, bool REAL, bool GROUPED = false>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_out,
                 const __grid_constant__ CUtensorMap tmap_out2, const __grid_constant__ CUtensorMap tmap_x,
@@ -700,6 +705,8 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
     const int npg = prm.n_passes;
     const int b_rows = 2 * half;                                       // matrix rows per part (and per even / odd half)
     const uint32_t b_box_bytes = (uint32_t)(b_rows < NSUB ? b_rows : NSUB) / CG * ST_KC * 2;
+    static_assert(!GROUPED || MT == 16, "tap groups are groups of 16");
+    const int n_groups = GROUPED ? (M + 15) / 16 : 1;                  // tap groups per chunk (GROUPED: 16 < M <= 64)
 
     if (warp == TMA_WARP && lane == 0) {
         prefetch_tmap(&tmap_b); prefetch_tmap(&tmap_out); prefetch_tmap(&tmap_out2); prefetch_tmap(&tmap_x);
@@ -728,15 +735,16 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 const int s = tile / prm.tiles_per_stream;
                 // first input row of this CTA's window: frame f0 uses rows f0 + M - WA .. f0 + M - 1 (taps m >= M are zero)
                 const int r0 = (tile % prm.tiles_per_stream) * (BM * CG) + (int)rank * BM + M - WA;
-                for (int kc = 0; kc < n_kc; ++kc) {
-                    mbar_wait<64>(smem_u32(&ctl->in_empty[in.idx]), in.phase ^ 1);
-                    const uint32_t bar = smem_u32(&ctl->in_full[in.idx]);
-                    const uint32_t dst = smem_u32(in_ring + in.idx * ST_IN_SLOT);
-                    mbar_expect_tx(bar, (uint32_t)IN_ROWS * 256u + (MT > 0 ? (uint32_t)MT * (REAL ? 256u : 128u) : 0u));
-                    tma_load_3d(dst, &tmap_x, bar, kc * 2 * ST_KC, r0, s);       // rows outside [0, NB) arrive as zeros
-                    if (MT > 0) tma_load_2d(dst + ST_IN_TAPS, &tmap_w, bar, kc * ST_KC * (REAL ? 2 : 1), 0);   // rows >= M arrive as zeros
-                    in.advance(ST_IN_SLOTS);
-                }
+                for (int kc = 0; kc < n_kc; ++kc)
+                    for (int g = 0; g < n_groups; ++g) {
+                        mbar_wait<64>(smem_u32(&ctl->in_empty[in.idx]), in.phase ^ 1);
+                        const uint32_t bar = smem_u32(&ctl->in_full[in.idx]);
+                        const uint32_t dst = smem_u32(in_ring + in.idx * ST_IN_SLOT);
+                        mbar_expect_tx(bar, (uint32_t)IN_ROWS * 256u + (MT > 0 ? (uint32_t)MT * (REAL ? 256u : 128u) : 0u));
+                        tma_load_3d(dst, &tmap_x, bar, kc * 2 * ST_KC, r0 - 16 * g, s);   // rows outside [0, NB) arrive as zeros
+                        if (MT > 0) tma_load_2d(dst + ST_IN_TAPS, &tmap_w, bar, kc * ST_KC * (REAL ? 2 : 1), 16 * g);   // rows >= M arrive as zeros
+                        in.advance(ST_IN_SLOTS);
+                    }
             }
         }
     } else if (warp == TMA_WARP) {
@@ -869,6 +877,72 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         RingPos in, a;
         for (int w = cl; w < prm.total_work; w += n_cl)
             for (int kc = 0; kc < n_kc; ++kc) {
+                const uint32_t so = a.idx * a_slot_bytes;
+                auto pack2 = [&](float a0, float a1) -> uint32_t {        // (a0 -> low half, a1 -> high half)
+                    if (parts == 1 && prm.fp16) { const __half2 hh = __floats2half2_rn(a0, a1); return *reinterpret_cast<const uint32_t*>(&hh); }
+                    const __nv_bfloat162 hb = __floats2bfloat162_rn(a0, a1);
+                    return *reinterpret_cast<const uint32_t*>(&hb);
+                };
+                // the (hi, lo) x (re, im) parts of eight frames as four 16-byte stores
+                auto store8 = [&](int j, const float2 (&yv)[8]) {
+                    uint32_t hr[4], hi[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) { hr[q] = pack2(yv[2 * q].x, yv[2 * q + 1].x); hi[q] = pack2(yv[2 * q].y, yv[2 * q + 1].y); }
+                    const uint32_t addr = cell0[j] + so;
+                    sts128(addr, hr[0], hr[1], hr[2], hr[3]);
+                    sts128(addr + im_off, hi[0], hi[1], hi[2], hi[3]);
+                    if (parts > 1) {
+                        uint32_t lr[4], li[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            lr[q] = pack2(yv[2 * q].x - __uint_as_float(hr[q] << 16), yv[2 * q + 1].x - __uint_as_float(hr[q] & 0xffff0000u));
+                            li[q] = pack2(yv[2 * q].y - __uint_as_float(hi[q] << 16), yv[2 * q + 1].y - __uint_as_float(hi[q] & 0xffff0000u));
+                        }
+                        sts128(addr + ST_TILE, lr[0], lr[1], lr[2], lr[3]);
+                        sts128(addr + im_off + ST_TILE, li[0], li[1], li[2], li[3]);
+                    }
+                };
+                if constexpr (GROUPED) {
+                    // 16 < M <= 64: accumulate over the tap groups; eight frames at a time so that the 16 partial sums,
+                    // the 16 taps and the 23 rows of a half fit in registers
+                    float2 ya[8], yb[8];
+#pragma unroll
+                    for (int g8 = 0; g8 < 8; ++g8) { ya[g8] = make_float2(0.f, 0.f); yb[g8] = make_float2(0.f, 0.f); }
+                    for (int g = 0; g < n_groups; ++g) {
+                        pq_x = SY_NOW();
+                        mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase);
+                        pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
+                        const uint32_t src = in_lane + in.idx * ST_IN_SLOT, tsrc = tap_lane + in.idx * ST_IN_SLOT;
+                        float2 tap[16];
+#pragma unroll
+                        for (int m = 0; m < 16; ++m) {
+                            if (REAL) tap[m] = lds_f2(tsrc + (uint32_t)m * 256u);
+                            else { const float hh = lds_f1(tsrc + (uint32_t)m * 128u); tap[m] = make_float2(hh, hh); }
+                        }
+#pragma unroll
+                        for (int j = 0; j < 2; ++j) {
+                            float2 row[23];
+#pragma unroll
+                            for (int r = 0; r < 23; ++r) row[r] = lds_f2(src + (uint32_t)(8 * j + r) * 256u);
+#pragma unroll
+                            for (int m = 0; m < 16; ++m)
+#pragma unroll
+                                for (int g8 = 0; g8 < 8; ++g8) {
+                                    if (j == 0) ya[g8] = ffma2(tap[m], row[g8 + 15 - m], ya[g8]);
+                                    else        yb[g8] = ffma2(tap[m], row[g8 + 15 - m], yb[g8]);
+                                }
+                        }
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
+                        in.advance(ST_IN_SLOTS);
+                        pq_c += SY_NOW() - pq_x;
+                    }
+                    pq_x = SY_NOW();
+                    mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
+                    pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
+                    store8(0, ya);
+                    store8(1, yb);
+                } else {
                 pq_x = SY_NOW();
                 mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase);
                 pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
@@ -888,32 +962,7 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
                 mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
                 pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
-                // polyphase MAC + split + de-interleaved store, eight frames at a time: eight independent FMA chains, then
-                // the (hi, lo) x (re, im) parts of the eight frames as four 16-byte stores.
-                const uint32_t so = a.idx * a_slot_bytes;
-                auto pack2 = [&](float a0, float a1) -> uint32_t {        // (a0 -> low half, a1 -> high half)
-                    if (parts == 1 && prm.fp16) { const __half2 hh = __floats2half2_rn(a0, a1); return *reinterpret_cast<const uint32_t*>(&hh); }
-                    const __nv_bfloat162 hb = __floats2bfloat162_rn(a0, a1);
-                    return *reinterpret_cast<const uint32_t*>(&hb);
-                };
-                auto store8 = [&](int j, const float2 (&yv)[8]) {
-                    uint32_t hr[4], hi[4];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) { hr[q] = pack2(yv[2 * q].x, yv[2 * q + 1].x); hi[q] = pack2(yv[2 * q].y, yv[2 * q + 1].y); }
-                    const uint32_t addr = cell0[j] + so;
-                    sts128(addr, hr[0], hr[1], hr[2], hr[3]);
-                    sts128(addr + im_off, hi[0], hi[1], hi[2], hi[3]);
-                    if (parts > 1) {
-                        uint32_t lr[4], li[4];
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            lr[q] = pack2(yv[2 * q].x - __uint_as_float(hr[q] << 16), yv[2 * q + 1].x - __uint_as_float(hr[q] & 0xffff0000u));
-                            li[q] = pack2(yv[2 * q].y - __uint_as_float(hi[q] << 16), yv[2 * q + 1].y - __uint_as_float(hi[q] & 0xffff0000u));
-                        }
-                        sts128(addr + ST_TILE, lr[0], lr[1], lr[2], lr[3]);
-                        sts128(addr + im_off + ST_TILE, li[0], li[1], li[2], li[3]);
-                    }
-                };
+                // polyphase MAC, eight frames at a time: eight independent FMA chains, then split + de-interleaved store
 #pragma unroll
                 for (int j = 0; j < FPW / 8; ++j) {
                     float2 yv[8];
@@ -934,6 +983,7 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
                 in.advance(ST_IN_SLOTS);
+                }
                 pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
                 fence_proxy_async();
                 __syncwarp();
@@ -957,11 +1007,11 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
 // =====================================================================================
 bool sym_supported(int P) { return P >= 64 && P <= kMaxP && P % 64 == 0; }
 
-template <int MT, int PARTS, bool REAL>
+template <int MT, int PARTS, bool REAL, bool GROUPED = false>
 static tina_status launch_symt(DevCtx* ctx, const Plan* plan, const CUtensorMap& tmap_out, const CUtensorMap& tmap_out2,
                                const CUtensorMap& tmap_x, const CUtensorMap& tmap_w, const SymParams& prm, int grid, cudaStream_t st)
 {
-    auto kern = pfb_symt_kernel<MT, PARTS, REAL>;
+    auto kern = pfb_symt_kernel<MT, PARTS, REAL, GROUPED>;
     tina_status as = ensure_smem(ctx, reinterpret_cast<const void*>(kern), (int)ST_SMEM_BYTES, "cudaFuncSetAttribute(pfb_symt_kernel)");
     if (as != TINA_OK) return as;
     cudaLaunchConfig_t cfg = {};
@@ -1001,7 +1051,8 @@ static tina_status launch_symt(DevCtx* ctx, const Plan* plan, const CUtensorMap&
 #endif
     count_launch();
     g_last_path = kPathUmma;
-    note_kernel(REAL ? "pfb_symt_kernel<real>" : "pfb_symt_kernel", 0.5);
+    note_kernel(GROUPED ? (REAL ? "pfb_symt_kernel<real, tap groups>" : "pfb_symt_kernel<tap groups>")
+                        : (REAL ? "pfb_symt_kernel<real>" : "pfb_symt_kernel"), 0.5);
     if (e != cudaSuccess) return check_cuda(e, "pfb_symt_kernel launch");
     return check_cuda(cudaGetLastError(), "pfb_symt_kernel launch");
 }
@@ -1058,7 +1109,7 @@ static tina_status launch_sym(DevCtx* ctx, const CUtensorMap& tmap, const CUtens
 bool sym_real_supported(int P) { return P >= 128 && P <= kMaxP && P % 64 == 0 && !options().sym_v1; }
 
 // complex kind with P % 64 == 0, or real kind with P % 64 == 0 and P >= 128 (TMA-staged kernel only);
-// window == nullptr (DFT batch, complex) or M <= 16
+// window == nullptr (DFT batch, complex) or M <= 64 (M > 16: TMA-staged kernel only, taps in groups of 16)
 tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool real, bool inverse,
                     tina_precision prec, void* out, cudaStream_t st)
 {
@@ -1136,6 +1187,7 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
         // input as [S][NB][row] floats (row = 2P complex, P real), boxes of 64 floats (32 complex columns / 32 pairs of
         // real samples) x (128 + MT - 1) rows; the window as [M][P] floats, boxes of (32 | 64) x MT (rows >= M read as zeros)
         const int MT = !window ? 0 : (M <= 4 ? 4 : (M <= 8 ? 8 : 16));
+        if (M > kMaxTapsPfb) return fail(TINA_ERR_UNSUPPORTED, "tina_pfb: at most %d taps", kMaxTapsPfb);
         const long long row_f = real ? P : 2LL * P;
         CUtensorMap tmap_x, tmap_w;
         memset(&tmap_x, 0, sizeof(tmap_x));
@@ -1168,6 +1220,12 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
         if (MT == 0) return real ? fail(TINA_ERR_UNSUPPORTED, "real kind needs a window") : TINA_SYMT2(0, false);
         if (MT == 4) return TINA_SYMT(4);
         if (MT == 8) return TINA_SYMT(8);
+        if (M > 16) {                                              // taps in groups of 16, accumulated in registers
+            if (real) return parts == 2 ? launch_symt<16, 2, true, true>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st)
+                                        : launch_symt<16, 1, true, true>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st);
+            return parts == 2 ? launch_symt<16, 2, false, true>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st)
+                              : launch_symt<16, 1, false, true>(ctx, plan, tmap_out, tmap_out2, tmap_x, tmap_w, prm, grid, st);
+        }
         return TINA_SYMT(16);
 #undef TINA_SYMT
 #undef TINA_SYMT2

@@ -821,9 +821,11 @@ tina_status umma_pfb(const void* x, int S, long long n_samples, int P, int M, co
     const int parts = prec == TINA_PREC_FP32 ? 2 : 1;
     const bool fp16 = prec == TINA_PREC_FP16;
 
-    if (window && M > 16) {
-        // Rare shape: more taps than the register window is unrolled for.  Run the subfilter
-        // stage on its own into a stream-ordered temporary, then the contraction as a DFT batch.
+    // the column-paired, TMA-staged kernel takes every M <= 64 fused (taps in groups of 16)
+    const bool symt_ok = !options().no_sym && !options().sym_v1 && (real ? (window && sym_real_supported(P)) : sym_supported(P));
+    if (window && M > 16 && !symt_ok) {
+        // Rare shape (P not a multiple of 64, or the round-1 kernels selected): more taps than the register window is
+        // unrolled for.  Run the subfilter stage on its own into a stream-ordered temporary, then the contraction as a DFT batch.
         float* y = nullptr;
         const size_t bytes = (size_t)S * F * K * sizeof(float);
         cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&y), bytes, st);

@@ -288,13 +288,24 @@ def test_pfb_tensor_path_edges(tina, oracle, P, M, F, real, S):
         assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
 
 
-@pytest.mark.parametrize("P,M,F,real,S", [(64, 32, 70, True, 2), (128, 17, 131, False, 2), (256, 64, 40, False, 1)])
-def test_pfb_many_taps_two_launch_route(tina, oracle, P, M, F, real, S):
-    """16 < M <= 64: subfilter kernel into a stream-ordered temporary, then the contraction (two launches),
-    with several streams."""
+@pytest.mark.parametrize("P,M,F,real,S", [(64, 32, 70, True, 2), (128, 17, 131, False, 2), (256, 64, 40, False, 1),
+                                           (1024, 32, 300, False, 2), (4096, 24, 131, True, 1), (128, 33, 260, True, 2),
+                                           (96, 20, 50, False, 1), (2048, 48, 257, False, 1)])
+def test_pfb_many_taps(tina, oracle, P, M, F, real, S):
+    """16 < M <= 64.  Where the column-paired kernel tiles the shape (P a multiple of 64; real kind P >= 128) the PFB
+    stays ONE fused launch, the taps processed in groups of 16 inside the kernel (M not a multiple of 16: the last
+    group's missing taps read as zeros); other shapes take the subfilter kernel into a stream-ordered temporary
+    followed by the contraction (two launches).  Several streams, ragged tiles, several accumulation chains."""
     rng = np.random.default_rng(690 + P)
     case = ti.pfb_case(P, M, F, real=real, streams=S, seed=691 + P, window=ti.random_taps(rng, P * M))
+    launches = tina.launch_count()
     got = _run_pfb(tina, case)
+    fused = P % 64 == 0 and (P >= 128 or not real)
+    if fused:
+        assert tina.last_kernel() == ("pfb_symt_kernel<real, tap groups>" if real else "pfb_symt_kernel<tap groups>")
+        assert tina.launch_count() - launches <= 2          # the kernel (+ the one-off twiddle plan)
+    else:
+        assert not tina.last_kernel().endswith("tap groups>")
     for s in range(S):
         assert rel_l2_rows(got[s], oracle.pfb(case.x[s], P, M, case.window)) <= TOL_FP32
 
