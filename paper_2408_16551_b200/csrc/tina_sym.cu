@@ -50,6 +50,7 @@ struct SymParams {
     int fp16;
     int k_splits, kc_per_split;
     int real;                  // 1: real kind (pfb_symt_kernel<.., REAL = true>): x is float32, out rows are P + 2 floats
+    int real_tma;              // real kind: tiles leave through row-pair tensor maps (even F); 0: register / shared-memory stores
     int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 16 no mirrored-tile stores, 32 no forward-tile stores
     unsigned long long* prof;  // -DTINA_DEV only (TINA_PROF): [grid][16] cycle counters
 };
@@ -623,6 +624,161 @@ __device__ __forceinline__ void sym_epilogue_real(const SymParams& prm, const Ep
     }
 }
 
+__device__ __forceinline__ void sts64f(uint32_t addr, float a, float b)
+{
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
+}
+
+// Real-kind epilogue through the TMA engine (even F, or one stream: see sym_pfb).  Output rows are P + 2 floats, so
+// only PAIRS of rows have a 16-byte-multiple pitch: the tensor maps view the output as [S][F/2][2 (P + 2)] and a
+// warp's 32 rows leave as 16-row boxes, even rows and odd rows separately.  TMA boxes must start 16-byte aligned:
+//   forward tile  (bins kb .. kb+15, floats 2 kb ..):        even rows aligned -> 32-float box; odd rows start 8
+//                 bytes off -> 28-float box over the floats 2 .. 29 of the tile, the edge pairs (floats 0-1, 30-31)
+//                 are stored from registers;
+//   mirrored tile (bins P/2-kb-15 .. P/2-kb, floats P-2kb-30 ..): the other way round (odd rows aligned).
+// So every lane fills one swizzled 128-byte row (its "full" tile) and one dense 112-byte row (its "part" tile) per
+// step and stores two 8-byte edges; later accumulation chains use the add-reduce forms (fp32 add at L2).
+__device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, const CUtensorMap* tmap32, const CUtensorMap* tmap28,
+                                                      const EpiCtx& e, const int q, const int lane)
+{
+    constexpr int CG = UMMA_CG;
+    const int P = prm.P, quarter = P >> 2, npg = prm.n_passes;
+    const uint32_t sb = e.stage + (uint32_t)q * SY_STAGE;
+    // staging (8 KB per warp): full tiles of the even rows (forward) and of the odd rows (mirrored), 16 x 128 B
+    // swizzled; part tiles of the odd rows (forward) and of the even rows (mirrored), 16 x 112 B dense
+    const uint32_t b_fe = sb, b_mo = sb + 2048u, b_f28 = sb + 4096u, b_m28 = sb + 4096u + 1792u;
+    const uint32_t taddr = e.tmem_base + ((uint32_t)(q * 32) << 16);
+    const bool odd = (lane & 1) != 0;
+    const uint32_t rr = (uint32_t)lane >> 1, sw = rr & 7u;
+    const uint32_t full_row = (odd ? b_mo : b_fe) + rr * 128u;
+    const uint32_t part_row = (odd ? b_f28 : b_m28) + rr * 112u;
+    uint32_t tf_phase = 0;
+    long long pe_w = 0, pe_d = 0, pe_d0 = 0, pe_x, pe_tot = SY_NOW();
+    for (int w = e.cl; w < prm.total_work; w += e.n_cl) {
+        const int tile = w / npg;
+        const int k0 = (w % npg) * SY_BINS;
+        const int ncol = 2 * min(SY_BINS, quarter - k0);
+        const int s = tile / prm.tiles_per_stream;
+        const long long row0 = (long long)(tile % prm.tiles_per_stream) * (BM * CG) + e.rank * BM + q * 32;
+        const bool row_ok = lane < (int)min(32LL, prm.F - row0);
+        float* const orow = prm.out + ((long long)s * prm.F + row0 + lane) * (long long)(P + 2);
+        const int pr0 = (int)(row0 >> 1);
+        // odd F (one stream only): the last row has no partner, the row-pair maps end before it; its lane (an even
+        // one) stores everything from registers
+        const bool lone = (prm.F & 1) && row0 + lane == prm.F - 1;
+        for (int ks = 0; ks < prm.k_splits; ++ks) {
+            if (ks > 0 && lane == 0) bulk_wait<0>();          // the previous chain's stores to this tile are complete
+            pe_x = SY_NOW();
+            mbar_wait<256>(e.t_full0, tf_phase);
+            mbar_wait<256>(e.t_full1, tf_phase);
+            pe_w += SY_NOW() - pe_x; pe_x = SY_NOW();
+            tf_phase ^= 1u;
+            tc_fence_after();
+            auto put = [&](float* g, float re, float im) {        // one complex value from registers (8-byte aligned)
+                if (row_ok && !SY_DBG(16)) {
+                    float2* g2 = reinterpret_cast<float2*>(g);
+                    if (ks > 0) atomicAdd(g2, make_float2(re, im)); else *g2 = make_float2(re, im);
+                }
+            };
+            for (int cb = 0; cb < ncol; cb += 32) {
+                const int kb = k0 + (cb >> 1);
+                const bool last = cb + 32 >= ncol;
+                const int f_col = 2 * kb, m_col = P - 2 * kb - 30;      // first float of the forward / mirrored tile in a row
+                if (lane == 0) bulk_wait_read<0>();               // the staged tiles of the previous step have been read
+                __syncwarp();
+                float e0x = 0.f, e0y = 0.f, e7x = 0.f, e7y = 0.f;   // the part tile's edge pairs (floats 0-1 and 30-31)
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    // 16 accumulator columns = 8 bins at a time (32 live accumulator registers instead of 64: the
+                    // 32-column form spilled, and spill reloads queue behind the saturated shared-memory pipe)
+                    uint32_t r1[16], r2[16];
+                    tmem_ld16(taddr + cb + 16 * h, r1);
+                    tmem_ld16(taddr + 256u + cb + 16 * h, r2);
+                    tmem_ld_wait();
+                    if (last && h == 1) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) {
+                            arrive_leader<CG>(e.t_empty0, e.rank, 0);
+                            arrive_leader<CG>(e.t_empty1, e.rank, 0);
+                        }
+                        pe_d += SY_NOW() - pe_x;
+                        if (ks == 0) pe_d0 += SY_NOW() - pe_x;
+                    }
+#define SY_F(v) __uint_as_float(v)
+                    if (kb == 0 && h == 0) {
+                        // the sine slots of bin 0 carry (-1)^q: X[P/4] = D1[1] - i D2[1] (unpaired)
+                        put(orow + 2 * quarter, SY_F(r1[1]), -SY_F(r2[1]));
+                        r1[1] = 0u; r2[1] = 0u;                  // Z = V = 0 for bin 0
+                    }
+#pragma unroll
+                    for (int gg = 0; gg < 4; ++gg) {
+                        const int g = 4 * h + gg;
+                        const float U0 = SY_F(r1[4 * gg]), Z0 = SY_F(r1[4 * gg + 1]), U1 = SY_F(r1[4 * gg + 2]), Z1 = SY_F(r1[4 * gg + 3]);
+                        const float W0 = SY_F(r2[4 * gg]), V0 = SY_F(r2[4 * gg + 1]), W1 = SY_F(r2[4 * gg + 2]), V1 = SY_F(r2[4 * gg + 3]);
+                        // forward chunk g: bins kb + 2g, kb + 2g + 1 (the imaginary part of bin 0 is +0);
+                        // mirrored chunk 7 - g: bins P/2 - kb - (2g + 1), P/2 - kb - 2g
+                        const float fa = U0 + W0, fb = (kb == 0 && g == 0) ? 0.f : -(Z0 + V0), fc = U1 + W1, fd = -(Z1 + V1);
+                        const float ma = U1 - W1, mb = Z1 - V1, mc = U0 - W0, md = Z0 - V0;
+                        // full tile: even rows forward chunk g, odd rows mirrored chunk 7 - g
+                        const uint32_t cf = odd ? (uint32_t)(7 - g) : (uint32_t)g;
+                        sts128(full_row + ((cf ^ sw) << 4), __float_as_uint(odd ? ma : fa), __float_as_uint(odd ? mb : fb),
+                               __float_as_uint(odd ? mc : fc), __float_as_uint(odd ? md : fd));
+                        // part tile (floats 2 .. 29 of the other tile): odd rows forward chunk g, even rows mirrored chunk
+                        // 7 - g; chunk c sits at bytes 16 c - 8 .. 16 c + 7 of the dense row, chunks 0 / 7 lose a half to the edges
+                        const float pa = odd ? fa : ma, pb = odd ? fb : mb, pc = odd ? fc : mc, pd = odd ? fd : md;
+                        const uint32_t c_dense = odd ? (uint32_t)g : (uint32_t)(7 - g);
+                        if (g == 0) {
+                            if (odd) { e0x = pa; e0y = pb; sts64f(part_row, pc, pd); }
+                            else     { e7x = pc; e7y = pd; sts64f(part_row + 104u, pa, pb); }
+                        } else if (g == 7) {
+                            if (odd) { e7x = pc; e7y = pd; sts64f(part_row + 104u, pa, pb); }
+                            else     { e0x = pa; e0y = pb; sts64f(part_row, pc, pd); }
+                        } else {
+                            sts64f(part_row + 16u * c_dense - 8u, pa, pb);
+                            sts64f(part_row + 16u * c_dense, pc, pd);
+                        }
+                        if (lone) {                                // (an even lane) every value of the row from registers
+                            put(orow + f_col + 4 * g, fa, fb); put(orow + f_col + 4 * g + 2, fc, fd);
+                            if (g != 7) put(orow + m_col + 4 * (7 - g), ma, mb);
+                            if (g != 0) put(orow + m_col + 4 * (7 - g) + 2, mc, md);
+                        }
+                    }
+#undef SY_F
+                }
+                {
+                    float* const pbase = orow + (odd ? f_col : m_col);
+                    put(pbase, e0x, e0y);
+                    put(pbase + 30, e7x, e7y);
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) {
+                    // paired-row coordinates: an odd row starts at float P + 2 of its pair
+                    if (SY_DBG(16)) { }
+                    else if (ks == 0) {
+                        tma_store_3d(tmap32, b_fe, f_col, pr0, s);
+                        tma_store_3d(tmap32, b_mo, P + 2 + m_col, pr0, s);
+                        tma_store_3d(tmap28, b_f28, P + 2 + f_col + 2, pr0, s);
+                        tma_store_3d(tmap28, b_m28, m_col + 2, pr0, s);
+                    } else {
+                        tma_reduce_add_3d(tmap32, b_fe, f_col, pr0, s);
+                        tma_reduce_add_3d(tmap32, b_mo, P + 2 + m_col, pr0, s);
+                        tma_reduce_add_3d(tmap28, b_f28, P + 2 + f_col + 2, pr0, s);
+                        tma_reduce_add_3d(tmap28, b_m28, m_col + 2, pr0, s);
+                    }
+                    bulk_commit();
+                }
+            }
+        }
+    }
+    if (lane == 0) bulk_wait<0>();                            // staging tiles must outlive their TMA reads
+    if (SY_PROF && prm.prof && q == 0 && lane == 0) {
+        unsigned long long* pp = prm.prof + blockIdx.x * 16 + 8;
+        pp[0] = SY_NOW() - pe_tot; pp[1] = pe_w; pp[2] = pe_d; pp[3] = pe_d0;
+    }
+}
+
 // =====================================================================================
 // pfb_symt_kernel: the same contraction with the INPUT WINDOW AND THE TAPS STAGED BY TMA (the north_star
 // sketch): per chunk of 32 complex columns the (128 + MT - 1) x 32 block of input
@@ -854,7 +1010,8 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
         ec.t_full0 = smem_u32(&ctl->t_full[0]); ec.t_full1 = smem_u32(&ctl->t_full[1]);
         ec.t_empty0 = smem_u32(&ctl->t_empty[0]); ec.t_empty1 = smem_u32(&ctl->t_empty[1]);
         ec.stage = smem_u32(stage); ec.tmem_base = tmem_base; ec.rank = rank; ec.cl = cl; ec.n_cl = n_cl;
-        if (REAL) sym_epilogue_real(prm, ec, warp - EPI_WARP0, lane);
+        if (REAL && prm.real_tma) sym_epilogue_real_tma(prm, &tmap_out, &tmap_out2, ec, warp - EPI_WARP0, lane);
+        else if (REAL) sym_epilogue_real(prm, ec, warp - EPI_WARP0, lane);
         else      sym_epilogue(prm, &tmap_out, &tmap_out2, ec, warp - EPI_WARP0, lane);
     } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ FIR producers =========================================
@@ -1045,8 +1202,8 @@ static tina_status launch_symt(DevCtx* ctx, const Plan* plan, const CUtensorMap&
         if (pe != cudaSuccess) return check_cuda(pe, "TINA_PROF counter read-back");
         double acc[16] = {0};
         for (int b = 0; b < grid; b += UMMA_CG) for (int i = 0; i < 16; ++i) acc[i] += (double)h[(size_t)b * 16 + i] / (grid / UMMA_CG);
-        fprintf(stderr, "[tina prof symt] leader mean cycles: mma0 tot %.0f a_full %.0f b_full %.0f t_empty %.0f | mma1 tot %.0f a %.0f b %.0f t %.0f | epi tot %.0f t_full %.0f drain %.0f | prod tot %.0f waits %.0f lds+mac+sts %.0f fence %.0f\n",
-                acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], acc[7], acc[8], acc[9], acc[10], acc[12], acc[13], acc[14], acc[15]);
+        fprintf(stderr, "[tina prof symt] leader mean cycles: mma0 tot %.0f a_full %.0f b_full %.0f t_empty %.0f | mma1 tot %.0f a %.0f b %.0f t %.0f | epi tot %.0f t_full %.0f drain %.0f (first chain %.0f) | prod tot %.0f waits %.0f lds+mac+sts %.0f fence %.0f\n",
+                acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], acc[7], acc[8], acc[9], acc[10], acc[11], acc[12], acc[13], acc[14], acc[15]);
     }
 #endif
     count_launch();
@@ -1166,6 +1323,10 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
     tkey.p[0] = x; tkey.p[1] = window; tkey.p[2] = out;
     tkey.n[0] = n_samples;
     tkey.i[0] = S; tkey.i[1] = P; tkey.i[2] = M; tkey.i[3] = real ? 1 : 0; tkey.i[4] = staged ? 1 : 0; tkey.i[5] = 1;   // tag 1: sym_pfb
+    // real kind: the TMA epilogue views the output as row PAIRS, which needs an even number of frames per stream
+    // (an odd F is fine for ONE stream: its last row is stored from registers)
+    prm.real_tma = (real && F >= 2 && (F % 2 == 0 || S == 1) && !options().no_out_tma) ? 1 : 0;
+    tkey.i[4] += 2 * prm.real_tma;
     TmapSet tset;
     const bool cached = tmap_cache_get(ctx, tkey, &tset);
     if (cached) { memcpy(&tmap_out, tset.m[0], 128); memcpy(&tmap_out2, tset.m[1], 128); }
@@ -1182,6 +1343,21 @@ tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, con
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(out) failed (%d)", (int)r);
+    }
+    if (real && prm.real_tma && !cached) {
+        // output as [S][F/2][2 (P + 2)] floats: 16-row boxes of 32 floats (swizzled) and of 28 floats (dense)
+        const cuuint64_t dims[3] = {(cuuint64_t)2 * (P + 2), (cuuint64_t)(F / 2), (cuuint64_t)S};
+        const cuuint64_t strides[2] = {(cuuint64_t)2 * (P + 2) * sizeof(float), (cuuint64_t)(F + (F & 1)) * (P + 2) * sizeof(float)};
+        const cuuint32_t box[3] = {32, 16, 1};
+        CUresult r = enc(&tmap_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        const cuuint32_t box2[3] = {28, 16, 1};
+        if (r == CUDA_SUCCESS)
+            r = enc(&tmap_out2, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, out, dims, strides, box2, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(out, row pairs) failed (%d)", (int)r);
     }
     if (staged) {
         // input as [S][NB][row] floats (row = 2P complex, P real), boxes of 64 floats (32 complex columns / 32 pairs of

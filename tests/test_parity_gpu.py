@@ -262,11 +262,13 @@ def test_pfb_batched_streams_and_tail(tina, oracle):
 
 
 @pytest.mark.parametrize("P,M,F,S", [(128, 4, 130, 2), (128, 4, 129, 2), (2048, 2, 258, 2), (1024, 3, 131, 3),
-                                     (2048, 2, 259, 2), (4096, 2, 131, 3), (2048, 3, 1, 2)])
+                                     (2048, 2, 259, 2), (4096, 2, 131, 3), (2048, 3, 1, 2),
+                                     (128, 4, 33, 1), (512, 8, 257, 1), (4096, 2, 67, 1), (8192, 2, 2, 1), (256, 4, 1, 1)])
 def test_pfb_real_batched_epilogue_paths(tina, oracle, P, M, F, S):
-    """Real kind, several streams: even F takes the TMA-store epilogue (row-pair tensor maps), odd F
-    with S > 1 the register/shared-memory store path; P >= 1024 adds several accumulation chains
-    (read-modify-write of the output) and several column passes."""
+    """Real kind: even F takes the TMA-store epilogue (row-pair tensor maps; 32- and 28-float boxes plus register
+    edges), odd F with ONE stream too (its last row is stored from registers), odd F with S > 1 and F = 1 the
+    register / shared-memory store path; P >= 1024 adds several accumulation chains (read-modify-write of the
+    output) and several column passes."""
     case = ti.pfb_case(P, M, F, real=True, streams=S, seed=650 + P + F)
     got = _run_pfb(tina, case)
     assert got.shape == (S, F, P // 2 + 1)
