@@ -110,6 +110,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
             if ((threadIdx.x & 31) == 0)
                 printf("[tina] mbarrier wait timed out: block %d warp %d barrier smem 0x%x parity %u\n",
                        (int)blockIdx.x, (int)(threadIdx.x >> 5), bar, parity);
+            // let the other stuck warps report too before the kernel is aborted
+            { const long long t1 = clock64(); while (clock64() - t1 < 600000000LL) { if (mbar_try_wait(bar, parity)) return; } }
 #endif
             __trap();
         }
