@@ -170,6 +170,12 @@ __device__ __forceinline__ void tma_store_3d(const void* tmap, uint32_t src, int
     asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
                  ::"l"(tmap), "r"(src), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
+// same with an L2 cache policy (createpolicy): used to keep a tile resident for a later add-reduce pass
+__device__ __forceinline__ void tma_store_3d_hint(const void* tmap, uint32_t src, int c0, int c1, int c2, uint64_t policy)
+{
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;"
+                 ::"l"(tmap), "r"(src), "r"(c0), "r"(c1), "r"(c2), "l"(policy) : "memory");
+}
 __device__ __forceinline__ void tma_reduce_add_3d(const void* tmap, uint32_t src, int c0, int c1, int c2)
 {
     asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];"

@@ -166,6 +166,10 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
     const uint32_t taddr = e.tmem_base + ((uint32_t)(q * 32) << 16);
     const uint32_t rowoff = (uint32_t)lane * 128u, sw = (uint32_t)lane & 7u;
     uint32_t tf_phase = 0;
+    // several accumulation chains (P > 1024): the first chain's tiles are stored with an L2 evict-last policy so that
+    // the later chains' add-reduce finds them resident
+    const bool keep_l2 = prm.k_splits > 1;
+    const uint64_t pol_keep = l2_policy_evict_last();
     long long pe_w = 0, pe_d = 0, pe_x, pe_tot = SY_NOW();
     for (int w = e.cl; w < prm.total_work; w += e.n_cl) {
         const int tile = w / npg;
@@ -230,6 +234,7 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
                 __syncwarp();
                 if (lane == 0) {
                     if (SY_DBG(32)) { }
+                    else if (ks == 0 && keep_l2) tma_store_3d_hint(tmap_out, sb_f, 2 * kb, (int)row0, s, pol_keep);
                     else if (ks == 0) tma_store_3d(tmap_out, sb_f, 2 * kb, (int)row0, s);
                     else              tma_reduce_add_3d(tmap_out, sb_f, 2 * kb, (int)row0, s);
                     bulk_commit();
@@ -263,11 +268,13 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
                     if (SY_DBG(16)) { }
                     else if (!last) {
                         const int cm = 2 * (P - kb - 16);
-                        if (ks == 0) tma_store_3d(tmap_out, sb_m, cm, (int)row0, s);
+                        if (ks == 0 && keep_l2) tma_store_3d_hint(tmap_out, sb_m, cm, (int)row0, s, pol_keep);
+                        else if (ks == 0) tma_store_3d(tmap_out, sb_m, cm, (int)row0, s);
                         else         tma_reduce_add_3d(tmap_out, sb_m, cm, (int)row0, s);
                     } else {
                         const int cm = 2 * (P - kb - 14);
-                        if (ks == 0) tma_store_3d(tmap_out2, sb_m, cm, (int)row0, s);
+                        if (ks == 0 && keep_l2) tma_store_3d_hint(tmap_out2, sb_m, cm, (int)row0, s, pol_keep);
+                        else if (ks == 0) tma_store_3d(tmap_out2, sb_m, cm, (int)row0, s);
                         else         tma_reduce_add_3d(tmap_out2, sb_m, cm, (int)row0, s);
                     }
                     bulk_commit();
@@ -653,6 +660,8 @@ __device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, cons
     const uint32_t full_row = (odd ? b_mo : b_fe) + rr * 128u;
     const uint32_t part_row = (odd ? b_f28 : b_m28) + rr * 112u;
     uint32_t tf_phase = 0;
+    const bool keep_l2 = prm.k_splits > 1;
+    const uint64_t pol_keep = l2_policy_evict_last();
     long long pe_w = 0, pe_d = 0, pe_d0 = 0, pe_x, pe_tot = SY_NOW();
     for (int w = e.cl; w < prm.total_work; w += e.n_cl) {
         const int tile = w / npg;
@@ -756,7 +765,12 @@ __device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, cons
                 if (lane == 0) {
                     // paired-row coordinates: an odd row starts at float P + 2 of its pair
                     if (SY_DBG(16)) { }
-                    else if (ks == 0) {
+                    else if (ks == 0 && keep_l2) {                // a later chain adds into this tile: keep it in L2
+                        tma_store_3d_hint(tmap32, b_fe, f_col, pr0, s, pol_keep);
+                        tma_store_3d_hint(tmap32, b_mo, P + 2 + m_col, pr0, s, pol_keep);
+                        tma_store_3d_hint(tmap28, b_f28, P + 2 + f_col + 2, pr0, s, pol_keep);
+                        tma_store_3d_hint(tmap28, b_m28, m_col + 2, pr0, s, pol_keep);
+                    } else if (ks == 0) {
                         tma_store_3d(tmap32, b_fe, f_col, pr0, s);
                         tma_store_3d(tmap32, b_mo, P + 2 + m_col, pr0, s);
                         tma_store_3d(tmap28, b_f28, P + 2 + f_col + 2, pr0, s);
