@@ -279,8 +279,8 @@ def run_reference(args, w):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "gpu_launches": 0,
-        "config": {"workload": args.workload, **{k: v for k, v in w.items() if k != "call"},
-                   "note": "each step = a bounded sample of the workload run through the float64 oracle"},
+        "config": config_of(args.workload, w),
+        "run": {"note": "each step = a bounded sample of the workload run through the float64 oracle (host cores, no GPU)"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
@@ -288,6 +288,25 @@ def run_reference(args, w):
 
 
 L2_BYTES = 126e6
+
+
+def l2_plan(w):
+    """(set_bytes, rotate, n_sets): working sets below ~1 GB are timed cold by rotating over distinct buffer sets."""
+    _, byts, _, _ = useful_flops_and_bytes(w)
+    set_bytes = 3 * 8.0 * w["B"] * w["N"] if w["call"] == "dft" else byts      # dft: x, out and back buffers
+    rotate = set_bytes < 8 * L2_BYTES
+    n_sets = int(min(512, max(4, np.ceil(2.5 * L2_BYTES / set_bytes)))) if rotate else 1
+    return set_bytes, rotate, n_sets
+
+
+def config_of(workload, w):
+    """The `config` object of the JSON line: the workload and how consecutive steps are kept out of L2.  Identical for
+    both arms (`--impl ours|reference`); everything that describes the RUN rather than the workload goes to `run`."""
+    set_bytes, rotate, n_sets = l2_plan(w)
+    return {"workload": workload, **{k: v for k, v in w.items() if k != "call"},
+            "l2": (f"cold: rotating over {n_sets} distinct buffer sets ({n_sets * set_bytes / 1e6:.0f} MB > 2x L2); the hot "
+                   "(same buffers) timing is in `hot`") if rotate else
+                  "inputs and outputs each exceed the 126 MB L2; no explicit flush"}
 
 
 def run_ours(args, w):
@@ -360,9 +379,7 @@ def run_ours(args, w):
     # Working sets smaller than ~8x L2 are timed twice: HOT (the same buffers every step) and COLD (rotating
     # over >= 4 distinct buffer sets totalling > 2x L2, so no step finds its data in L2).  HBM fractions and
     # `value` are quoted from the cold run.
-    set_bytes = 3 * 8.0 * w["B"] * w["N"] if w["call"] == "dft" else byts      # dft: x, out and back buffers
-    rotate = set_bytes < 8 * L2_BYTES
-    n_sets = int(min(512, max(4, np.ceil(2.5 * L2_BYTES / set_bytes)))) if rotate else 1
+    set_bytes, rotate, n_sets = l2_plan(w)
     steps_of = [make_set() for _ in range(n_sets)]
 
     def barrier():
@@ -489,12 +506,9 @@ def run_ours(args, w):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": ("bf16x3->f32" if w.get("prec", 0) == 0 else ("bf16" if w.get("prec", 0) == 1 else "f16")) if (tensor_bound or w["call"] == "pfb_fft") else "f32",
         "data": "synthetic", "spectra_per_s": world * frames / (ms_per_step * 1e-3),
-        "config": {"workload": args.workload, **{k: v for k, v in w.items() if k != "call"},
-                   "l2": (f"cold: rotating over {n_sets} distinct buffer sets ({n_sets * set_bytes / 1e6:.0f} MB > 2x L2); the hot "
-                          "(same buffers) timing is in `hot`") if rotate else
-                         "inputs and outputs each exceed the 126 MB L2; no explicit flush",
-                   "path": {0: "none", 1: "cuda-core", 2: "tcgen05"}[tina.last_path()],
-                   "parallelism": f"frame-sharded replicas x{world}, no collective"},
+        "config": config_of(args.workload, w),
+        "run": {"path": {0: "none", 1: "cuda-core", 2: "tcgen05"}[tina.last_path()],
+                "parallelism": f"frame-sharded replicas x{world}, no collective"},
         "roofline": roof, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "tina_env": env,
     }
     if args.profile:
