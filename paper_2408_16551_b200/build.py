@@ -10,7 +10,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtina.so")
-SOURCES = ["tina_api.cu", "tina_simt.cu", "tina_umma.cu", "tina_sym.cu", "tina_firt.cu", "tina_ct.cu", "tina_ctr.cu", "tina_arith.cu", "tina_peaks.cu"]
+SOURCES = ["tina_api.cu", "tina_simt.cu", "tina_umma.cu", "tina_sym.cu", "tina_symf.cu", "tina_firt.cu", "tina_ct.cu", "tina_ctr.cu", "tina_arith.cu", "tina_peaks.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

@@ -54,6 +54,7 @@ static void load_options_locked()
     o.ctr_ws = on("TINA_CTR_WS");
     o.no_sym = on("TINA_NO_SYM");
     o.sym_v1 = on("TINA_SYM_V1");
+    o.fold = on("TINA_SYM_FOLD");
 #ifdef TINA_DEV
     auto num = [](const char* n) { const char* v = getenv(n); return v ? atoi(v) : 0; };
     o.debug_skip = num("TINA_DEBUG_SKIP");
@@ -428,6 +429,7 @@ const char* tina_last_error(void) { return t_err; }
 tina_status tina_clear_plan_cache(void)
 {
     umma_clear_plans();
+    symf_clear_plans();
     dev_ctx_release_all();
     return TINA_OK;
 }

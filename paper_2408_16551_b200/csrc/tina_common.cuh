@@ -43,6 +43,7 @@ struct Options {
     bool ctr_ws = false;       // TINA_CTR_WS: warp-specialised factorised real kernel
     bool no_sym = false;       // TINA_NO_SYM: complex dense contraction without the k <-> P-k column pairing
     bool sym_v1 = false;       // TINA_SYM_V1: column-paired contraction with register-window producers (no TMA input staging)
+    bool fold = false;         // TINA_SYM_FOLD: complex kind with the row pairs folded as well (pfb_symf_kernel; measured: no faster)
     // -DTINA_DEV only (always 0 / false otherwise):
     int debug_skip = 0, ksplit = 0, a_slots = 0, b_entries = 0, cl4 = 0;
     bool prof = false;
@@ -117,6 +118,11 @@ bool sym_supported(int P);
 bool sym_real_supported(int P);     // real kind: even / odd samples against the columns of the bins [0, P/4)
 tina_status sym_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool real, bool inverse,
                     tina_precision prec, void* out, cudaStream_t st);
+// complex kind with the row pairs (p, P-p) folded as well (tina_symf.cu): window == nullptr or M <= 16
+bool symf_supported(int P, int M, bool has_window);
+tina_status symf_pfb(const void* x, int S, long long n_samples, int P, int M, const float* window, bool inverse,
+                     tina_precision prec, void* out, cudaStream_t st);
+void symf_clear_plans();
 // PFB with the factorised (two-stage, 32 x 32) Fourier stage: complex kind, P = 1024, M <= 16 (tina_ct.cu)
 tina_status ct_pfb(const void* x, int S, long long n_samples, int M, const float* window, void* out, cudaStream_t st);
 tina_status arith_ew(const float* a, const float* b, float* o, long long n, bool mul, cudaStream_t st);

@@ -344,6 +344,32 @@ def test_pfb_column_paired_variants_agree(tina, oracle, tina_env):
         tina_env(**{k: 0 for k in env})
 
 
+@pytest.mark.parametrize("P,M,F,S", [(64, 4, 200, 1), (128, 16, 257, 2), (320, 5, 300, 1), (192, 3, 257, 2), (1024, 16, 700, 3),
+                                     (1024, 1, 130, 1), (2048, 2, 300, 2), (4096, 8, 131, 1), (8192, 2, 40, 1)])
+def test_pfb_row_paired_kernel(tina, oracle, tina_env, P, M, F, S):
+    """TINA_SYM_FOLD=1: the complex kind with the row pairs (p, P - p) of the Fourier matrix folded as well
+    (pfb_symf_kernel, tina_symf.cu): narrow last passes (P = 320, 192), two chunks per pass (P = 64), the unpaired
+    samples p = 0 and p = P/2, the Nyquist bin through the extra matrix rows, several accumulation chains (P >= 4096),
+    several streams and ragged tiles; DFT batches (no window) forward and inverse, single pass too."""
+    import torch
+    tina_env(TINA_SYM_FOLD=1)
+    rng = np.random.default_rng(1640 + P + M)
+    case = ti.pfb_case(P, M, F, real=False, streams=S, seed=1641 + P + F, window=ti.random_taps(rng, P * M))
+    got = _run_pfb(tina, case)
+    assert tina.last_kernel() == "pfb_symf_kernel"
+    for s in range(S):
+        ref = oracle.pfb(case.x[s], P, M, case.window)
+        assert rel_l2_rows(got[s], ref) <= TOL_FP32
+    if M <= 4:
+        x = ti.noise_complex(np.random.default_rng(P), 300 * P).reshape(300, P)
+        Z = tina.dft(_cuda(x)); xb = tina.dft(Z, inverse=True); torch.cuda.synchronize()
+        assert tina.last_kernel() == "pfb_symf_kernel"
+        assert rel_l2_rows(Z.cpu().numpy(), oracle.dft(x)) <= TOL_FP32
+        assert rel_l2_rows(xb.cpu().numpy(), x.astype(np.complex128)) <= 2 * TOL_FP32
+        Zb = tina.dft(_cuda(x), prec=1); torch.cuda.synchronize()
+        assert rel_l2_rows(Zb.cpu().numpy(), oracle.dft(x)) <= TOL_BF16
+
+
 def test_pfb_complex_multichain_batched(tina, oracle):
     """Complex kind, K = 4096: four accumulation chains (TMA add-reduce epilogue), 8 column passes,
     ragged last tile, 2 streams."""
