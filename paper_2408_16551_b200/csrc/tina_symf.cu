@@ -400,11 +400,20 @@ pfb_symf_kernel(const __grid_constant__ FoldMaps maps, const SymParams prm, cons
 #pragma unroll
                         for (int g = 0; g < 8; ++g) yv[g] = MT == 1 ? fmul2(tap[0], row[8 * j + g]) : row[8 * j + g];
                     }
+                    if (kc == 0) {                                   // (warp-uniform) the general form, for the two unpaired samples
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) {
-                        const float px = __shfl_xor_sync(0xffffffffu, yv[g].x, 16), py = __shfl_xor_sync(0xffffffffu, yv[g].y, 16);
-                        yv[g].x = fmaf(cp, px, co * yv[g].x);
-                        yv[g].y = fmaf(cp, py, co * yv[g].y);
+                        for (int g = 0; g < 8; ++g) {
+                            const float px = __shfl_xor_sync(0xffffffffu, yv[g].x, 16), py = __shfl_xor_sync(0xffffffffu, yv[g].y, 16);
+                            yv[g].x = fmaf(cp, px, co * yv[g].x);
+                            yv[g].y = fmaf(cp, py, co * yv[g].y);
+                        }
+                    } else {
+#pragma unroll
+                        for (int g = 0; g < 8; ++g) {
+                            const float px = __shfl_xor_sync(0xffffffffu, yv[g].x, 16), py = __shfl_xor_sync(0xffffffffu, yv[g].y, 16);
+                            yv[g].x = fmaf(co, yv[g].x, px);
+                            yv[g].y = fmaf(co, yv[g].y, py);
+                        }
                     }
                     uint32_t hr[4], hi[4];
 #pragma unroll
