@@ -33,6 +33,14 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// arrive once the register `dep` has been written: used to hand a staged buffer back as soon as the ld.shared that
+// filled `dep` (the LAST load from that buffer; shared-memory loads of a warp complete in order) has returned, without
+// waiting for the arithmetic that consumes the data (the predicate is always true, it only carries the dependency)
+__device__ __forceinline__ void mbar_arrive_after(uint32_t bar, uint32_t dep)
+{
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tor.b32 t, %1, 1;\n\tsetp.ne.u32 p, t, 0;\n\t"
+                 "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n\t}" ::"r"(bar), "r"(dep) : "memory");
+}
 // shared::cluster address of the same smem offset in CTA `cta` of the cluster
 __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t cta)
 {

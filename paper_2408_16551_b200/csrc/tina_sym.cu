@@ -919,6 +919,10 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
 #pragma unroll
                     for (int j = 0; j < WA - 1 + FPW; ++j) rg.row[j] = lds_f2(src + (uint32_t)j * 256u);
                 }
+                // the window is in registers once its last load has returned: hand the input slot back to the TMA warp now,
+                // a whole subfilter computation earlier than after the stores (the copy of the next chunk but one needs the lead)
+                if (lane == 0) mbar_arrive_after(smem_u32(&ctl->in_empty[in.idx]), __float_as_uint(rg.row[WA - 2 + FPW].y));
+                in.advance(ST_IN_SLOTS);
                 pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
                 mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1);
                 pq_w += SY_NOW() - pq_x; pq_x = SY_NOW();
@@ -939,10 +943,6 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     }
                     store8(j, yv);
                 }
-                // the window has been consumed: hand the input slot back to the TMA warp
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
-                in.advance(ST_IN_SLOTS);
                 }
                 pq_c += SY_NOW() - pq_x; pq_x = SY_NOW();
                 fence_proxy_async();
