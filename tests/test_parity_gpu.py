@@ -370,6 +370,25 @@ def test_pfb_row_paired_kernel(tina, oracle, tina_env, P, M, F, S):
         assert rel_l2_rows(Zb.cpu().numpy(), oracle.dft(x)) <= TOL_BF16
 
 
+@pytest.mark.parametrize("P,M,S,F,real", [(1024, 16, 4, 2100, False), (2048, 8, 1, 4099, True), (256, 4, 4, 16384, False), (512, 40, 2, 1500, False)])
+def test_pfb_repeated_launches_bit_identical(tina, P, M, S, F, real):
+    """300 back-to-back launches on the same buffers give bit-identical results (the ring / barrier protocols of the
+    fused kernels, the early hand-back of the input slot and the add-reduce order of later accumulation chains are
+    deterministic; a race would show up as a differing launch)."""
+    import torch
+    n = (F + M - 1) * P
+    g = torch.Generator(device="cuda").manual_seed(P + M)
+    x = torch.randn(S, n, device="cuda", generator=g) if real else torch.view_as_complex(torch.randn(S, n, 2, device="cuda", generator=g))
+    w = torch.randn(M, P, device="cuda", generator=g)
+    out = tina.pfb(x, P, M, w); torch.cuda.synchronize()
+    ref = out.clone()
+    for it in range(300):
+        out = tina.pfb(x, P, M, w, out=out)
+        if it % 50 == 49:
+            torch.cuda.synchronize()
+            assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref)), it
+
+
 def test_pfb_complex_multichain_batched(tina, oracle):
     """Complex kind, K = 4096: four accumulation chains (TMA add-reduce epilogue), 8 column passes,
     ragged last tile, 2 streams."""
