@@ -12,12 +12,16 @@
 // load latency, 0.46 of the HBM roofline):
 //   * the Toeplitz matrix is built ONCE per CTA from the taps, straight into shared memory, and stays resident
 //     (no per-call toeplitz_kernel, no tensor map, no B ring, no L2 traffic for B);
-//   * the signal is staged by TMA: a 3-D map {128, L / 128, C} over x, boxes of 32 floats x 128 rows; chunk kc of
+//   * the signal is staged by TMA: a 3-D map {128, L / 128, C} over x, 128-byte-swizzled boxes of 32 floats x 128 rows; chunk kc of
 //     a tile is the box at column 32 (kc % 4) of row (tile row + kc / 4) -- the overlap of the A rows costs
 //     nothing but L2 bandwidth, and rows past the end of a channel arrive as zeros;
-//   * the producers only convert: ld.shared.v2 -> bf16x2 hi, exact remainder, bf16x2 lo -> two conflict-free
-//     32-bit st.shared into the 64-byte-swizzled A tiles;
-//   * four TMEM accumulator stages of 128 columns, so the epilogue of a tile overlaps the MMAs of the next three.
+//   * the producers only convert, and the A operand lives in TENSOR MEMORY, not in shared memory: a producer lane
+//     owns one row of the staged 128 x 32 block (ld.shared.v4 from the 128-byte-swizzled TMA box), packs bf16x2 hi
+//     and the exact remainder's bf16x2 lo, and writes both with tcgen05.st into the 128 TMEM columns kept for A
+//     (4 slots x (16 hi + 16 lo) columns); the MMAs read A from there (tcgen05.mma with a TMEM A operand), so the
+//     operand costs neither st.shared nor tensor-core shared-memory reads -- shared-memory bandwidth was the bound
+//     of the shared-memory-operand version (r02 captures: 82 % of the 128 B/clk pipe);
+//   * three TMEM accumulator stages of 128 columns, so the epilogue of a tile overlaps the MMAs of the next two.
 // CTA pair, tcgen05.mma.cta_group::2, M = 256 (each CTA 128 rows), N = 128 (each CTA holds 64 rows of B).
 // Needs L % 128 == 0 (the 3-D view) and M <= 193; other shapes keep the round-1 route or the CUDA-core kernel.
 #include "tina_umma.cuh"
@@ -31,17 +35,19 @@ using namespace ptx;
 
 constexpr int FT_T = 128;                         // outputs per block (GEMM N) and A row pitch
 constexpr int FT_KC = 32;                         // contraction elements per chunk (64-byte rows, SWIZZLE_64B)
-constexpr int FT_A_TILE = BM * FT_KC * 2;         // 8 KB
-constexpr int FT_A_SLOT = 2 * FT_A_TILE;          // hi | lo
+constexpr int FT_A_COLS = FT_KC / 2;              // TMEM columns of one part (hi or lo) of an A chunk: bf16 pairs
+constexpr int FT_A_SLOTS = 4;                     // A chunks resident in TMEM
 constexpr int FT_B_TILE = (FT_T / UMMA_CG) * FT_KC * 2;   // 4 KB: this CTA's 64 rows of one chunk and part
 constexpr int FT_IN_SLOT = BM * FT_KC * 4;        // 16 KB fp32
 constexpr int FT_PITCH = 129;                     // staged row pitch (floats) of the epilogue: odd, see below
 constexpr int FT_STAGE = 32 * FT_PITCH * 4;       // per epilogue warp
-constexpr int FT_ACC = 4;                         // TMEM accumulator stages of 128 columns
+constexpr int FT_ACC = 3;                         // TMEM accumulator stages of 128 columns
+constexpr int FT_A_COL0 = FT_ACC * FT_T;          // first TMEM column of the A slots
+static_assert(FT_A_COL0 + FT_A_SLOTS * 2 * FT_A_COLS <= 512, "TMEM budget");
 
 struct FirtCtl {
     uint64_t a_full[4], a_empty[4];
-    uint64_t in_full[4], in_empty[4];
+    uint64_t in_full[8], in_empty[8];
     uint64_t t_full[FT_ACC], t_empty[FT_ACC];
     uint64_t b_free, b_ready;          // per-channel taps: "all MMAs that read the old matrix are done" / "new matrix written"
     uint32_t tmem_base;
@@ -54,10 +60,10 @@ struct FirtParams {
     int M, n_kc;               // taps, chunks (Kp / 32)
     int taps_stride;           // 0: one tap vector; M: one per channel
     int tiles_per_chan, total_work;
-    int a_slots, in_slots;     // ring depths (even: see the producers)
+    int in_slots;              // input ring depth (even: see the producers)
     int b_part_bytes;          // bytes of one part (hi or lo) of the resident band matrix, multiple of 1024
     unsigned long long* prof;  // -DTINA_DEV only (TINA_PROF): [grid][16] cycle counters
-    int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 128 no global stores, 256 no TMA loads, 512 no MMAs, 1024 no operand stores, 2048 no TMEM read-out
+    int debug;                 // -DTINA_DEV only (TINA_DEBUG_SKIP): 128 no global stores, 256 no TMA loads, 512 no MMAs, 1024 no operand writes, 2048 no TMEM read-out
 };
 #ifdef TINA_DEV
 #define FT_DBG(b) (prm.debug & (b))
@@ -93,8 +99,7 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
     // n' in [64 rank - 32 (n_kc - 1), 64 rank + 64) once (hi | lo) and chunk kc's B tile starts 32 (n_kc - 1 - kc) rows in.
     uint8_t* b_res = smem;
     const uint32_t b_part = (uint32_t)prm.b_part_bytes;                   // bytes of one part, multiple of 1024
-    uint8_t* a_ring = b_res + 2 * (size_t)b_part;
-    uint8_t* in_ring = a_ring + (size_t)prm.a_slots * FT_A_SLOT;
+    uint8_t* in_ring = b_res + 2 * (size_t)b_part;
     uint8_t* stage = in_ring + (size_t)prm.in_slots * FT_IN_SLOT;
     FirtCtl* ctl = reinterpret_cast<FirtCtl*>(stage + 4 * FT_STAGE);
 
@@ -103,7 +108,8 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
     constexpr uint32_t leader = 0;
     constexpr uint16_t pair_mask = 3;
     const int cl = blockIdx.x / CG, n_cl = gridDim.x / CG;
-    const uint32_t n_a = (uint32_t)prm.a_slots, n_in = (uint32_t)prm.in_slots;
+    constexpr uint32_t n_a = FT_A_SLOTS;
+    const uint32_t n_in = (uint32_t)prm.in_slots;
     // contiguous ranges of tiles per pair: a pair stays inside a channel as long as possible (per-channel taps
     // rebuild the Toeplitz matrix only when the channel changes)
     const int per = (prm.total_work + n_cl - 1) / n_cl;
@@ -111,9 +117,11 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
 
     if (warp == TMA_WARP && lane == 0) {
         prefetch_tmap(&tmap_x);
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < FT_A_SLOTS; ++i) {
             mbar_init(smem_u32(&ctl->a_full[i]), N_PROD_WARPS / 2 + (rank == 0 ? CG - 1 : 0));   // one producer group per chunk
             mbar_init(smem_u32(&ctl->a_empty[i]), 1);
+        }
+        for (int i = 0; i < 8; ++i) {
             mbar_init(smem_u32(&ctl->in_full[i]), 1);
             mbar_init(smem_u32(&ctl->in_empty[i]), N_PROD_WARPS / 2);
         }
@@ -216,19 +224,18 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                     pm_x = FT_NOW(); mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase); pm_a += FT_NOW() - pm_x;
                     tc_fence_after();
                     if (lane == 0) {
-                        const uint64_t a_hi = smem_desc_sw64(smem_u32(a_ring + a.idx * FT_A_SLOT));
-                        const uint64_t a_lo = smem_desc_sw64(smem_u32(a_ring + a.idx * FT_A_SLOT + FT_A_TILE));
+                        const uint32_t a_hi = tmem_base + FT_A_COL0 + a.idx * (2 * FT_A_COLS), a_lo = a_hi + FT_A_COLS;
                         const uint32_t b_off = (uint32_t)(n_kc - 1 - kc) * (FT_KC * 64u);     // 32 rows of 64 B per chunk step
                         const uint64_t b_hi = smem_desc_sw64(b_s + b_off);
                         const uint64_t b_lo = smem_desc_sw64(b_s + b_off + b_part);
                         uint32_t acc = kc > 0;
                         if (!FT_DBG(512)) {
 #pragma unroll
-                        for (int k = 0; k < FT_KC / 16; ++k) { umma_bf16<CG>(d, a_lo + 2 * k, b_hi + 2 * k, idesc, acc); acc = 1; }
+                        for (int k = 0; k < FT_KC / 16; ++k) { umma_bf16_ts<CG>(d, a_lo + 8 * k, b_hi + 2 * k, idesc, acc); acc = 1; }
 #pragma unroll
-                        for (int k = 0; k < FT_KC / 16; ++k) umma_bf16<CG>(d, a_hi + 2 * k, b_hi + 2 * k, idesc, 1);
+                        for (int k = 0; k < FT_KC / 16; ++k) umma_bf16_ts<CG>(d, a_hi + 8 * k, b_hi + 2 * k, idesc, 1);
 #pragma unroll
-                        for (int k = 0; k < FT_KC / 16; ++k) umma_bf16<CG>(d, a_hi + 2 * k, b_lo + 2 * k, idesc, 1);
+                        for (int k = 0; k < FT_KC / 16; ++k) umma_bf16_ts<CG>(d, a_hi + 8 * k, b_lo + 2 * k, idesc, 1);
                         }
                         commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
                         if (kc == n_kc - 1) commit_cg<CG>(smem_u32(&ctl->t_full[t.idx]), pair_mask);
@@ -300,17 +307,16 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
         if (prm.prof && q == 0 && lane == 0) { unsigned long long* pp = prm.prof + blockIdx.x * 16; pp[5] = FT_NOW() - pe_tot; pp[6] = pe_w; pp[7] = pe_s; }
     } else if (warp >= PROD_WARP0 && warp < PROD_WARP0 + N_PROD_WARPS) {
         // ============================ producers: fp32 -> bf16 hi / lo =========================
-        // Two groups of four warps take alternate chunks (a chunk's fence / barrier round trip overlaps the other
-        // group's conversion; ring depths are even, so a slot always belongs to one group); within a group warp pwl
-        // converts rows 32 pwl .. +31 of the staged 128 x 32 block; lanes 0-15 take an even row, lanes 16-31 the next
-        // one, each lane two adjacent contraction elements (one 32-bit operand word per part).
+        // Two groups of four warps take alternate chunks (a chunk's tcgen05.st / barrier round trip overlaps the other
+        // group's conversion; the ring depths are even, so a slot always belongs to one group); within a group warp pwl
+        // converts rows 32 pwl .. +31 of the staged 128 x 32 block, ONE ROW PER LANE (= its lane of TMEM lane quarter
+        // pwl = warp % 4): eight 16-byte loads from the 128-byte-swizzled row (a quarter warp covers all 32 banks),
+        // 16 + 16 packed bf16x2 words, two tcgen05.st.
         const int pw = warp - PROD_WARP0;
         const uint32_t grp = (uint32_t)pw >> 2, pwl = (uint32_t)pw & 3u;
-        constexpr int RPW = 2 * FPW;                                       // rows per warp and chunk
-        const uint32_t hl = (uint32_t)lane >> 4, wl = (uint32_t)lane & 15u;
-        const uint32_t in_lane = smem_u32(in_ring) + (pwl * RPW + hl) * 128u + wl * 8u;
-        const uint32_t a_lane = smem_u32(a_ring) + (pwl * RPW + hl) * 64u + (wl & 3u) * 4u;
-        const uint32_t wc = wl >> 2;                                       // 16-byte chunk of the operand word
+        static_assert(PROD_WARP0 % 4 == 0 && FT_KC == 32, "producer warp pwl owns TMEM lanes 32 pwl .. +31");
+        const uint32_t in_lane = smem_u32(in_ring) + (pwl * 32u + (uint32_t)lane) * 128u, sw = (uint32_t)lane & 7u;
+        const uint32_t a_t = tmem_base + ((pwl * 32u) << 16) + FT_A_COL0;
         RingPos in, a;
         uint32_t bf_phase = 0;
         long long pp_i = 0, pp_a = 0, pp_x, pp_tot = FT_NOW();
@@ -327,31 +333,31 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
             for (int kc = 0; kc < n_kc; ++kc, ++n_chunk) {
                 if ((n_chunk & 1u) != grp) { in.advance(n_in); a.advance(n_a); continue; }
                 pp_x = FT_NOW(); mbar_wait(smem_u32(&ctl->in_full[in.idx]), in.phase); pp_i += FT_NOW() - pp_x;
-                float2 v[RPW / 2];
+                uint32_t hb[FT_A_COLS], lb[FT_A_COLS];
 #pragma unroll
-                for (int i = 0; i < RPW / 2; ++i) v[i] = firt_lds_f2(in_lane + in.idx * FT_IN_SLOT + (uint32_t)i * 256u);
-                uint32_t hb[RPW / 2], lb[RPW / 2];
-#pragma unroll
-                for (int i = 0; i < RPW / 2; ++i) {
-                    const __nv_bfloat162 hi = __floats2bfloat162_rn(v[i].x, v[i].y);
-                    hb[i] = *reinterpret_cast<const uint32_t*>(&hi);
-                    const __nv_bfloat162 lo = __floats2bfloat162_rn(v[i].x - __uint_as_float(hb[i] << 16),
-                                                                     v[i].y - __uint_as_float(hb[i] & 0xffff0000u));
-                    lb[i] = *reinterpret_cast<const uint32_t*>(&lo);
+                for (int c = 0; c < 8; ++c) {
+                    const float4 v = lds128f(in_lane + in.idx * FT_IN_SLOT + ((((uint32_t)c) ^ sw) << 4));
+                    const __nv_bfloat162 h0 = __floats2bfloat162_rn(v.x, v.y), h1 = __floats2bfloat162_rn(v.z, v.w);
+                    hb[2 * c] = *reinterpret_cast<const uint32_t*>(&h0);
+                    hb[2 * c + 1] = *reinterpret_cast<const uint32_t*>(&h1);
+                    const __nv_bfloat162 l0 = __floats2bfloat162_rn(v.x - __uint_as_float(hb[2 * c] << 16),
+                                                                     v.y - __uint_as_float(hb[2 * c] & 0xffff0000u));
+                    const __nv_bfloat162 l1 = __floats2bfloat162_rn(v.z - __uint_as_float(hb[2 * c + 1] << 16),
+                                                                     v.w - __uint_as_float(hb[2 * c + 1] & 0xffff0000u));
+                    lb[2 * c] = *reinterpret_cast<const uint32_t*>(&l0);
+                    lb[2 * c + 1] = *reinterpret_cast<const uint32_t*>(&l1);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->in_empty[in.idx]));
                 in.advance(n_in);
                 pp_x = FT_NOW(); mbar_wait(smem_u32(&ctl->a_empty[a.idx]), a.phase ^ 1); pp_a += FT_NOW() - pp_x;
-                if (!FT_DBG(1024))
-#pragma unroll
-                for (int i = 0; i < RPW / 2; ++i) {
-                    // row r = 32 pwl + 2 i + hl: swizzle phase (r >> 1) & 3 = i & 3
-                    const uint32_t addr = a_lane + a.idx * FT_A_SLOT + (uint32_t)i * 128u + ((wc ^ ((uint32_t)i & 3u)) << 4);
-                    sts32(addr, hb[i]);
-                    sts32(addr + FT_A_TILE, lb[i]);
+                tc_fence_after();
+                if (!FT_DBG(1024)) {
+                    tmem_st16(a_t + a.idx * (2 * FT_A_COLS), hb);
+                    tmem_st16(a_t + a.idx * (2 * FT_A_COLS) + FT_A_COLS, lb);
+                    tmem_st_wait();
                 }
-                fence_proxy_async();
+                tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&ctl->a_full[a.idx]));
                 a.advance(n_a);
@@ -389,16 +395,14 @@ bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, i
     const size_t fixed = 2 * (size_t)prm.b_part_bytes + 4 * FT_STAGE + sizeof(FirtCtl);
     // Ring depths are EVEN: the two producer groups take alternate chunks, and a slot shared by both groups would let a
     // group test the parity of a barrier that is a whole phase behind (measured: a rare deadlock with a 3-slot ring).
-    prm.a_slots = 4; prm.in_slots = 4;
-    if (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) prm.a_slots = 2;
-    if (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) prm.in_slots = 2;
-    if (fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT > 232448) return false;
+    prm.in_slots = 8;
+    while (prm.in_slots > 2 && fixed + (size_t)prm.in_slots * FT_IN_SLOT > 232448) prm.in_slots -= 2;
+    if (fixed + (size_t)prm.in_slots * FT_IN_SLOT > 232448) return false;
 #ifdef TINA_DEV
-    if (options().a_slots) prm.a_slots = options().a_slots;
     if (options().b_entries) prm.in_slots = options().b_entries;
     prm.debug = options().debug_skip;
 #endif
-    const size_t smem = fixed + (size_t)prm.a_slots * FT_A_SLOT + (size_t)prm.in_slots * FT_IN_SLOT;
+    const size_t smem = fixed + (size_t)prm.in_slots * FT_IN_SLOT;
 
     EncodeTiledFn enc = encode_fn();
     if (!enc) { *status = fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found"); return true; }
@@ -410,7 +414,7 @@ bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, i
         const cuuint64_t strides[2] = {(cuuint64_t)FT_T * sizeof(float), (cuuint64_t)L * sizeof(float)};
         const cuuint32_t box[3] = {FT_KC, BM, 1};
         CUresult r = enc(&tmap_x, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(x), dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) { *status = fail(TINA_ERR_CUDA, "cuTensorMapEncodeTiled(fir input) failed (%d)", (int)r); return true; }
     }
