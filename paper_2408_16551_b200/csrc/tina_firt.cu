@@ -206,7 +206,10 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
             uint32_t br_phase = 0;
             long long pm_a = 0, pm_t = 0, pm_x, pm_tot = FT_NOW();
             const uint32_t idesc = idesc_bf16(BM * CG, FT_T, false);
-            const uint32_t b_s = smem_u32(b_res);
+            // descriptors of the resident band matrix, chunk 0 (the 14-bit address field takes the per-chunk offset
+            // by plain addition: all of shared memory is below 2^18 bytes)
+            const uint64_t b_hi0 = smem_desc_sw64(smem_u32(b_res)), b_lo0 = smem_desc_sw64(smem_u32(b_res) + b_part);
+            const uint32_t a_t0 = tmem_base + FT_A_COL0;
             for (int w = w_begin; w < w_end; ++w) {
                 if (new_channel(w)) {
                     // every MMA issued so far has read the old matrix: release it once they are done, then wait
@@ -223,11 +226,13 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                 for (int kc = 0; kc < n_kc; ++kc) {
                     pm_x = FT_NOW(); mbar_wait(smem_u32(&ctl->a_full[a.idx]), a.phase); pm_a += FT_NOW() - pm_x;
                     tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t a_hi = tmem_base + FT_A_COL0 + a.idx * (2 * FT_A_COLS), a_lo = a_hi + FT_A_COLS;
-                        const uint32_t b_off = (uint32_t)(n_kc - 1 - kc) * (FT_KC * 64u);     // 32 rows of 64 B per chunk step
-                        const uint64_t b_hi = smem_desc_sw64(b_s + b_off);
-                        const uint64_t b_lo = smem_desc_sw64(b_s + b_off + b_part);
+                    // one ELECTED thread issues (the compiler then knows a single thread is active and emits the
+                    // tcgen05 instructions straight; under `lane == 0` it wraps each in an any-thread loop, and the
+                    // issuing thread, not the tensor pipe, bounded the kernel: ~150 cycles per instruction against 64)
+                    if (elect_one()) {
+                        const uint32_t a_hi = a_t0 + a.idx * (2 * FT_A_COLS), a_lo = a_hi + FT_A_COLS;
+                        const uint64_t b_step = (uint64_t)((uint32_t)(n_kc - 1 - kc) * (FT_KC * 64u) >> 4);     // 32 rows of 64 B per chunk step
+                        const uint64_t b_hi = b_hi0 + b_step, b_lo = b_lo0 + b_step;
                         uint32_t acc = kc > 0;
                         if (!FT_DBG(512)) {
 #pragma unroll
@@ -294,8 +299,18 @@ fir_umma_kernel(const __grid_constant__ CUtensorMap tmap_x, const FirtParams prm
                 if (lane < head) g[lane] = at(lane);
                 // (an aligned-float4 variant -- two ld.shared.v4 of the staged row and a funnel shift by `head` instead of
                 // four scalar loads -- was measured slower: 0.177 against 0.137 ms; the scalar form stays)
-                for (int v = lane; v < nv4; v += 32) {
-                    const int l = head + 4 * v;
+                // float4 number v = 32 it + j covers elements head + 128 it + 4 j .. + 3: row `it` of the staged tile for
+                // j < 31, but the last one of each row straddles rows it and it + 1 when head > 0 -- its bank would collide
+                // with lane 0's (a 2-way conflict on every load), so lane 31 sits out and the 31 seams go out afterwards,
+                // seam `it` by lane `it` (banks it + 31 and it + 1: conflict-free)
+                if (head == 0 || lane < 31) {
+                    for (int v = lane; v < nv4; v += 32) {
+                        const int l = head + 4 * v;
+                        *reinterpret_cast<float4*>(g + l) = make_float4(at(l), at(l + 1), at(l + 2), at(l + 3));
+                    }
+                }
+                if (head != 0 && 32 * lane + 31 < nv4) {
+                    const int l = head + 4 * (32 * lane + 31);
                     *reinterpret_cast<float4*>(g + l) = make_float4(at(l), at(l + 1), at(l + 2), at(l + 3));
                 }
                 const int tail0 = head + 4 * nv4;
@@ -395,7 +410,9 @@ bool firt_fir(const float* x, const float* taps, float* y, int C, long long L, i
     const size_t fixed = 2 * (size_t)prm.b_part_bytes + 4 * FT_STAGE + sizeof(FirtCtl);
     // Ring depths are EVEN: the two producer groups take alternate chunks, and a slot shared by both groups would let a
     // group test the parity of a barrier that is a whole phase behind (measured: a rare deadlock with a 3-slot ring).
-    prm.in_slots = 8;
+    // Six slots of read-ahead (96 KB per SM), measured on c3: 2 -> 0.135 ms, 4 -> 0.107, 6 -> 0.1005, 8 -> 0.1095 (deeper
+    // read-ahead lets the loads crowd the stores out at the memory controllers)
+    prm.in_slots = 6;
     while (prm.in_slots > 2 && fixed + (size_t)prm.in_slots * FT_IN_SLOT > 232448) prm.in_slots -= 2;
     if (fixed + (size_t)prm.in_slots * FT_IN_SLOT > 232448) return false;
 #ifdef TINA_DEV
