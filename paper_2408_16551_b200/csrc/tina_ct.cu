@@ -186,7 +186,7 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         fence_proxy_async();
         __syncthreads();
         // ---- stage 1: D1 = A1 * W32  (tile t -> TMEM columns 64 t .. 64 t + 63)
-        if (tid == 0) {
+        if (warp == 0 && elect_one()) {
             tc_fence_after();
 #pragma unroll
             for (int t = 0; t < CT_NT; ++t) {
@@ -222,7 +222,7 @@ pfb_ct_kernel(const float2* __restrict__ x, long long stream_stride, const float
         tc_fence_before();
         __syncthreads();
         // ---- stage 2: D2 = A2 * W32  (over D1: every warp has read its part)
-        if (tid == 0) {
+        if (warp == 0 && elect_one()) {
             tc_fence_after();
 #pragma unroll
             for (int t = 0; t < CT_NT; ++t) {
@@ -442,7 +442,7 @@ pfb_ctws_kernel(const float2* __restrict__ x, long long stream_stride, const flo
     } else {
         // ================================================================== MMA issuer (warp 16; warps 17-19 idle)
         setmaxnreg_dec<32>();
-        if (warp == 16 && lane == 0) {
+        if (warp == 16 && elect_one()) {
             const uint32_t idesc = idesc_bf16(128, 64);
             const uint64_t d_bh = smem_desc_sw128(smem_u32(sm.bm)), d_bl = smem_desc_sw128(smem_u32(sm.bm + 8192));
             constexpr uint64_t TILE_DESC = (uint64_t)(2 * CT_TILE) >> 4, PART_DESC = (uint64_t)CT_TILE >> 4;

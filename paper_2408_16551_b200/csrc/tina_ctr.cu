@@ -225,7 +225,7 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
         // stage-1 MMAs of tile 1 execute, epilogue 1 of tile 1 while the stage-2 MMAs of tile 0 execute, epilogue 2 of
         // tile 0 while the stage-2 MMAs of tile 1 execute; only the stage-1 MMAs of tile 0 are waited for in full.
         // ---- stage 1 (transposed): D1^T[t] = B1 * A1[t]^T -> TMEM columns 128 t .. 128 t + 127 = (frame, a)
-        if (tid == 0) {
+        if (warp == 0 && elect_one()) {
             tc_fence_after();
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
@@ -282,7 +282,7 @@ pfb_ctr_kernel(const float* __restrict__ x, long long stream_stride, const float
             tc_fence_before();
             __syncthreads();
             // ---- stage 2 of tile t: D_R = Re(G') * B1[0..63]^T -> columns 128 t .. + 63,  D_I = Im(G') * B1[0..63]^T -> + 64 .. + 127
-            if (tid == 0) {
+            if (warp == 0 && elect_one()) {
                 tc_fence_after();
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
@@ -584,7 +584,7 @@ pfb_ctrws_kernel(const float* __restrict__ x, long long stream_stride, const flo
     } else {
         // ================================================================== MMA issuer (warp 16; warps 17-19 idle)
         cw_reg_dec<40>();
-        if (warp == 16 && lane == 0) {
+        if (warp == 16 && elect_one()) {
             const uint32_t idesc1 = idesc_bf16(128, 128), idesc2 = idesc_bf16(128, 64);
             const uint64_t d_bh = smem_desc_sw128(smem_u32(sm.bm[0])), d_bl = smem_desc_sw128(smem_u32(sm.bm[1]));
             const uint64_t d_a1 = smem_desc_sw128(smem_u32(&sm.a1[0][0][0])), d_a2 = smem_desc_sw128(smem_u32(&sm.a2[0][0][0]));

@@ -766,7 +766,7 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                         uint32_t bi = e_i % ST_B_ENTRIES, bp = (e_i / ST_B_ENTRIES) & 1u;
                         pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); pm_b += SY_NOW() - pm_x;
                         tc_fence_after();
-                        if (lane == 0) {
+                        if (elect_one()) {
                             const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + bi * ST_B_ENTRY));
                             uint32_t acc = kc > kc_begin;
                             if (parts > 1) {
@@ -784,7 +784,7 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             e_i += EO; bi = e_i % ST_B_ENTRIES; bp = (e_i / ST_B_ENTRIES) & 1u;
                             pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); pm_b += SY_NOW() - pm_x;
                             tc_fence_after();
-                            if (lane == 0) {
+                            if (elect_one()) {
                                 const uint64_t bd = smem_desc_sw64(smem_u32(b_ring + bi * ST_B_ENTRY));
                                 const uint64_t ad = smem_desc_mn_sw128(a_hi, ST_A_LBO, ST_A_SBO);
 #pragma unroll
@@ -794,7 +794,7 @@ pfb_symt_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                             __syncwarp();
                         }
                         be += EPC;
-                        if (lane == 0) {
+                        if (elect_one()) {
                             commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
                             if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[h]), pair_mask);
                         }
