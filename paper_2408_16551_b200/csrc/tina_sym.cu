@@ -449,6 +449,7 @@ __device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, cons
     const uint32_t full_row = (odd ? b_mo : b_fe) + rr * 128u;
     const uint32_t part_row = (odd ? b_f28 : b_m28) + rr * 112u;
     uint32_t tf_phase = 0;
+    const bool issuer = elect_one();                          // see sym_epilogue: one elected thread issues and waits
     const bool keep_l2 = prm.k_splits > 1;
     const uint64_t pol_keep = l2_policy_evict_last();
     long long pe_w = 0, pe_d = 0, pe_d0 = 0, pe_x, pe_tot = SY_NOW();
@@ -465,7 +466,7 @@ __device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, cons
         // one) stores everything from registers
         const bool lone = (prm.F & 1) && row0 + lane == prm.F - 1;
         for (int ks = 0; ks < prm.k_splits; ++ks) {
-            if (ks > 0 && lane == 0) bulk_wait<0>();          // the previous chain's stores to this tile are complete
+            if (ks > 0 && issuer) bulk_wait<0>();          // the previous chain's stores to this tile are complete
             pe_x = SY_NOW();
             mbar_wait<256>(e.t_full0, tf_phase);
             mbar_wait<256>(e.t_full1, tf_phase);
@@ -482,7 +483,7 @@ __device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, cons
                 const int kb = k0 + (cb >> 1);
                 const bool last = cb + 32 >= ncol;
                 const int f_col = 2 * kb, m_col = P - 2 * kb - 30;      // first float of the forward / mirrored tile in a row
-                if (lane == 0) bulk_wait_read<0>();               // the staged tiles of the previous step have been read
+                if (issuer) bulk_wait_read<0>();                // the staged tiles of the previous step have been read
                 __syncwarp();
                 float e0x = 0.f, e0y = 0.f, e7x = 0.f, e7y = 0.f;   // the part tile's edge pairs (floats 0-1 and 30-31)
 #pragma unroll
@@ -551,7 +552,7 @@ __device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, cons
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) {
+                if (issuer) {
                     // paired-row coordinates: an odd row starts at float P + 2 of its pair
                     if (SY_DBG(16)) { }
                     else if (ks == 0 && keep_l2) {                // a later chain adds into this tile: keep it in L2
@@ -575,7 +576,7 @@ __device__ __forceinline__ void sym_epilogue_real_tma(const SymParams& prm, cons
             }
         }
     }
-    if (lane == 0) bulk_wait<0>();                            // staging tiles must outlive their TMA reads
+    if (issuer) bulk_wait<0>();                               // staging tiles must outlive their TMA reads
     if (SY_PROF && prm.prof && q == 0 && lane == 0) {
         unsigned long long* pp = prm.prof + blockIdx.x * 16 + 8;
         pp[0] = SY_NOW() - pe_tot; pp[1] = pe_w; pp[2] = pe_d; pp[3] = pe_d0;

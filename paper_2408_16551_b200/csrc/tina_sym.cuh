@@ -99,6 +99,10 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
     const uint32_t taddr = e.tmem_base + ((uint32_t)(q * 32) << 16);
     const uint32_t rowoff = (uint32_t)lane * 128u, sw = (uint32_t)lane & 7u;
     uint32_t tf_phase = 0;
+    // ONE elected thread per warp issues every TMA store and waits on their bulk groups (the groups belong to the thread
+    // that committed them).  Elected rather than `lane == 0`: ptxas then knows a single thread is active and emits the
+    // uniform-datapath instructions straight instead of inside an any-thread loop.
+    const bool issuer = elect_one();
     // several accumulation chains (P > 1024): the first chain's tiles are stored with an L2 evict-last policy so that
     // the later chains' add-reduce finds them resident
     const bool keep_l2 = prm.k_splits > 1;
@@ -113,7 +117,7 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
         const bool row_ok = lane < (int)min(32LL, prm.F - row0);
         float* const orow = prm.out + ((long long)s * prm.F + row0 + lane) * (2LL * P);
         for (int ks = 0; ks < prm.k_splits; ++ks) {
-            if (ks > 0 && lane == 0) bulk_wait<0>();          // the previous chain's stores to this tile are complete
+            if (ks > 0 && issuer) bulk_wait<0>();          // the previous chain's stores to this tile are complete
             pe_x = SY_NOW();
             mbar_wait<256>(e.t_full0, tf_phase);
             mbar_wait<256>(e.t_full1, tf_phase);
@@ -171,7 +175,7 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
                     put(P - kb, SY_F(r1[0]) - SY_F(r2[1]), SY_F(r2[0]) + SY_F(r1[1]));          // mirror of j = 0
                 }
                 if (last) put(P - kb - 15, SY_F(r1[30]) - SY_F(r2[31]), SY_F(r2[30]) + SY_F(r1[31]));   // mirror of j = 15
-                if (lane == 0) bulk_wait_read<1>();           // the forward tile of the previous step has been read
+                if (issuer) bulk_wait_read<1>();           // the forward tile of the previous step has been read
                 __syncwarp();
 #pragma unroll
                 for (int g = 0; g < 8; ++g) {
@@ -182,7 +186,7 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) {
+                if (issuer) {
                     if (SY_DBG(32)) { }
                     else if (ks == 0 && keep_l2) tma_store_3d_hint(tmap_out, sb_f, 2 * kb, (int)row0, s, pol_keep);
                     else if (ks == 0) tma_store_3d(tmap_out, sb_f, 2 * kb, (int)row0, s);
@@ -213,7 +217,7 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) {
+                if (issuer) {
                     if (SY_DBG(16)) { }
                     else if (!last) {
                         const int cm = 2 * (P - kb - 16);
@@ -231,7 +235,7 @@ __device__ __forceinline__ void sym_epilogue(const SymParams& prm, const CUtenso
             }
         }
     }
-    if (lane == 0) bulk_wait<0>();                            // staging tiles must outlive their TMA reads
+    if (issuer) bulk_wait<0>();                               // staging tiles must outlive their TMA reads
     if (SY_PROF && prm.prof && q == 0 && lane == 0) {
         unsigned long long* pp = prm.prof + blockIdx.x * 16 + 8;
         pp[0] = SY_NOW() - pe_tot; pp[1] = pe_w; pp[2] = pe_d;
