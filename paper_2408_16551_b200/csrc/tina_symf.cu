@@ -274,7 +274,7 @@ pfb_symf_kernel(const __grid_constant__ FoldMaps maps, const SymParams prm, cons
                         auto with_entry = [&](auto&& issue) {
                             mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase);
                             tc_fence_after();
-                            if (lane == 0) {
+                            if (elect_one()) {
                                 issue(smem_u32(b_ring + b.idx * SF_B_ENTRY));
                                 commit_cg<CG>(smem_u32(&ctl->b_empty[b.idx]), pair_mask);
                             }
@@ -315,7 +315,7 @@ pfb_symf_kernel(const __grid_constant__ FoldMaps maps, const SymParams prm, cons
                             with_entry([&](uint32_t bt) { umma_bf16<CG>(d_sin, a_mh, smem_desc_sw32(bt), idesc_n, 1); });   // S_lo
                             if (kc == 0) with_entry([&](uint32_t bt) { umma_bf16<CG>(d_cos, a_mh, smem_desc_sw32(bt), idesc_n, 1); });   // Csp_lo
                         }
-                        if (lane == 0) {
+                        if (elect_one()) {
                             commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
                             if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[h]), pair_mask);
                         }
