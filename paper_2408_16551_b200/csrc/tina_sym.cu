@@ -183,7 +183,7 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
                         // ---- B_hi: (A_lo x B_hi) then (A_hi x B_hi)
                         pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
                         tc_fence_after();
-                        if (lane == 0) {
+                        if (elect_one()) {
                             const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * SY_B_ENTRY));
                             uint32_t acc = kc > kc_begin;
                             if (parts > 1) {
@@ -202,7 +202,7 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
                         if (parts > 1) {
                             pm_x = SY_NOW(); mbar_wait(smem_u32(&ctl->b_full[b.idx]), b.phase); pm_b += SY_NOW() - pm_x;
                             tc_fence_after();
-                            if (lane == 0) {
+                            if (elect_one()) {
                                 const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + b.idx * SY_B_ENTRY));
                                 const uint64_t ad = smem_desc_sw128(a_hi);
 #pragma unroll
@@ -212,7 +212,7 @@ pfb_sym_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant
                             __syncwarp();
                             b.advance(SY_B_ENTRIES);
                         }
-                        if (lane == 0) {
+                        if (elect_one()) {
                             commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), pair_mask);
                             if (kc == kc_end - 1) commit_cg<CG>(smem_u32(&ctl->t_full[h]), pair_mask);
                         }

@@ -370,7 +370,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     uint32_t bi = e % N_B, bp = (e / N_B) & 1u;
                     PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); PF_END(pf_b);
                     tc_fence_after();
-                    if (lane == 0) {
+                    if (elect_one()) {
                         const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + bi * B_ENTRY));
                         uint32_t acc = kc > kc_begin;
                         if (TINA_DBG(4)) { } else
@@ -391,7 +391,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                         ++e; bi = e % N_B; bp = (e / N_B) & 1u;
                         PF_BEGIN(); mbar_wait(smem_u32(&ctl->b_full[bi]), bp); PF_END(pf_b);
                         tc_fence_after();
-                        if (lane == 0) {
+                        if (elect_one()) {
                             const uint64_t bd = smem_desc_sw128(smem_u32(b_ring + bi * B_ENTRY));
                             const uint64_t ad = smem_desc_sw128(a_hi);
                             if (!TINA_DBG(4))
@@ -403,7 +403,7 @@ pfb_umma_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constan
                     }
                 }
                 g += (uint32_t)(n_sub * parts);
-                if (lane == 0) {
+                if (elect_one()) {
                     commit_cg<CG>(smem_u32(&ctl->a_empty[a.idx]), SHARE ? (uint16_t)0xF : pair_mask);
                     // one "accumulator ready" barrier per 256-column TMEM block: the two halves finish (and are
                     // drained) independently, so one half's drain overlaps the other half's MMAs
