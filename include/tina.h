@@ -64,8 +64,9 @@ typedef enum {
  * Supported: C >= 1, 1 <= M <= 4096, L >= M.  Even L with M <= 193 runs as a banded-Toeplitz
  * contraction on the tensor cores (blocks of 128 outputs, bf16x3 error-compensated, rel. L2 per
  * channel <= 1e-5, the unfolding view of Eq. (17)-(19)) -- with L % 128 == 0 on
- * the kernel that keeps the Toeplitz band matrix resident in shared memory and stages the signal by
- * TMA; any other shape on the CUDA-core register-window kernel (fp32 FMA).  Errors: NULL_POINTER, BAD_SHAPE, UNSUPPORTED
+ * the kernel that keeps the Toeplitz band matrix resident in shared memory, stages the signal by
+ * TMA and holds the signal operand in tensor memory; any other shape on the CUDA-core
+ * register-window kernel (fp32 FMA).  Errors: NULL_POINTER, BAD_SHAPE, UNSUPPORTED
  * (M > 4096), ALIGNMENT (x, y not 16-byte aligned), CUDA.                                          */
 tina_status tina_fir(const float* x, const float* taps, float* y,
                      int C, long long L, int M, void* stream);

@@ -99,7 +99,7 @@ def test_fir_toeplitz_tensor_path(tina, oracle, C, L, K):
 @pytest.mark.parametrize("per_channel", [False, True])
 def test_fir_resident_toeplitz_kernel(tina, oracle, C, L, K, per_channel):
     """L % 128 == 0 and K <= 193: fir_umma_kernel (Toeplitz matrix resident in shared memory, signal staged by TMA,
-    four accumulator stages).  Single block, one tap, the largest K, ragged last tile, more channels than CTA pairs
+    operand in tensor memory, three accumulator stages).  Single block, one tap, the largest K, ragged last tile, more channels than CTA pairs
     (per-channel taps rebuild the matrix at every channel change); asymmetric random taps."""
     import torch
     rng = np.random.default_rng(190 + C + K)
@@ -387,6 +387,27 @@ def test_pfb_repeated_launches_bit_identical(tina, P, M, S, F, real):
         if it % 50 == 49:
             torch.cuda.synchronize()
             assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref)), it
+
+
+@pytest.mark.parametrize("C,L,K,per_channel", [(64, 128 * 1024, 64, False), (70, 128 * 130, 33, True), (3, 128 * 2049, 193, False)])
+def test_fir_repeated_launches_bit_identical(tina, C, L, K, per_channel):
+    """300 back-to-back launches of fir_umma_kernel on the same buffers give bit-identical results: its operand slots in
+    tensor memory (tcgen05.st by the producers, read by tcgen05.mma), the two producer groups on alternate chunks, the
+    three accumulator stages and the per-channel rebuild of the resident band matrix are deterministic; a race would
+    show up as a differing launch."""
+    import torch
+    g = torch.Generator(device="cuda").manual_seed(C + K)
+    x = torch.randn(C, L, device="cuda", generator=g)
+    a = torch.randn((C, K) if per_channel else (K,), device="cuda", generator=g)
+    run = tina.fir_multi if per_channel else tina.fir
+    out = run(x, a); torch.cuda.synchronize()
+    assert tina.last_kernel().startswith("fir_umma_kernel")
+    ref = out.clone()
+    for it in range(300):
+        out = run(x, a, out=out)
+        if it % 50 == 49:
+            torch.cuda.synchronize()
+            assert torch.equal(out, ref), it
 
 
 def test_pfb_complex_multichain_batched(tina, oracle):
