@@ -77,7 +77,9 @@ peak_umma_kernel(int iters, int n_cols)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    if (threadIdx.x == 0) {
+    // one ELECTED thread issues (under `threadIdx.x == 0` ptxas wraps every tcgen05.mma in an any-thread loop, and the
+    // narrow-tile figures then measure the issuing thread instead of the tensor pipe)
+    if (threadIdx.x < 32 && elect_one()) {
         const uint64_t ad = smem_desc_sw128(smem_u32(a_tile)), bd = smem_desc_sw128(smem_u32(b_tile));
         // kind::tf32: a/b format 2; kind::f16 with bf16: format 1; fp32 accumulate; M = 128, N = 256
         const uint32_t fmt = TF32 ? 2u : 1u;
