@@ -78,11 +78,14 @@ def _check(st: int) -> None:
         raise TinaError(st, L.tina_status_string(st).decode(), L.tina_last_error().decode())
 
 
-def _stream_ptr(stream) -> int:
+def _stream_ptr(stream, device=None) -> int:
+    """Raw CUDA stream handle: `stream` (a torch.cuda.Stream), else torch's current stream on `device` (a torch.device
+    of the call's tensors; the current device when None)."""
     import torch
     if stream is None:
         try:        # raw handle of torch's current stream without building a Stream object (a few microseconds per call)
-            return int(torch._C._cuda_getCurrentRawStream(torch.cuda.current_device()))
+            idx = device.index if (device is not None and device.index is not None) else torch.cuda.current_device()
+            return int(torch._C._cuda_getCurrentRawStream(idx))
         except AttributeError:
             stream = torch.cuda.current_stream()
     return int(stream.cuda_stream)
@@ -172,7 +175,7 @@ def fir(x, taps, out=None, stream=None):
     C, L = x.shape
     M = taps.shape[0]
     out = _out(out, (C, max(L - M + 1, 0)), torch.float32, x.device)
-    _check(lib().tina_fir(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream)))
+    _check(lib().tina_fir(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream, x.device)))
     return out
 
 
@@ -187,7 +190,7 @@ def fir_multi(x, taps, out=None, stream=None):
     C, L = x.shape
     M = taps.shape[1]
     out = _out(out, (C, max(L - M + 1, 0)), torch.float32, x.device)
-    _check(lib().tina_fir_multi(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream)))
+    _check(lib().tina_fir_multi(x.data_ptr(), taps.data_ptr(), out.data_ptr(), C, L, M, _stream_ptr(stream, x.device)))
     return out
 
 
@@ -276,15 +279,20 @@ def dft(x, inverse: bool = False, prec: int = PREC_FP32, out=None, stream=None):
         raise ValueError("x must be [B, N]")
     B, N = x.shape
     out = _out(out, x.shape, torch.complex64, x.device)
-    _check(lib().tina_dft(x.data_ptr(), out.data_ptr(), B, N, int(bool(inverse)), prec, _stream_ptr(stream)))
+    _check(lib().tina_dft(x.data_ptr(), out.data_ptr(), B, N, int(bool(inverse)), prec, _stream_ptr(stream, x.device)))
     return out
 
 
 def _pfb_args(x, P, M, window):
+    """Checks of a PFB call's inputs WITHOUT building tensor views (a view costs more than the launch of a small
+    problem): returns kind, S, n_samples, F and whether x was one-dimensional."""
     import torch
-    if x.dim() == 1:
-        x = x[None, :]
-    if x.dim() != 2:
+    nd = x.dim()
+    if nd == 1:
+        S, n = 1, x.shape[0]
+    elif nd == 2:
+        S, n = x.shape
+    else:
         raise ValueError("x must be [n_samples] or [S, n_samples]")
     if x.dtype == torch.complex64:
         kind = COMPLEX
@@ -292,55 +300,61 @@ def _pfb_args(x, P, M, window):
         kind = REAL
     else:
         raise TypeError("x must be complex64 (complex kind) or float32 (real kind)")
-    _dev(x, x.dtype, "x")
-    _dev(window, torch.float32, "window")
+    if not (x.is_cuda and x.is_contiguous()):
+        _dev(x, x.dtype, "x")                                  # raises with the reason
+    if not (window.is_cuda and window.dtype == torch.float32 and window.is_contiguous()):
+        _dev(window, torch.float32, "window")
     if window.numel() != P * M:
         raise ValueError("window must have P*M entries")
-    S, n = x.shape
-    F = pfb_num_frames(n, P, M)
-    return x, kind, S, n, F
+    F = n // P - M + 1 if (P >= 1 and M >= 1) else 0         # tina_pfb_num_frames (include/tina.h)
+    return kind, S, n, F, nd == 1
+
+
+def _pfb_out(out, squeeze, S, F, last, dtype, device):
+    """The result buffer of a PFB call: [S, F, last], or [F, last] for a one-dimensional x (a caller-supplied buffer
+    of either form is accepted then).  Returns (buffer whose data_ptr is passed, tensor handed back to the caller)."""
+    import torch
+    F = max(F, 0)
+    if out is None:
+        out = torch.empty((F, last) if squeeze else (S, F, last), dtype=dtype, device=device)
+        return out, out
+    if squeeze and out.dim() == 3:
+        _out(out, (1, F, last), dtype, device)
+        return out, out[0]
+    shape = (F, last) if squeeze else (S, F, last)
+    if not (out.is_cuda and out.dtype == dtype and out.shape == shape and out.device == device and out.is_contiguous()):
+        _out(out, shape, dtype, device)                        # raises with the reason
+    return out, out
 
 
 def pfb(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=None):
     """tina_pfb_batched: x [S, n_samples] (or [n_samples]) complex64 | float32 CUDA,
     window [P*M] float32 CUDA -> [S, F, P] (complex kind) or [S, F, P/2+1] (real kind) complex64."""
     import torch
-    squeeze = x.dim() == 1
-    x, kind, S, n, F = _pfb_args(x, P, M, window)
-    if squeeze and out is not None and out.dim() == 2:
-        out = out[None]
-    NK = P if kind == COMPLEX else P // 2 + 1
-    out = _out(out, (S, max(F, 0), NK), torch.complex64, x.device)
+    kind, S, n, F, squeeze = _pfb_args(x, P, M, window)
+    buf, res = _pfb_out(out, squeeze, S, F, P if kind == COMPLEX else P // 2 + 1, torch.complex64, x.device)
     _check(lib().tina_pfb_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind, prec,
-                                  out.data_ptr(), _stream_ptr(stream)))
-    return out[0] if squeeze else out
+                                  buf.data_ptr(), _stream_ptr(stream, x.device)))
+    return res
 
 
 def pfb_fft(x, P: int, M: int, window, out=None, stream=None):
     """tina_pfb_fft_batched: PFB with the factorised Fourier stage (complex P=1024 or real P=4096); same result as pfb()."""
     import torch
-    squeeze = x.dim() == 1
-    x, kind, S, n, F = _pfb_args(x, P, M, window)
-    if squeeze and out is not None and out.dim() == 2:
-        out = out[None]
-    NK = P if kind == COMPLEX else P // 2 + 1
-    out = _out(out, (S, max(F, 0), NK), torch.complex64, x.device)
+    kind, S, n, F, squeeze = _pfb_args(x, P, M, window)
+    buf, res = _pfb_out(out, squeeze, S, F, P if kind == COMPLEX else P // 2 + 1, torch.complex64, x.device)
     _check(lib().tina_pfb_fft_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind,
-                                      out.data_ptr(), _stream_ptr(stream)))
-    return out[0] if squeeze else out
+                                      buf.data_ptr(), _stream_ptr(stream, x.device)))
+    return res
 
 
 def pfb_fir(x, P: int, M: int, window, out=None, stream=None):
     """tina_pfb_fir_batched: subfilter stage only -> y [S, F, P] (dtype of x)."""
-    import torch
-    squeeze = x.dim() == 1
-    x, kind, S, n, F = _pfb_args(x, P, M, window)
-    if squeeze and out is not None and out.dim() == 2:
-        out = out[None]
-    out = _out(out, (S, max(F, 0), P), x.dtype, x.device)
+    kind, S, n, F, squeeze = _pfb_args(x, P, M, window)
+    buf, res = _pfb_out(out, squeeze, S, F, P, x.dtype, x.device)
     _check(lib().tina_pfb_fir_batched(x.data_ptr(), S, n, P, M, window.data_ptr(), kind,
-                                      out.data_ptr(), _stream_ptr(stream)))
-    return out[0] if squeeze else out
+                                      buf.data_ptr(), _stream_ptr(stream, x.device)))
+    return res
 
 
 def pfb_host(x, P: int, M: int, window, prec: int = PREC_FP32, out=None, stream=None):
