@@ -74,6 +74,12 @@ def workload_spec(name: str):
     raise SystemExit(f"unknown workload {name}")
 
 
+def roof_floors(issued_flops, algorithmic_bytes, tensor_tflops, hbm_gbs):
+    """Time floors (seconds) of one step under the two roofs: issued tensor flops at `tensor_tflops`, algorithmic bytes
+    at `hbm_gbs`.  The larger one is the roof that binds."""
+    return issued_flops / (tensor_tflops * 1e12), algorithmic_bytes / (hbm_gbs * 1e9)
+
+
 def useful_flops_and_bytes(w):
     """Algorithmic flops (DFT contraction, the dominant kernel's tensor work) and HBM bytes
     per step -- SURVEY.md section 8(d) / DESIGN.md "Algorithmic work"."""
@@ -498,8 +504,7 @@ def run_ours(args, w):
         # at the measured copy bandwidth).  A dense contraction whose arithmetic intensity is below the machine balance
         # (c2: N = 256, 8 N^2 flops x 1.5 issued per 16 N bytes = 192 flop/B against 1662 / 6.55 = 254) sits on the
         # memory side of the ridge: its line reports the HBM fraction as `frac` and keeps the tensor figures beside it.
-        t_tensor = flops * ratio / (pk_b * 1e12)
-        t_hbm = byts / (peaks["hbm_gbs"] * 1e9)
+        t_tensor, t_hbm = roof_floors(flops * ratio, byts, pk_b, peaks["hbm_gbs"])
         roof["floor_ms"] = {"tensor_issued_burst": t_tensor * 1e3, "hbm": t_hbm * 1e3}
         if t_hbm > t_tensor:
             tensor_side = {k: roof[k] for k in ("achieved", "peak", "unit", "frac", "peak_source")}
